@@ -1,0 +1,142 @@
+/* arachne_attn.h — C ABI of libarachne_attn.so (B200 / sm_100a only).
+ *
+ * One operation: a DiT block's full 3D self-attention, forward and backward, over a PACKED
+ * batch of heterogeneous-length video-latent token sequences (block-diagonal: a token
+ * attends only to tokens of its own sequence), with QK-RMSNorm and 3D (t,h,w) RoPE applied
+ * to Q and K on the way in.
+ *
+ * Where the operation is defined.  The paper (Arachne, arxiv 2607.01701; PAPER.md) only
+ * NAMES it: "the DiT architecture's full self-attention over a unified sequence of 3D
+ * patches of length L, which incurs quadratic (O(L^2)) complexity ... the dominant
+ * performance bottleneck" (§III Observation 2; the alpha2*B*S^2 term of
+ * Eq. 9).  It gives no formula for the attention itself.  The exact
+ * arithmetic is therefore fixed by BASELINE.json (north_star, configs[0]) and the readings
+ * R1-R18 listed in DESIGN.md §3; the defining equations are restated in DESIGN.md §2 and
+ * implemented, independently of this library, by oracle/arachne_oracle.c.
+ *
+ *   x^      = gamma * x / sqrt(mean_d(x_d^2) + eps)          (per token, per head; x = Q or K row)
+ *   x~      = RoPE3D(x^ ; pos(n))     pos(n) = (n / (Hg*Wg), (n / Wg) % Hg, n % Wg)
+ *   s_ij    = softmax_scale * <q~_i, k~_j>                    i, j in the same sequence
+ *   LSE_i   = ln sum_j exp(s_ij)      P_ij = exp(s_ij - LSE_i)      O_i = sum_j P_ij V_j
+ *   backward: given dO, gradients dQ, dK (w.r.t. the RAW Q, K, through RoPE and RMSNorm) and dV.
+ *
+ * Conventions common to every entry point
+ *   - All tensor pointers are DEVICE pointers unless the name ends in _host.
+ *   - q, k, v, o, d_o, dq, dk, dv : bf16, logical shape [N, H, D], contiguous (token-major;
+ *     element (n,h,d) at ((n*H)+h)*D+d).  N = total_tokens, H = num_heads, D = head_dim.
+ *   - lse : fp32 [H, N] (natural log).  gamma_q, gamma_k : fp32 [D] or NULL (= all ones).
+ *   - Pointers must be 16-byte aligned.  The caller owns every tensor and the workspace;
+ *     the library owns only the plan.  Nothing is allocated, freed or synchronised inside
+ *     fwd/bwd; all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*).
+ *   - Outputs are fully overwritten.  Rows of other sequences are never read or written
+ *     on behalf of a sequence (block-diagonal), including at ragged tile tails.
+ *   - Every function returns an arachne_status (0 = OK) and never throws or aborts.
+ *     Invalid arguments are rejected before any kernel is launched.
+ */
+#ifndef ARACHNE_ATTN_H_
+#define ARACHNE_ATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  ARACHNE_OK = 0,
+  ARACHNE_ERR_NULL_POINTER = 1,
+  ARACHNE_ERR_BAD_HEAD_DIM = 2,      /* head_dim not in {64, 128}                          */
+  ARACHNE_ERR_BAD_ROPE_DIMS = 3,     /* a rope dim is odd / negative, or they do not sum to D */
+  ARACHNE_ERR_BAD_CU_SEQLENS = 4,    /* cu_seqlens[0] != 0 or not strictly increasing       */
+  ARACHNE_ERR_GRID_MISMATCH = 5,     /* T*Hg*Wg != cu_seqlens[b+1]-cu_seqlens[b]            */
+  ARACHNE_ERR_TOTAL_TOKENS = 6,      /* cu_seqlens[B] != total_tokens                       */
+  ARACHNE_ERR_MISALIGNED = 7,        /* a tensor / workspace pointer is not 16-byte aligned */
+  ARACHNE_ERR_WORKSPACE_TOO_SMALL = 8,
+  ARACHNE_ERR_BAD_ARCH = 9,          /* current device is not compute capability 10.x       */
+  ARACHNE_ERR_CUDA = 10,             /* CUDA runtime error; text in arachne_last_error_message */
+  ARACHNE_ERR_BAD_SHAPE = 11,        /* num_seqs/num_heads/total_tokens <= 0, or too large  */
+  ARACHNE_ERR_BAD_PARAM = 12         /* non-finite / non-positive theta, eps < 0, bad flags */
+} arachne_status;
+
+enum {
+  ARACHNE_FLAG_DETERMINISTIC = 1,    /* bwd: bit-reproducible run to run (same device, plan) */
+  ARACHNE_FLAG_NO_NORM = 2,          /* debug: skip RMSNorm (x^ = x)                         */
+  ARACHNE_FLAG_NO_ROPE = 4           /* debug: skip RoPE (x~ = x^)                           */
+};
+
+/* Problem description.  Plain data, copied by arachne_plan_create. */
+typedef struct {
+  int32_t num_seqs;       /* B                                                            */
+  int32_t total_tokens;   /* N = sum_b L_b                                                */
+  int32_t num_heads;      /* H                                                            */
+  int32_t head_dim;       /* D in {64, 128}                                               */
+  int32_t rope_dims[3];   /* (d_t, d_h, d_w): each even and >= 0, sum == head_dim; axis a
+                             owns the contiguous slice of head_dim of width d_a, in this
+                             order; inside a slice, pair p is elements (2p, 2p+1)          */
+  float rope_theta;       /* angle = pos_a * theta^(-2p/d_a); 10000                        */
+  float rms_eps;          /* added to the mean square, inside the sqrt; 1e-6               */
+  float softmax_scale;    /* 0 => 1/sqrt(head_dim)                                         */
+  int32_t flags;          /* ARACHNE_FLAG_*                                                */
+} arachne_attn_params;
+
+typedef struct arachne_plan arachne_plan;
+
+/* Build the reusable schedule for one packing (a DiT cascade runs ~60 layers x
+ * (2 fwd + 1 bwd) on the same packing).  Validates everything,
+ * builds the tile work lists in longest-processing-time-first order (heaviest
+ * (sequence, head) groups first, tiles of one group adjacent for L2 reuse of its K/V)
+ * and the RoPE cos/sin tables, and uploads them to the current device.
+ *   cu_seqlens_host : int32 [B+1] HOST, cu_seqlens[0] = 0, strictly increasing, [B] = N
+ *   grids_host      : int32 [B][3] HOST = (T, Hg, Wg) latent grid of each sequence;
+ *                     tokens of a sequence are in row-major (t, h, w) order, w fastest
+ * On success *out owns host + small device arrays; free with arachne_plan_destroy.
+ * Synchronous (uses cudaMalloc/cudaMemcpy). */
+int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params,
+                        const int32_t* cu_seqlens_host, const int32_t* grids_host);
+void arachne_plan_destroy(arachne_plan* plan);
+
+/* Bytes of caller-owned device workspace needed by one call.  pass: 0 = fwd, 1 = bwd.
+ * Returns 0 if plan is NULL or pass is invalid. */
+size_t arachne_workspace_bytes(const arachne_plan* plan, int pass);
+
+/* Number of kernels one call enqueues (for launch accounting). pass: 0 = fwd, 1 = bwd. */
+int arachne_num_launches(const arachne_plan* plan, int pass);
+
+/* Forward.  q, k, v: raw bf16 [N,H,D] (Q, K pre-norm, pre-RoPE).  Writes o (bf16 [N,H,D])
+ * and lse (fp32 [H,N]).  workspace: >= arachne_workspace_bytes(plan, 0), 256-byte aligned
+ * recommended (16 required); its contents are scratch. */
+int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
+                            const float* gamma_q, const float* gamma_k, void* o, float* lse,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Backward.  Needs the o and lse that fwd produced for the same inputs and plan, and d_o
+ * (bf16 [N,H,D]).  Writes dq, dk (gradients w.r.t. the RAW q, k) and dv, all bf16 [N,H,D].
+ * With ARACHNE_FLAG_DETERMINISTIC the result is bit-identical from run to run on the same
+ * device and plan (no atomics; fixed summation order). */
+int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
+                            const float* gamma_q, const float* gamma_k, const void* o,
+                            const float* lse, const void* d_o, void* dq, void* dk, void* dv,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
+ * memory, pinned or pageable): allocate device buffers, copy in, run on a private stream,
+ * copy the results back, free, and return after everything has completed.  These are the
+ * calls bench.py times for its "e2e" figure. */
+int arachne_varlen_attn_fwd_host(const arachne_plan* plan, const void* q_host, const void* k_host,
+                                 const void* v_host, const float* gamma_q_host,
+                                 const float* gamma_k_host, void* o_host, float* lse_host);
+int arachne_varlen_attn_fwd_bwd_host(const arachne_plan* plan, const void* q_host,
+                                     const void* k_host, const void* v_host,
+                                     const float* gamma_q_host, const float* gamma_k_host,
+                                     const void* d_o_host, void* o_host, float* lse_host,
+                                     void* dq_host, void* dk_host, void* dv_host);
+
+const char* arachne_status_string(int status);
+/* Text of the last CUDA error seen by the calling thread ("" if none). */
+const char* arachne_last_error_message(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARACHNE_ATTN_H_ */
