@@ -1,0 +1,165 @@
+"""Thin ctypes binding over libarachne_attn.so (include/arachne_attn.h) — argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels.  torch is used for device
+memory and streams.  There is NO fallback: importing this module raises if the library has not
+been built (python -m paper_2607_01701_b200.build), and every call raises on a non-zero status.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libarachne_attn.so")
+if not os.path.exists(_LIB_PATH):
+    raise ImportError(
+        f"{_LIB_PATH} is missing: build it with `python -m paper_2607_01701_b200.build` "
+        "(nvcc, sm_100a). There is no CPU fallback.")
+_lib = ctypes.CDLL(_LIB_PATH)
+
+FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE = 1, 2, 4
+
+EXPORTS = [
+    "arachne_plan_create", "arachne_plan_destroy", "arachne_workspace_bytes", "arachne_num_launches",
+    "arachne_varlen_attn_fwd", "arachne_varlen_attn_bwd", "arachne_varlen_attn_fwd_host",
+    "arachne_varlen_attn_fwd_bwd_host", "arachne_status_string", "arachne_last_error_message",
+]
+
+
+class AttnParams(ctypes.Structure):
+    _fields_ = [
+        ("num_seqs", ctypes.c_int32), ("total_tokens", ctypes.c_int32), ("num_heads", ctypes.c_int32),
+        ("head_dim", ctypes.c_int32), ("rope_dims", ctypes.c_int32 * 3), ("rope_theta", ctypes.c_float),
+        ("rms_eps", ctypes.c_float), ("softmax_scale", ctypes.c_float), ("flags", ctypes.c_int32),
+    ]
+
+
+_vp, _i32p, _fp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_void_p
+_lib.arachne_plan_create.restype = ctypes.c_int
+_lib.arachne_plan_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p]
+_lib.arachne_plan_destroy.restype = None
+_lib.arachne_plan_destroy.argtypes = [_vp]
+_lib.arachne_workspace_bytes.restype = ctypes.c_size_t
+_lib.arachne_workspace_bytes.argtypes = [_vp, ctypes.c_int]
+_lib.arachne_num_launches.restype = ctypes.c_int
+_lib.arachne_num_launches.argtypes = [_vp, ctypes.c_int]
+_lib.arachne_varlen_attn_fwd.restype = ctypes.c_int
+_lib.arachne_varlen_attn_fwd.argtypes = [_vp] * 8 + [_vp, ctypes.c_size_t, _vp]
+_lib.arachne_varlen_attn_bwd.restype = ctypes.c_int
+_lib.arachne_varlen_attn_bwd.argtypes = [_vp] * 12 + [_vp, ctypes.c_size_t, _vp]
+_lib.arachne_varlen_attn_fwd_host.restype = ctypes.c_int
+_lib.arachne_varlen_attn_fwd_host.argtypes = [_vp] * 8
+_lib.arachne_varlen_attn_fwd_bwd_host.restype = ctypes.c_int
+_lib.arachne_varlen_attn_fwd_bwd_host.argtypes = [_vp] * 12
+_lib.arachne_status_string.restype = ctypes.c_char_p
+_lib.arachne_status_string.argtypes = [ctypes.c_int]
+_lib.arachne_last_error_message.restype = ctypes.c_char_p
+
+
+class ArachneError(RuntimeError):
+    def __init__(self, status: int):
+        self.status = status
+        msg = _lib.arachne_status_string(status).decode()
+        detail = _lib.arachne_last_error_message().decode()
+        super().__init__(f"arachne status {status}: {msg}" + (f" ({detail})" if status == 10 and detail else ""))
+
+
+def _check(status: int):
+    if status != 0:
+        raise ArachneError(status)
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """arachne_plan_create / arachne_plan_destroy."""
+
+    def __init__(self, cu_seqlens, grids, num_heads, head_dim, rope_dims, rope_theta=10000.0, rms_eps=1e-6,
+                 softmax_scale=0.0, flags=0):
+        cu = [int(x) for x in cu_seqlens]
+        gr = [int(x) for g in grids for x in g]
+        self.params = AttnParams()
+        self.params.num_seqs = len(cu) - 1
+        self.params.total_tokens = cu[-1] if cu else 0
+        self.params.num_heads = num_heads
+        self.params.head_dim = head_dim
+        self.params.rope_dims[:] = [int(x) for x in rope_dims]
+        self.params.rope_theta = rope_theta
+        self.params.rms_eps = rms_eps
+        self.params.softmax_scale = softmax_scale
+        self.params.flags = flags
+        self._h = _vp()
+        cu_arr = (ctypes.c_int32 * len(cu))(*cu)
+        gr_arr = (ctypes.c_int32 * max(len(gr), 1))(*gr)
+        _check(_lib.arachne_plan_create(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr))
+        self.N, self.H, self.D = self.params.total_tokens, num_heads, head_dim
+
+    def workspace_bytes(self, bwd: bool) -> int:
+        return int(_lib.arachne_workspace_bytes(self._h, 1 if bwd else 0))
+
+    def num_launches(self, bwd: bool) -> int:
+        return int(_lib.arachne_num_launches(self._h, 1 if bwd else 0))
+
+    def close(self):
+        if self._h:
+            _lib.arachne_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _stream_ptr(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def arachne_varlen_attn_fwd(plan: Plan, q, k, v, o, lse, workspace, gamma_q=None, gamma_k=None, stream=None):
+    """q,k,v,o: bf16 CUDA [N,H,D]; lse: fp32 CUDA [H,N]; workspace: uint8 CUDA >= plan.workspace_bytes(False)."""
+    _check(_lib.arachne_varlen_attn_fwd(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
+                                        _ptr(lse), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                        _stream_ptr(stream)))
+
+
+def arachne_varlen_attn_bwd(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, workspace, gamma_q=None, gamma_k=None,
+                            stream=None):
+    _check(_lib.arachne_varlen_attn_bwd(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
+                                        _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(workspace),
+                                        workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
+def arachne_varlen_attn_fwd_host(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None):
+    """Same as fwd but every tensor is a HOST (CPU, preferably pinned) tensor; copies are inside the call."""
+    _check(_lib.arachne_varlen_attn_fwd_host(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k),
+                                             _ptr(o), _ptr(lse)))
+
+
+def arachne_varlen_attn_fwd_bwd_host(plan: Plan, q, k, v, d_o, o, lse, dq, dk, dv, gamma_q=None, gamma_k=None):
+    _check(_lib.arachne_varlen_attn_fwd_bwd_host(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k),
+                                                 _ptr(d_o), _ptr(o), _ptr(lse), _ptr(dq), _ptr(dk), _ptr(dv)))
+
+
+# ---- convenience wrappers that allocate outputs / workspace with torch (plumbing only)
+def plan_for(st, flags=0, **kw) -> Plan:
+    return Plan(st["cu_seqlens"], st["grids"], st["H"], st["D"], st["rope_dims"], flags=flags, **kw)
+
+
+def forward(plan: Plan, q, k, v, gamma_q=None, gamma_k=None, workspace=None):
+    o = torch.empty_like(q)
+    lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=q.device)
+    ws = workspace if workspace is not None else torch.empty(plan.workspace_bytes(False), dtype=torch.uint8, device=q.device)
+    arachne_varlen_attn_fwd(plan, q, k, v, o, lse, ws, gamma_q, gamma_k)
+    return o, lse
+
+
+def backward(plan: Plan, q, k, v, o, lse, d_o, gamma_q=None, gamma_k=None, workspace=None):
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    ws = workspace if workspace is not None else torch.empty(plan.workspace_bytes(True), dtype=torch.uint8, device=q.device)
+    arachne_varlen_attn_bwd(plan, q, k, v, o, lse, d_o, dq, dk, dv, ws, gamma_q, gamma_k)
+    return dq, dk, dv

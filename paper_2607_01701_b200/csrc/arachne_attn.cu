@@ -1,0 +1,380 @@
+// libarachne_attn.so — C ABI (include/arachne_attn.h) over the sm_100a kernels.
+// Host side: validation, the plan (tile work list in LPT order, RoPE tables), workspace carving
+// and kernel launches.  No torch types, no hidden allocation or synchronisation in fwd/bwd.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/arachne_attn.h"
+#include "bwd.cuh"
+#include "common.cuh"
+#include "fwd.cuh"
+#include "prep.cuh"
+
+using namespace arachne;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int cuda_fail(cudaError_t e, const char* what) {
+  g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return ARACHNE_ERR_CUDA;
+}
+#define ARACHNE_CUDA(call)                                  \
+  do {                                                      \
+    cudaError_t e__ = (call);                               \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call);   \
+  } while (0)
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+}  // namespace
+
+struct arachne_plan {
+  arachne_attn_params p;
+  std::vector<int32_t> cu;
+  std::vector<SeqInfo> seqs;
+  int n_tiles_total = 0;
+  int n_items = 0;
+  int num_sms = 0;
+  int device = 0;
+  // device arrays (owned)
+  SeqInfo* d_seqs = nullptr;
+  int* d_tile_seq = nullptr;
+  WorkItem* d_items = nullptr;
+  int* d_counter = nullptr;
+  float2* d_rope = nullptr;
+  ProblemDesc pd{};
+  // workspace layout
+  size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0;
+};
+
+namespace {
+
+template <int D>
+int configure_kernels() {
+  ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
+  ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
+  ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
+  return ARACHNE_OK;
+}
+
+struct FwdWs { uint8_t *qt, *kt, *vt; };
+struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
+
+size_t fwd_ws_bytes(const arachne_plan* pl) { return 3 * pl->img_bytes; }
+size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + 2 * pl->grad_bytes; }
+
+template <int D>
+int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
+               void* o, float* lse, void* ws, cudaStream_t st) {
+  uint8_t* w = static_cast<uint8_t*>(ws);
+  FwdWs f{w, w + pl->img_bytes, w + 2 * pl->img_bytes};
+  PrepParams pp{};
+  pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
+  pp.v = static_cast<const __nv_bfloat16*>(v);
+  pp.gamma_q = gq; pp.gamma_k = gk;
+  pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
+  pp.out_fmt = FMT_F16;
+  prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
+  ARACHNE_CUDA(cudaGetLastError());
+  FwdParams fp{f.qt, f.kt, f.vt, static_cast<__nv_bfloat16*>(o), lse};
+  const int grid = std::min(pl->num_sms, pl->n_items);
+  fwd_kernel<D><<<grid, 192, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
+  ARACHNE_CUDA(cudaGetLastError());
+  return ARACHNE_OK;
+}
+
+template <int D>
+int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
+               const void* o, const float* lse, const void* d_o, void* dq, void* dk, void* dv, void* ws,
+               cudaStream_t st) {
+  uint8_t* w = static_cast<uint8_t*>(ws);
+  BwdWs b{};
+  b.qt = w; w += pl->img_bytes;
+  b.kt = w; w += pl->img_bytes;
+  b.vt = w; w += pl->img_bytes;
+  b.dot = w; w += pl->img_bytes;
+  b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
+  b.delta_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
+  b.gq_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
+  b.gk_t = reinterpret_cast<float*>(w);
+  PrepParams pp{};
+  pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
+  pp.v = static_cast<const __nv_bfloat16*>(v); pp.d_o = static_cast<const __nv_bfloat16*>(d_o);
+  pp.o = static_cast<const __nv_bfloat16*>(o); pp.lse = lse;
+  pp.gamma_q = gq; pp.gamma_k = gk;
+  pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
+  pp.out_fmt = FMT_BF16;
+  prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
+  ARACHNE_CUDA(cudaGetLastError());
+  BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv)};
+  const int grid = std::min(pl->num_sms, pl->n_items);
+  bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
+  ARACHNE_CUDA(cudaGetLastError());
+  bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 2);
+  ARACHNE_CUDA(cudaGetLastError());
+  PostParams po{b.gq_t, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk)};
+  const long long rows = static_cast<long long>(pl->p.total_tokens) * pl->p.num_heads;
+  post_kernel<D><<<dim3(static_cast<unsigned>((rows + 7) / 8), 2), 256, 0, st>>>(pl->pd, po);
+  ARACHNE_CUDA(cudaGetLastError());
+  return ARACHNE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* arachne_status_string(int s) {
+  switch (s) {
+    case ARACHNE_OK: return "ok";
+    case ARACHNE_ERR_NULL_POINTER: return "null pointer";
+    case ARACHNE_ERR_BAD_HEAD_DIM: return "head_dim must be 64 or 128";
+    case ARACHNE_ERR_BAD_ROPE_DIMS: return "rope_dims must be even, non-negative and sum to head_dim";
+    case ARACHNE_ERR_BAD_CU_SEQLENS: return "cu_seqlens must start at 0 and be strictly increasing";
+    case ARACHNE_ERR_GRID_MISMATCH: return "T*Hg*Wg != sequence length";
+    case ARACHNE_ERR_TOTAL_TOKENS: return "cu_seqlens[num_seqs] != total_tokens";
+    case ARACHNE_ERR_MISALIGNED: return "pointer not 16-byte aligned";
+    case ARACHNE_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case ARACHNE_ERR_BAD_ARCH: return "device is not compute capability 10.x (B200 / sm_100a required)";
+    case ARACHNE_ERR_CUDA: return "CUDA runtime error";
+    case ARACHNE_ERR_BAD_SHAPE: return "bad shape";
+    case ARACHNE_ERR_BAD_PARAM: return "bad parameter";
+    default: return "unknown status";
+  }
+}
+
+const char* arachne_last_error_message(void) { return g_last_error.c_str(); }
+
+int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids) {
+  if (!out || !params || !cu || !grids) return ARACHNE_ERR_NULL_POINTER;
+  *out = nullptr;
+  const arachne_attn_params& p = *params;
+  if (p.head_dim != 64 && p.head_dim != 128) return ARACHNE_ERR_BAD_HEAD_DIM;
+  if (p.num_seqs <= 0 || p.num_heads <= 0 || p.total_tokens <= 0 || p.num_heads > 65535) return ARACHNE_ERR_BAD_SHAPE;
+  int rsum = 0;
+  for (int a = 0; a < 3; ++a) {
+    if (p.rope_dims[a] < 0 || (p.rope_dims[a] & 1)) return ARACHNE_ERR_BAD_ROPE_DIMS;
+    rsum += p.rope_dims[a];
+  }
+  if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
+  if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~7))
+    return ARACHNE_ERR_BAD_PARAM;
+  if (cu[0] != 0) return ARACHNE_ERR_BAD_CU_SEQLENS;
+  for (int b = 0; b < p.num_seqs; ++b)
+    if (cu[b + 1] <= cu[b]) return ARACHNE_ERR_BAD_CU_SEQLENS;          // R16: L_b >= 1
+  if (cu[p.num_seqs] != p.total_tokens) return ARACHNE_ERR_TOTAL_TOKENS;
+  for (int b = 0; b < p.num_seqs; ++b) {
+    const int32_t* g = grids + 3 * b;
+    if (g[0] <= 0 || g[1] <= 0 || g[2] <= 0) return ARACHNE_ERR_GRID_MISMATCH;
+    if (static_cast<long long>(g[0]) * g[1] * g[2] != static_cast<long long>(cu[b + 1] - cu[b])) return ARACHNE_ERR_GRID_MISMATCH;
+  }
+  int dev = 0;
+  cudaDeviceProp prop{};
+  ARACHNE_CUDA(cudaGetDevice(&dev));
+  ARACHNE_CUDA(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) return ARACHNE_ERR_BAD_ARCH;
+
+  arachne_plan* pl = new (std::nothrow) arachne_plan();
+  if (!pl) { g_last_error = "out of host memory"; return ARACHNE_ERR_CUDA; }
+  pl->p = p;
+  if (pl->p.softmax_scale == 0.f) pl->p.softmax_scale = 1.0f / std::sqrt(static_cast<float>(p.head_dim));   // R8
+  pl->device = dev;
+  pl->num_sms = prop.multiProcessorCount;
+  pl->cu.assign(cu, cu + p.num_seqs + 1);
+  int tile_base = 0, ext[3] = {1, 1, 1};
+  for (int b = 0; b < p.num_seqs; ++b) {
+    SeqInfo s{};
+    s.tok_start = cu[b]; s.len = cu[b + 1] - cu[b];
+    s.tile_base = tile_base; s.n_tiles = (s.len + kTileRows - 1) / kTileRows;
+    s.T = grids[3 * b]; s.Hg = grids[3 * b + 1]; s.Wg = grids[3 * b + 2];
+    tile_base += s.n_tiles;
+    for (int a = 0; a < 3; ++a) ext[a] = std::max(ext[a], grids[3 * b + a]);
+    pl->seqs.push_back(s);
+  }
+  pl->n_tiles_total = tile_base;
+  pl->n_items = tile_base * p.num_heads;
+  std::vector<int> tile_seq(pl->n_tiles_total);
+  for (int b = 0; b < p.num_seqs; ++b)
+    for (int t = 0; t < pl->seqs[b].n_tiles; ++t) tile_seq[pl->seqs[b].tile_base + t] = b;
+  // Work list: (sequence, head) groups in longest-processing-time-first order (a tile of sequence b
+  // costs n_tiles_b inner iterations), tiles of one group adjacent so that CTAs running side by
+  // side stream the same K/V (or Q/dO) tiles through L2.
+  std::vector<int> order(p.num_seqs);
+  for (int b = 0; b < p.num_seqs; ++b) order[b] = b;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return pl->seqs[a].n_tiles > pl->seqs[b].n_tiles; });
+  std::vector<WorkItem> items;
+  items.reserve(pl->n_items);
+  for (int b : order)
+    for (int h = 0; h < p.num_heads; ++h)
+      for (int t = 0; t < pl->seqs[b].n_tiles; ++t) items.push_back(WorkItem{b, h, t, 0});
+  // RoPE tables in fp64 -> fp32 (readings R4, R5)
+  std::vector<float2> tab;
+  RopeDesc rd{};
+  for (int a = 0; a < 3; ++a) {
+    rd.off[a] = static_cast<int>(tab.size());
+    rd.half[a] = p.rope_dims[a] / 2;
+    for (int x = 0; x < ext[a]; ++x)
+      for (int pr = 0; pr < rd.half[a]; ++pr) {
+        const double phi = static_cast<double>(x) * std::pow(static_cast<double>(p.rope_theta), -2.0 * pr / p.rope_dims[a]);
+        tab.push_back(make_float2(static_cast<float>(std::cos(phi)), static_cast<float>(std::sin(phi))));
+      }
+  }
+  if (tab.empty()) tab.push_back(make_float2(1.f, 0.f));
+
+  auto fail = [&](cudaError_t e, const char* what) { int rc = cuda_fail(e, what); arachne_plan_destroy(pl); return rc; };
+  cudaError_t e;
+#define PLAN_UP(dptr, vec, T)                                                                                   \
+  if ((e = cudaMalloc(reinterpret_cast<void**>(&dptr), (vec).size() * sizeof(T))) != cudaSuccess) return fail(e, "cudaMalloc"); \
+  if ((e = cudaMemcpy(dptr, (vec).data(), (vec).size() * sizeof(T), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e, "cudaMemcpy");
+  PLAN_UP(pl->d_seqs, pl->seqs, SeqInfo)
+  PLAN_UP(pl->d_tile_seq, tile_seq, int)
+  PLAN_UP(pl->d_items, items, WorkItem)
+  PLAN_UP(pl->d_rope, tab, float2)
+#undef PLAN_UP
+  if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_counter), 4 * sizeof(int))) != cudaSuccess) return fail(e, "cudaMalloc");
+  if ((e = cudaMemset(pl->d_counter, 0, 4 * sizeof(int))) != cudaSuccess) return fail(e, "cudaMemset");
+  int rc = p.head_dim == 128 ? configure_kernels<128>() : configure_kernels<64>();
+  if (rc != ARACHNE_OK) { arachne_plan_destroy(pl); return rc; }
+
+  rd.tab = pl->d_rope;
+  ProblemDesc& pd = pl->pd;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.sched_counter = pl->d_counter;
+  pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
+  pd.N = p.total_tokens; pd.H = p.num_heads;
+  pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
+  pd.no_norm = (p.flags & ARACHNE_FLAG_NO_NORM) ? 1 : 0;
+  pd.no_rope = (p.flags & ARACHNE_FLAG_NO_ROPE) ? 1 : 0;
+  pd.rope = rd;
+  pl->tile_bytes = static_cast<size_t>(kTileRows) * p.head_dim * 2;
+  pl->img_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * pl->tile_bytes, 1024);
+  pl->rowvec_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * sizeof(float), 1024);
+  pl->grad_bytes = align_up(static_cast<size_t>(p.total_tokens) * p.num_heads * p.head_dim * sizeof(float), 1024);
+  *out = pl;
+  return ARACHNE_OK;
+}
+
+void arachne_plan_destroy(arachne_plan* pl) {
+  if (!pl) return;
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_counter); cudaFree(pl->d_rope);
+  delete pl;
+}
+
+size_t arachne_workspace_bytes(const arachne_plan* pl, int pass) {
+  if (!pl) return 0;
+  if (pass == 0) return fwd_ws_bytes(pl);
+  if (pass == 1) return bwd_ws_bytes(pl);
+  return 0;
+}
+
+int arachne_num_launches(const arachne_plan* pl, int pass) {
+  if (!pl) return 0;
+  return pass == 0 ? 2 : (pass == 1 ? 4 : 0);
+}
+
+int arachne_varlen_attn_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
+                            const float* gamma_k, void* o, float* lse, void* ws, size_t ws_bytes, void* stream) {
+  if (!pl || !q || !k || !v || !o || !lse || !ws) return ARACHNE_ERR_NULL_POINTER;
+  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(ws) ||
+      (gamma_q && misaligned(gamma_q)) || (gamma_k && misaligned(gamma_k)))
+    return ARACHNE_ERR_MISALIGNED;
+  if (ws_bytes < fwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  return pl->p.head_dim == 128 ? launch_fwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, ws, st)
+                               : launch_fwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, ws, st);
+}
+
+int arachne_varlen_attn_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
+                            const float* gamma_k, const void* o, const float* lse, const void* d_o, void* dq, void* dk,
+                            void* dv, void* ws, size_t ws_bytes, void* stream) {
+  if (!pl || !q || !k || !v || !o || !lse || !d_o || !dq || !dk || !dv || !ws) return ARACHNE_ERR_NULL_POINTER;
+  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(d_o) ||
+      misaligned(dq) || misaligned(dk) || misaligned(dv) || misaligned(ws) || (gamma_q && misaligned(gamma_q)) ||
+      (gamma_k && misaligned(gamma_k)))
+    return ARACHNE_ERR_MISALIGNED;
+  if (ws_bytes < bwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  return pl->p.head_dim == 128
+             ? launch_bwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, ws, st)
+             : launch_bwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, ws, st);
+}
+
+// ---------------------------------------------------------------- host-buffer convenience calls
+namespace {
+struct DevBufs {
+  std::vector<void*> ptrs;
+  ~DevBufs() { for (void* p : ptrs) cudaFree(p); }
+  int alloc(void** p, size_t bytes) {
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
+    ptrs.push_back(*p);
+    return ARACHNE_OK;
+  }
+};
+}  // namespace
+
+static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, const void* k_h, const void* v_h,
+                    const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h, void* dq_h,
+                    void* dk_h, void* dv_h) {
+  if (!pl || !q_h || !k_h || !v_h || !o_h || !lse_h) return ARACHNE_ERR_NULL_POINTER;
+  if (with_bwd && (!do_h || !dq_h || !dk_h || !dv_h)) return ARACHNE_ERR_NULL_POINTER;
+  const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
+  const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
+  const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
+  DevBufs bufs;
+  void *q, *k, *v, *o, *lse, *ws, *d_o = nullptr, *dq = nullptr, *dk = nullptr, *dv = nullptr, *gq = nullptr, *gk = nullptr;
+  int rc;
+  const size_t wsb = std::max(fwd_ws_bytes(pl), with_bwd ? bwd_ws_bytes(pl) : size_t(0));
+  if ((rc = bufs.alloc(&q, nb)) || (rc = bufs.alloc(&k, nb)) || (rc = bufs.alloc(&v, nb)) || (rc = bufs.alloc(&o, nb)) ||
+      (rc = bufs.alloc(&lse, lb)) || (rc = bufs.alloc(&ws, wsb)))
+    return rc;
+  if (gq_h && (rc = bufs.alloc(&gq, gb))) return rc;
+  if (gk_h && (rc = bufs.alloc(&gk, gb))) return rc;
+  if (with_bwd && ((rc = bufs.alloc(&d_o, nb)) || (rc = bufs.alloc(&dq, nb)) || (rc = bufs.alloc(&dk, nb)) || (rc = bufs.alloc(&dv, nb))))
+    return rc;
+  cudaStream_t st;
+  ARACHNE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  struct StreamGuard { cudaStream_t s; ~StreamGuard() { cudaStreamDestroy(s); } } guard{st};
+  ARACHNE_CUDA(cudaMemcpyAsync(q, q_h, nb, cudaMemcpyHostToDevice, st));
+  ARACHNE_CUDA(cudaMemcpyAsync(k, k_h, nb, cudaMemcpyHostToDevice, st));
+  ARACHNE_CUDA(cudaMemcpyAsync(v, v_h, nb, cudaMemcpyHostToDevice, st));
+  if (gq) ARACHNE_CUDA(cudaMemcpyAsync(gq, gq_h, gb, cudaMemcpyHostToDevice, st));
+  if (gk) ARACHNE_CUDA(cudaMemcpyAsync(gk, gk_h, gb, cudaMemcpyHostToDevice, st));
+  if (with_bwd) ARACHNE_CUDA(cudaMemcpyAsync(d_o, do_h, nb, cudaMemcpyHostToDevice, st));
+  rc = arachne_varlen_attn_fwd(pl, q, k, v, static_cast<float*>(gq), static_cast<float*>(gk), o, static_cast<float*>(lse), ws, wsb, st);
+  if (rc) return rc;
+  ARACHNE_CUDA(cudaMemcpyAsync(o_h, o, nb, cudaMemcpyDeviceToHost, st));
+  ARACHNE_CUDA(cudaMemcpyAsync(lse_h, lse, lb, cudaMemcpyDeviceToHost, st));
+  if (with_bwd) {
+    rc = arachne_varlen_attn_bwd(pl, q, k, v, static_cast<float*>(gq), static_cast<float*>(gk), o, static_cast<float*>(lse), d_o,
+                                 dq, dk, dv, ws, wsb, st);
+    if (rc) return rc;
+    ARACHNE_CUDA(cudaMemcpyAsync(dq_h, dq, nb, cudaMemcpyDeviceToHost, st));
+    ARACHNE_CUDA(cudaMemcpyAsync(dk_h, dk, nb, cudaMemcpyDeviceToHost, st));
+    ARACHNE_CUDA(cudaMemcpyAsync(dv_h, dv, nb, cudaMemcpyDeviceToHost, st));
+  }
+  ARACHNE_CUDA(cudaStreamSynchronize(st));
+  return ARACHNE_OK;
+}
+
+int arachne_varlen_attn_fwd_host(const arachne_plan* pl, const void* q_h, const void* k_h, const void* v_h,
+                                 const float* gq_h, const float* gk_h, void* o_h, float* lse_h) {
+  return run_host(pl, false, q_h, k_h, v_h, gq_h, gk_h, nullptr, o_h, lse_h, nullptr, nullptr, nullptr);
+}
+
+int arachne_varlen_attn_fwd_bwd_host(const arachne_plan* pl, const void* q_h, const void* k_h, const void* v_h,
+                                     const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h,
+                                     void* dq_h, void* dk_h, void* dv_h) {
+  return run_host(pl, true, q_h, k_h, v_h, gq_h, gk_h, do_h, o_h, lse_h, dq_h, dk_h, dv_h);
+}
+
+}  // extern "C"

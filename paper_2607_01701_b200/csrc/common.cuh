@@ -1,0 +1,54 @@
+// Device-visible plan structures shared by all arachne kernels (include/arachne_attn.h is the
+// public boundary; this header is internal).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace arachne {
+
+constexpr int kTileRows = 128;   // tokens per tile (query tile == key tile)
+
+// One packed sequence (BASELINE.json north_star: "packed batch ... per-sequence (T,H,W) latent grid").
+struct SeqInfo {
+  int tok_start;   // cu_seqlens[b]
+  int len;         // L_b
+  int tile_base;   // index of the sequence's first 128-token tile in the tiled workspace
+  int n_tiles;     // ceil(L_b / 128)
+  int T, Hg, Wg;   // latent grid; token n -> (n / (Hg*Wg), (n / Wg) % Hg, n % Wg)   (reading R7)
+  int pad;
+};
+
+// One unit of work for every persistent kernel: (sequence, head, 128-token tile of that sequence).
+// Forward / dQ kernels read it as a QUERY tile, the dK/dV kernel as a KEY tile.  The host orders
+// the list longest-processing-time-first by (sequence, head) group, tiles of a group adjacent.
+struct WorkItem {
+  int seq;
+  int head;
+  int tile;
+  int pad;
+};
+
+// cos/sin tables of the 3D RoPE (readings R4-R6): entry (axis a, position x, pair p) at
+// tab[off[a] + x * half[a] + p] = (cos, sin)(x * theta^(-2p/d_a)), computed in fp64 on the host.
+struct RopeDesc {
+  const float2* tab;
+  int off[3];
+  int half[3];   // d_a / 2
+};
+
+struct ProblemDesc {
+  const SeqInfo* seqs;
+  const int* tile_seq;       // [n_tiles_total] tile -> sequence
+  const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
+  int* sched_counter;        // dynamic tile scheduler: next item to hand out
+  int n_items;
+  int n_tiles_total;
+  int num_seqs;
+  int N, H;
+  float eps;
+  float softmax_scale;
+  int no_norm, no_rope;
+  RopeDesc rope;
+};
+
+}  // namespace arachne

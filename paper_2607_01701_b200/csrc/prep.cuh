@@ -1,0 +1,242 @@
+// Elementwise (HBM-bound) kernels around the tensor-core kernels:
+//   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> 16-bit operand tile images;
+//                 V, dO -> tile images (zero-padded tails); D_i = rowsum(dO*O); LSE*log2e padded.
+//   post_kernel : §8 a8.  dq~, dk~ (fp32) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK.
+// One warp owns one (token, head) row; lane l owns the D/32 contiguous elements [l*D/32, ...),
+// so both elements of every RoPE pair (2p, 2p+1) sit in the same lane and the only cross-lane
+// work is the sum of squares.  All loads/stores are whole 128/256-byte row segments.
+#pragma once
+#include "common.cuh"
+#include "sm100.cuh"
+
+namespace arachne {
+
+struct PrepParams {
+  const __nv_bfloat16* q;
+  const __nv_bfloat16* k;
+  const __nv_bfloat16* v;
+  const __nv_bfloat16* d_o;    // nullable (forward)
+  const __nv_bfloat16* o;      // nullable (forward)
+  const float* lse;            // nullable (forward)
+  const float* gamma_q;        // nullable => ones
+  const float* gamma_k;
+  uint8_t* qt;                 // [H][n_tiles][128*D*2]
+  uint8_t* kt;
+  uint8_t* vt;
+  uint8_t* dot;                // nullable
+  float* lse2_t;               // [H][n_tiles][128]  lse * log2(e); +inf on pad rows
+  float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
+  int out_fmt;                 // FMT_F16 (forward: LSE accuracy) or FMT_BF16 (backward)
+};
+
+__device__ __forceinline__ float warp_sum(float x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  return x;
+}
+
+template <int EPL>
+__device__ __forceinline__ void load_bf16_row(const __nv_bfloat16* p, float (&x)[EPL]) {
+  if constexpr (EPL == 4) {
+    const uint2 u = *reinterpret_cast<const uint2*>(p);
+    x[0] = __uint_as_float(u.x << 16); x[1] = __uint_as_float(u.x & 0xffff0000u);
+    x[2] = __uint_as_float(u.y << 16); x[3] = __uint_as_float(u.y & 0xffff0000u);
+  } else {
+    const uint32_t u = *reinterpret_cast<const uint32_t*>(p);
+    x[0] = __uint_as_float(u << 16); x[1] = __uint_as_float(u & 0xffff0000u);
+  }
+}
+
+// (cos, sin) of the RoPE pair `pp` (0..D/2-1) at grid position pos[]
+__device__ __forceinline__ float2 rope_cs(const RopeDesc& rp, int pp, const int (&pos)[3]) {
+  int a = 0, p = pp;
+  if (p >= rp.half[0]) { p -= rp.half[0]; a = 1; if (p >= rp.half[1]) { p -= rp.half[1]; a = 2; } }
+  return __ldg(&rp.tab[rp.off[a] + pos[a] * rp.half[a] + p]);
+}
+
+// byte offset of element d of row r inside a [128][D] tile image
+__device__ __forceinline__ uint32_t image_off(int r, int d) {
+  return static_cast<uint32_t>(d >> 6) * (kTileRows * 128) + swz_off(r, (d & 63) >> 3) + (d & 7) * 2;
+}
+
+template <int EPL>
+__device__ __forceinline__ void store_image(uint8_t* img, int r, int d0, const float (&y)[EPL], int fmt) {
+  uint8_t* dst = img + image_off(r, d0);
+  if constexpr (EPL == 4) {
+    uint2 u;
+    if (fmt == FMT_F16) { u.x = pack_f16x2(y[0], y[1]); u.y = pack_f16x2(y[2], y[3]); }
+    else                { u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]); }
+    *reinterpret_cast<uint2*>(dst) = u;
+  } else {
+    *reinterpret_cast<uint32_t*>(dst) = fmt == FMT_F16 ? pack_f16x2(y[0], y[1]) : pack_bf16x2(y[0], y[1]);
+  }
+}
+
+// x~ = RoPE(gamma * x * rsqrt(mean(x^2) + eps))  (readings R1-R5), one row per warp
+template <int D>
+__device__ __forceinline__ void norm_rope_store(const ProblemDesc& pd, const __nv_bfloat16* src, const float* gamma,
+                                                uint8_t* img, int r, bool valid, const int (&pos)[3], int lane, int fmt) {
+  constexpr int EPL = D / 32;
+  const int d0 = lane * EPL;
+  float x[EPL];
+  if (valid) {
+    load_bf16_row<EPL>(src + d0, x);
+    if (!pd.no_norm) {
+      float ss = 0.f;
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) ss += x[i] * x[i];
+      ss = warp_sum(ss);
+      const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) x[i] *= rinv * (gamma ? __ldg(&gamma[d0 + i]) : 1.0f);
+    }
+    if (!pd.no_rope) {
+#pragma unroll
+      for (int i = 0; i < EPL; i += 2) {
+        const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
+        const float x0 = x[i], x1 = x[i + 1];
+        x[i] = x0 * cs.x - x1 * cs.y;
+        x[i + 1] = x0 * cs.y + x1 * cs.x;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) x[i] = 0.f;   // zero-padded tail rows (never NaN: 0 * P stays 0)
+  }
+  store_image<EPL>(img, r, d0, x, fmt);
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp) {
+  constexpr int EPL = D / 32;
+  constexpr int TILE_BYTES = kTileRows * D * 2;
+  const int gtile = blockIdx.x, h = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x < 4) pd.sched_counter[threadIdx.x] = 0;
+  const SeqInfo sq = pd.seqs[pd.tile_seq[gtile]];
+  const int t = gtile - sq.tile_base;
+  const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
+  const size_t row_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows;
+  const int d0 = lane * EPL;
+  for (int r = warp; r < kTileRows; r += 8) {
+    const int n = t * kTileRows + r;            // token index inside the sequence
+    const bool valid = n < sq.len;
+    int pos[3];
+    const int hw = sq.Hg * sq.Wg;
+    pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
+    const size_t src = (static_cast<size_t>(sq.tok_start + n) * pd.H + h) * D;
+    norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, pos, lane, pp.out_fmt);
+    norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, pos, lane, pp.out_fmt);
+    float x[EPL];
+    if (valid) load_bf16_row<EPL>(pp.v + src + d0, x);
+    else {
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) x[i] = 0.f;
+    }
+    store_image<EPL>(pp.vt + img_off, r, d0, x, FMT_BF16);     // bf16 -> bf16 is exact
+    if (pp.dot) {
+      float g[EPL], oo[EPL];
+      float dsum = 0.f;
+      if (valid) {
+        load_bf16_row<EPL>(pp.d_o + src + d0, g);
+        load_bf16_row<EPL>(pp.o + src + d0, oo);
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) dsum += g[i] * oo[i];
+      } else {
+#pragma unroll
+        for (int i = 0; i < EPL; ++i) g[i] = 0.f;
+      }
+      store_image<EPL>(pp.dot + img_off, r, d0, g, FMT_BF16);
+      dsum = warp_sum(dsum);                                    // D_i = sum_d dO*O   (§8 a5)
+      if (lane == 0) {
+        pp.delta_t[row_off + r] = valid ? dsum : 0.f;
+        // pad rows get +inf so that P = exp2(s - inf) = 0 for them in the backward kernels
+        pp.lse2_t[row_off + r] = valid ? pp.lse[static_cast<size_t>(h) * pd.N + sq.tok_start + n] * 1.4426950408889634f
+                                       : __int_as_float(0x7f800000);
+      }
+    }
+  }
+}
+
+struct PostParams {
+  const float* gq_t;            // dl/dq~ fp32 [N,H,D] (already multiplied by softmax_scale)
+  const float* gk_t;
+  const __nv_bfloat16* q;       // raw
+  const __nv_bfloat16* k;
+  const float* gamma_q;
+  const float* gamma_k;
+  __nv_bfloat16* dq;
+  __nv_bfloat16* dk;
+};
+
+// dx = r*u - r^3 * x * (sum_d u_d x_d)/D,  u = gamma * R^T g~   (§8 a8; oracle: norm_rope_row_bwd)
+template <int D>
+__global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp) {
+  constexpr int EPL = D / 32;
+  const int lane = threadIdx.x & 31;
+  const long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5);   // (token, head)
+  if (row >= static_cast<long long>(pd.N) * pd.H) return;
+  const int tok = static_cast<int>(row / pd.H);
+  const bool is_k = blockIdx.y == 1;
+  const float* gt = is_k ? pp.gk_t : pp.gq_t;
+  const __nv_bfloat16* xraw = is_k ? pp.k : pp.q;
+  const float* gamma = is_k ? pp.gamma_k : pp.gamma_q;
+  __nv_bfloat16* out = is_k ? pp.dk : pp.dq;
+  // sequence of this token: binary search over cu_seqlens (num_seqs is small)
+  int lo = 0, hi = pd.num_seqs - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (pd.seqs[mid].tok_start <= tok) lo = mid; else hi = mid - 1;
+  }
+  const SeqInfo sq = pd.seqs[lo];
+  const int n = tok - sq.tok_start;
+  int pos[3];
+  pos[0] = n / (sq.Hg * sq.Wg); pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
+  const int d0 = lane * EPL;
+  const size_t off = static_cast<size_t>(row) * D + d0;
+  float g[EPL], x[EPL];
+  if constexpr (EPL == 4) {
+    const float4 f = *reinterpret_cast<const float4*>(gt + off);
+    g[0] = f.x; g[1] = f.y; g[2] = f.z; g[3] = f.w;
+  } else {
+    const float2 f = *reinterpret_cast<const float2*>(gt + off);
+    g[0] = f.x; g[1] = f.y;
+  }
+  load_bf16_row<EPL>(xraw + off, x);
+  if (!pd.no_rope) {
+#pragma unroll
+    for (int i = 0; i < EPL; i += 2) {
+      const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
+      const float g0 = g[i], g1 = g[i + 1];
+      g[i] = g0 * cs.x + g1 * cs.y;          // rotate by -phi
+      g[i + 1] = -g0 * cs.y + g1 * cs.x;
+    }
+  }
+  float y[EPL];
+  if (!pd.no_norm) {
+    float ss = 0.f, ux = 0.f;
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) {
+      g[i] *= gamma ? __ldg(&gamma[d0 + i]) : 1.0f;     // u = gamma * g
+      ss += x[i] * x[i];
+      ux += g[i] * x[i];
+    }
+    ss = warp_sum(ss);
+    ux = warp_sum(ux);
+    const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
+    const float c = rinv * rinv * rinv * ux * (1.0f / D);
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) y[i] = rinv * g[i] - c * x[i];
+  } else {
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) y[i] = g[i];
+  }
+  if constexpr (EPL == 4) {
+    uint2 u; u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]);
+    *reinterpret_cast<uint2*>(out + off) = u;
+  } else {
+    *reinterpret_cast<uint32_t*>(out + off) = pack_bf16x2(y[0], y[1]);
+  }
+}
+
+}  // namespace arachne

@@ -1,0 +1,102 @@
+"""Shared helpers for the GPU parity tests: run the CUDA path through the C ABI binding, run the
+oracle on the SAME bytes, and compute the error metrics of reading R17 (per tensor AND per
+sequence, so a broken short sequence cannot hide behind a long one)."""
+import numpy as np
+import torch
+
+# tolerances stated by BASELINE.json north_star
+TOL = dict(O_rel=1e-2, O_abs=2e-2, LSE_abs=1e-3, dQ_rel=2e-2, dK_rel=2e-2, dV_rel=2e-2)
+
+
+def rel_l2(a, b):
+    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
+    den = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a - b))
+
+
+def run_gpu(st, t, flags=0, gamma_q=None, gamma_k=None, with_bwd=True, plan_kw=None):
+    from paper_2607_01701_b200 import binding
+
+    plan = binding.plan_for(st, flags=flags, **(plan_kw or {}))
+    gq = None if gamma_q is None else torch.as_tensor(gamma_q, dtype=torch.float32, device="cuda")
+    gk = None if gamma_k is None else torch.as_tensor(gamma_k, dtype=torch.float32, device="cuda")
+    o, lse = binding.forward(plan, t["q"], t["k"], t["v"], gq, gk)
+    out = {"O": o, "LSE": lse, "plan": plan}
+    if with_bwd:
+        dq, dk, dv = binding.backward(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], gq, gk)
+        out.update(dQ=dq, dK=dk, dV=dv)
+    torch.cuda.synchronize()
+    return out
+
+
+def to_np(x):
+    return x.detach().float().cpu().numpy().astype(np.float64)
+
+
+def check_full(st, got, ref, with_bwd=True, tol=TOL):
+    """Element-by-element comparison of every output, per sequence.  Returns dict of worst metrics."""
+    cu = st["cu_seqlens"]
+    worst = {}
+    keys = ["O"] + (["dQ", "dK", "dV"] if with_bwd else [])
+    g = {k: to_np(got[k]) for k in keys + ["LSE"]}
+    for b in range(len(cu) - 1):
+        s, e = cu[b], cu[b + 1]
+        for k in keys:
+            r = rel_l2(g[k][s:e], ref[k][s:e])
+            worst[k + "_rel"] = max(worst.get(k + "_rel", 0.0), r)
+            assert r <= tol[k + "_rel"], f"{k} rel-L2 {r:.3e} > {tol[k + '_rel']} in sequence {b} (L={e - s})"
+        a = float(np.max(np.abs(g["O"][s:e] - ref["O"][s:e])))
+        worst["O_abs"] = max(worst.get("O_abs", 0.0), a)
+        assert a <= tol["O_abs"], f"O max-abs {a:.3e} in sequence {b}"
+        la = float(np.max(np.abs(g["LSE"][:, s:e] - ref["LSE"][:, s:e])))
+        worst["LSE_abs"] = max(worst.get("LSE_abs", 0.0), la)
+        assert la <= tol["LSE_abs"], f"LSE max-abs {la:.3e} in sequence {b}"
+    return worst
+
+
+def check_rows(st, got, ref, rows, tol=TOL):
+    """Sampled-row comparison (O, LSE, dQ exact per row) for configs too large for the full oracle."""
+    cu = st["cu_seqlens"]
+    rows = np.asarray(rows)
+    idx = torch.as_tensor(rows, device=got["O"].device)
+    heads = ref.get("heads", list(range(st["H"])))
+    hidx = torch.as_tensor(heads, device=got["O"].device)
+    gO = to_np(got["O"][idx][:, hidx])
+    gL = to_np(got["LSE"][hidx][:, idx])
+    gdQ = to_np(got["dQ"][idx][:, hidx]) if "dQ" in got and "dQ" in ref else None
+    worst = {}
+    for b in range(len(cu) - 1):
+        sel = np.nonzero((rows >= cu[b]) & (rows < cu[b + 1]))[0]
+        if len(sel) == 0:
+            continue
+        r = rel_l2(gO[sel], ref["O"][sel])
+        worst["O_rel"] = max(worst.get("O_rel", 0.0), r)
+        assert r <= tol["O_rel"], f"O rel-L2 {r:.3e} in sequence {b}"
+        a = float(np.max(np.abs(gO[sel] - ref["O"][sel])))
+        worst["O_abs"] = max(worst.get("O_abs", 0.0), a)
+        assert a <= tol["O_abs"]
+        la = float(np.max(np.abs(gL[:, sel] - ref["LSE"][:, sel])))
+        worst["LSE_abs"] = max(worst.get("LSE_abs", 0.0), la)
+        assert la <= tol["LSE_abs"], f"LSE max-abs {la:.3e} in sequence {b}"
+        if gdQ is not None:
+            r = rel_l2(gdQ[sel], ref["dQ"][sel])
+            worst["dQ_rel"] = max(worst.get("dQ_rel", 0.0), r)
+            assert r <= tol["dQ_rel"], f"dQ rel-L2 {r:.3e} in sequence {b}"
+    return worst
+
+
+def check_masked_kv(st, got_masked, ref, tol=TOL):
+    """dK/dV of the masked-dO run (all key rows) against the oracle's row-subset backward."""
+    cu = st["cu_seqlens"]
+    heads = ref.get("heads", list(range(st["H"])))
+    hidx = torch.as_tensor(heads, device=got_masked["dK"].device)
+    worst = {}
+    for b in range(len(cu) - 1):
+        s, e = cu[b], cu[b + 1]
+        for k in ("dK", "dV"):
+            if not np.any(ref[k][s:e]):
+                continue
+            r = rel_l2(to_np(got_masked[k][s:e][:, hidx]), ref[k][s:e])
+            worst[k + "_rel"] = max(worst.get(k + "_rel", 0.0), r)
+            assert r <= tol[k + "_rel"], f"{k} (masked dO) rel-L2 {r:.3e} in sequence {b}"
+    return worst
