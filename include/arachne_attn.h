@@ -103,6 +103,19 @@ size_t arachne_workspace_bytes(const arachne_plan* plan, int pass);
 /* Number of kernels one call enqueues (for launch accounting). pass: 0 = fwd, 1 = bwd. */
 int arachne_num_launches(const arachne_plan* plan, int pass);
 
+/* Name of kernel `idx` (0-based, launch order) of a pass; "" if out of range. */
+const char* arachne_kernel_name(int pass, int idx);
+
+/* Per-kernel device timing for benchmarks (bench.py's roofline figure).  When enabled, fwd/bwd
+ * record a CUDA event before the first and after every kernel on the caller's stream (no
+ * synchronisation is added); the plan keeps the events of the last 32 calls per pass.
+ * arachne_plan_kernel_times synchronises on those events and writes to ms_sum[i] the SUM over
+ * the recorded calls of kernel i's duration in milliseconds (ms_sum has n_kernels >=
+ * arachne_num_launches entries) and the number of calls to *n_calls.  Enabling resets the ring.
+ * Not thread-safe with concurrent fwd/bwd on the same plan. */
+int arachne_plan_enable_profiling(arachne_plan* plan, int enable);
+int arachne_plan_kernel_times(const arachne_plan* plan, int pass, float* ms_sum, int n_kernels, int* n_calls);
+
 /* Forward.  q, k, v: raw bf16 [N,H,D] (Q, K pre-norm, pre-RoPE).  Writes o (bf16 [N,H,D])
  * and lse (fp32 [H,N]).  workspace: >= arachne_workspace_bytes(plan, 0), 256-byte aligned
  * recommended (16 required); its contents are scratch. */

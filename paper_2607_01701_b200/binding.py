@@ -24,6 +24,7 @@ EXPORTS = [
     "arachne_plan_create", "arachne_plan_destroy", "arachne_workspace_bytes", "arachne_num_launches",
     "arachne_varlen_attn_fwd", "arachne_varlen_attn_bwd", "arachne_varlen_attn_fwd_host",
     "arachne_varlen_attn_fwd_bwd_host", "arachne_status_string", "arachne_last_error_message",
+    "arachne_kernel_name", "arachne_plan_enable_profiling", "arachne_plan_kernel_times",
 ]
 
 
@@ -55,6 +56,13 @@ _lib.arachne_varlen_attn_fwd_bwd_host.argtypes = [_vp] * 12
 _lib.arachne_status_string.restype = ctypes.c_char_p
 _lib.arachne_status_string.argtypes = [ctypes.c_int]
 _lib.arachne_last_error_message.restype = ctypes.c_char_p
+_lib.arachne_kernel_name.restype = ctypes.c_char_p
+_lib.arachne_kernel_name.argtypes = [ctypes.c_int, ctypes.c_int]
+_lib.arachne_plan_enable_profiling.restype = ctypes.c_int
+_lib.arachne_plan_enable_profiling.argtypes = [_vp, ctypes.c_int]
+_lib.arachne_plan_kernel_times.restype = ctypes.c_int
+_lib.arachne_plan_kernel_times.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_float), ctypes.c_int,
+                                           ctypes.POINTER(ctypes.c_int)]
 
 
 class ArachneError(RuntimeError):
@@ -102,6 +110,18 @@ class Plan:
 
     def num_launches(self, bwd: bool) -> int:
         return int(_lib.arachne_num_launches(self._h, 1 if bwd else 0))
+
+    def enable_profiling(self, enable=True):
+        _check(_lib.arachne_plan_enable_profiling(self._h, 1 if enable else 0))
+
+    def kernel_times(self, bwd: bool):
+        """[(kernel name, mean ms per call)] over the calls recorded since enable_profiling()."""
+        n = self.num_launches(bwd)
+        ms = (ctypes.c_float * n)()
+        calls = ctypes.c_int(0)
+        _check(_lib.arachne_plan_kernel_times(self._h, 1 if bwd else 0, ms, n, ctypes.byref(calls)))
+        c = max(calls.value, 1)
+        return [(_lib.arachne_kernel_name(1 if bwd else 0, i).decode(), ms[i] / c) for i in range(n)], calls.value
 
     def close(self):
         if self._h:

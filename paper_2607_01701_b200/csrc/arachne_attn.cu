@@ -55,6 +55,13 @@ struct arachne_plan {
   ProblemDesc pd{};
   // workspace layout
   size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0;
+  // optional per-kernel timing (arachne_plan_enable_profiling): ring of kProfSlots calls per pass,
+  // kernels+1 events per call, recorded on the caller's stream (no synchronisation).
+  static constexpr int kProfSlots = 32;
+  static constexpr int kMaxKernels = 4;
+  bool profiling = false;
+  mutable long long prof_calls[2] = {0, 0};
+  cudaEvent_t prof_ev[2][kProfSlots][kMaxKernels + 1] = {};
 };
 
 namespace {
@@ -73,6 +80,12 @@ struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_
 size_t fwd_ws_bytes(const arachne_plan* pl) { return 3 * pl->img_bytes; }
 size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + 2 * pl->grad_bytes; }
 
+inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st) {
+  if (!pl->profiling) return;
+  const int slot = static_cast<int>(pl->prof_calls[pass] % arachne_plan::kProfSlots);
+  cudaEventRecord(pl->prof_ev[pass][slot][idx], st);
+}
+
 template <int D>
 int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
                void* o, float* lse, void* ws, cudaStream_t st) {
@@ -84,12 +97,16 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
   pp.out_fmt = FMT_F16;
+  prof_mark(pl, 0, 0, st);
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 0, 1, st);
   FwdParams fp{f.qt, f.kt, f.vt, static_cast<__nv_bfloat16*>(o), lse};
   const int grid = std::min(pl->num_sms, pl->n_items);
   fwd_kernel<D><<<grid, 192, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 0, 2, st);
+  if (pl->profiling) pl->prof_calls[0]++;
   return ARACHNE_OK;
 }
 
@@ -114,18 +131,24 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.out_fmt = FMT_BF16;
+  prof_mark(pl, 1, 0, st);
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 1, 1, st);
   BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv)};
   const int grid = std::min(pl->num_sms, pl->n_items);
   bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 1, 2, st);
   bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 2);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 1, 3, st);
   PostParams po{b.gq_t, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk)};
   const long long rows = static_cast<long long>(pl->p.total_tokens) * pl->p.num_heads;
   post_kernel<D><<<dim3(static_cast<unsigned>((rows + 7) / 8), 2), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
+  prof_mark(pl, 1, 4, st);
+  if (pl->profiling) pl->prof_calls[1]++;
   return ARACHNE_OK;
 }
 
@@ -265,6 +288,10 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
 
 void arachne_plan_destroy(arachne_plan* pl) {
   if (!pl) return;
+  for (auto& pass : pl->prof_ev)
+    for (auto& slot : pass)
+      for (cudaEvent_t ev : slot)
+        if (ev) cudaEventDestroy(ev);
   cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_counter); cudaFree(pl->d_rope);
   delete pl;
 }
@@ -279,6 +306,45 @@ size_t arachne_workspace_bytes(const arachne_plan* pl, int pass) {
 int arachne_num_launches(const arachne_plan* pl, int pass) {
   if (!pl) return 0;
   return pass == 0 ? 2 : (pass == 1 ? 4 : 0);
+}
+
+const char* arachne_kernel_name(int pass, int idx) {
+  static const char* fwd[] = {"prep_kernel(fwd: RMSNorm+RoPE -> fp16 tiles)", "fwd_kernel"};
+  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> bf16 tiles, delta)", "bwd_kernel<dKdV>", "bwd_kernel<dQ>",
+                              "post_kernel(un-RoPE + RMSNorm bwd)"};
+  if (pass == 0 && idx >= 0 && idx < 2) return fwd[idx];
+  if (pass == 1 && idx >= 0 && idx < 4) return bwd[idx];
+  return "";
+}
+
+int arachne_plan_enable_profiling(arachne_plan* pl, int enable) {
+  if (!pl) return ARACHNE_ERR_NULL_POINTER;
+  if (enable && !pl->prof_ev[0][0][0]) {
+    for (auto& pass : pl->prof_ev)
+      for (auto& slot : pass)
+        for (cudaEvent_t& ev : slot) ARACHNE_CUDA(cudaEventCreate(&ev));
+  }
+  pl->profiling = enable != 0;
+  pl->prof_calls[0] = pl->prof_calls[1] = 0;
+  return ARACHNE_OK;
+}
+
+int arachne_plan_kernel_times(const arachne_plan* pl, int pass, float* ms_sum, int n_kernels, int* n_calls) {
+  if (!pl || !ms_sum || !n_calls) return ARACHNE_ERR_NULL_POINTER;
+  if (pass < 0 || pass > 1 || !pl->profiling) return ARACHNE_ERR_BAD_PARAM;
+  const int nk = arachne_num_launches(pl, pass);
+  if (n_kernels < nk) return ARACHNE_ERR_BAD_PARAM;
+  const long long calls = std::min<long long>(pl->prof_calls[pass], arachne_plan::kProfSlots);
+  for (int i = 0; i < nk; ++i) ms_sum[i] = 0.f;
+  for (long long c = 0; c < calls; ++c)
+    for (int i = 0; i < nk; ++i) {
+      float ms = 0.f;
+      ARACHNE_CUDA(cudaEventSynchronize(pl->prof_ev[pass][c][i + 1]));
+      ARACHNE_CUDA(cudaEventElapsedTime(&ms, pl->prof_ev[pass][c][i], pl->prof_ev[pass][c][i + 1]));
+      ms_sum[i] += ms;
+    }
+  *n_calls = static_cast<int>(calls);
+  return ARACHNE_OK;
 }
 
 int arachne_varlen_attn_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
