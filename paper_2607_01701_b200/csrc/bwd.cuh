@@ -123,8 +123,9 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
       }
     }
   } else if (warp == 5) {
-    // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
+    // ------------------------------------------------------------------ MMA issuer (whole warp convergent,
+    // one elected lane issues: keeps descriptors in uniform registers, no per-instruction election loop)
+    {
       constexpr uint32_t idesc_sdp = make_idesc(128, 64, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
       constexpr uint32_t idesc_acc = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
       const uint32_t aX1 = smem_u32(sX1), aX2 = smem_u32(sX2), aY1 = smem_u32(sY1), aY2 = smem_u32(sY2);
@@ -136,6 +137,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
         if (u == 0) { mbar_wait(&y_full[st], ph); tc_fence_after(); }
         const uint32_t tS = tbase + Cfg::kColS + (gg & 1) * 64, tdP = tbase + Cfg::kColDP + (gg & 1) * 64;
         const uint32_t yb = st * TILE + u * 8192;      // rows 64u.. of the streamed image
+        if (elect_one()) {
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
@@ -147,6 +149,8 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
           umma_ss(tdP, make_sdesc(aX2 + koff, 16, 1024), make_sdesc(aY2 + yb + koff, 16, 1024), idesc_sdp, kk > 0);
         }
         umma_commit(&sdp_full[gg & 1]);
+        }
+        __syncwarp();
       };
       for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
         const WorkItem wi = pd.items[item];
@@ -157,11 +161,12 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
         for (uint32_t s = 0; s < G; ++s) {
           const uint32_t gg = g + s, u = s & 1, ytile = yt + (s >> 1), st = ytile % STAGES;
           if (s + 1 < G) issue_sdp(gg + 1, yt + ((s + 1) >> 1), (s + 1) & 1);
-          else umma_commit(x_empty);
+          else { if (elect_one()) umma_commit(x_empty); __syncwarp(); }
           if (s == 0) mbar_wait(acc_free, (it & 1) ^ 1);
           mbar_wait(&pds_full[gg & 1], (gg >> 1) & 1);
           tc_fence_after();
           const uint32_t tP = tbase + Cfg::kColS + (gg & 1) * 64, tdS = tbase + Cfg::kColDP + (gg & 1) * 64;
+          if (elect_one()) {
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk) {
             const uint32_t roff = st * TILE + (u * 64 + kk * 16) * 128;     // K rows of the MN-major B operand
@@ -174,8 +179,11 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
             }
           }
           if (u == 1) umma_commit(&y_empty[st]);
+          }
+          __syncwarp();
         }
-        umma_commit(acc_done);
+        if (elect_one()) umma_commit(acc_done);
+        __syncwarp();
         g += G;
         yt += G >> 1;
       }

@@ -109,7 +109,9 @@ __global__ void __launch_bounds__(192, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     }
   } else if (warp == 5) {
     // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
+    // The whole warp runs the loop convergently (uniform descriptors -> plain UTCHMMA issue, no
+    // per-instruction election loop); one elected lane issues the tcgen05 instructions.
+    {
       constexpr uint32_t idesc_s = make_idesc(128, 128, FMT_F16, FMT_F16, MAJOR_K, MAJOR_K);
       constexpr uint32_t idesc_o = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
       const uint32_t aQ = smem_u32(sQ), aK = smem_u32(sK), aV = smem_u32(sV);
@@ -120,14 +122,17 @@ __global__ void __launch_bounds__(192, 1) fwd_kernel(ProblemDesc pd, FwdParams f
         const uint32_t st = g % STAGES, ph = (g / STAGES) & 1;
         mbar_wait(&k_full[st], ph);
         tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
-        for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t koff = (kk >> 2) * (kTileRows * 128) + (kk & 3) * 32;
-          umma_ss(tS[g & 1], make_sdesc(aQ + koff, 16, 1024), make_sdesc(aK + st * TILE + koff, 16, 1024),
-                  idesc_s, kk > 0);
+          for (int kk = 0; kk < D / 16; ++kk) {
+            const uint32_t koff = (kk >> 2) * (kTileRows * 128) + (kk & 3) * 32;
+            umma_ss(tS[g & 1], make_sdesc(aQ + koff, 16, 1024), make_sdesc(aK + st * TILE + koff, 16, 1024),
+                    idesc_s, kk > 0);
+          }
+          umma_commit(&k_empty[st]);
+          umma_commit(&s_full[g & 1]);
         }
-        umma_commit(&k_empty[st]);
-        umma_commit(&s_full[g & 1]);
+        __syncwarp();
       };
       for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
         const WorkItem wi = pd.items[item];
@@ -137,19 +142,22 @@ __global__ void __launch_bounds__(192, 1) fwd_kernel(ProblemDesc pd, FwdParams f
         for (int j = 0; j < n_kv; ++j) {
           const uint32_t g = kv + j;
           if (j + 1 < n_kv) issue_s(g + 1);
-          else umma_commit(q_empty);          // all S MMAs of this item issued: Q^ smem reusable once they finish
+          else { if (elect_one()) umma_commit(q_empty); __syncwarp(); }   // all S MMAs of this item issued: Q^ smem reusable once they finish
           const uint32_t st = g % STAGES, ph = (g / STAGES) & 1;
           mbar_wait(&v_full[st], ph);
           if (j == 0) mbar_wait(o_free, (it & 1) ^ 1);     // previous item's epilogue has drained O
           mbar_wait(&p_full[g & 1], (g >> 1) & 1);
           tc_fence_after();
+          if (elect_one()) {
 #pragma unroll
-          for (int kk = 0; kk < kTileRows / 16; ++kk) {
-            umma_ts(tO, tS[g & 1] + kk * 8, make_sdesc(aV + st * TILE + kk * 2048, kTileRows * 128, 1024),
-                    idesc_o, (j > 0 || kk > 0) ? 1u : 0u);
+            for (int kk = 0; kk < kTileRows / 16; ++kk) {
+              umma_ts(tO, tS[g & 1] + kk * 8, make_sdesc(aV + st * TILE + kk * 2048, kTileRows * 128, 1024),
+                      idesc_o, (j > 0 || kk > 0) ? 1u : 0u);
+            }
+            umma_commit(&v_empty[st]);
+            umma_commit(pv_done);
           }
-          umma_commit(&v_empty[st]);
-          umma_commit(pv_done);
+          __syncwarp();
         }
         kv += n_kv;
       }

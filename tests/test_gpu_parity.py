@@ -77,11 +77,13 @@ def test_debug_flags_and_scale(orc):
 
 
 def test_large_gamma_rescale_path(orc):
-    """gamma = 3 on both sides -> logits up to sqrt(D)*9: the running max keeps growing across tiles,
-    so the lazy O-rescale path must fire and be right."""
+    """gamma = 2 on both sides -> logits up to sqrt(D)*4 = 45 (16x the softmax temperature of the
+    BASELINE configs): the running max grows by more than 2^8 across tiles, so the lazy O-rescale path
+    must fire and be right.  (gamma = 3 puts |s| near 100, where the bf16 rounding of the backward's
+    recomputed logits, |s|*2^-9 ~ 0.2, alone exceeds north_star's 2e-2 gradient gate: DESIGN.md §6.)"""
     st = inputs.pack([(5, 16, 16)], 2, 128, index=3)
     t = inputs.make_inputs(st, device="cuda")
-    g = np.full(128, 3.0, np.float32)
+    g = np.full(128, 2.0, np.float32)
     got = pu.run_gpu(st, t, gamma_q=g, gamma_k=g)
     a = _np(t)
     ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], gamma_q=g, gamma_k=g)
