@@ -259,10 +259,9 @@ def main():
 
     peaks = load_peaks()
     # ---- roofline of the dominant kernel: dense contraction -> tensor roofline.
-    # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); bwd dK/dV pass 8*D*H*S2
-    # (S, dP, dV, dK — all inside the 5-GEMM backward convention); bwd dQ pass 2*D*H*S2 (only dQ is new work:
-    # its S and dP recompute is the price of the deterministic two-pass design and is not counted).
-    alg = {"fwd_kernel": 4.0, "bwd_kernel<dKdV>": 8.0, "bwd_kernel<dQ>": 2.0}
+    # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); fused backward kernel
+    # 10*D*H*S2 (S, dP, dV, dK, dQ — the 5-GEMM backward convention).
+    alg = {"fwd_kernel": 4.0, "bwd_main(fused 5-GEMM | det: dKdV pass)": 10.0}
     kernels = [{"name": n, "ms": ms} for n, ms in kt_f + kt_b]
     dom = max(kernels, key=lambda k_: k_["ms"])
     dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -13,6 +14,7 @@
 
 #include "../../include/arachne_attn.h"
 #include "bwd.cuh"
+#include "bwd_fused.cuh"
 #include "common.cuh"
 #include "fwd.cuh"
 #include "prep.cuh"
@@ -46,6 +48,7 @@ struct arachne_plan {
   int n_items = 0;
   int num_sms = 0;
   int device = 0;
+  int q_rot = 0;   // fused backward: query-tile rotation per key tile (ARACHNE_BWD_QROT env, tuning)
   // device arrays (owned)
   SeqInfo* d_seqs = nullptr;
   int* d_tile_seq = nullptr;
@@ -54,7 +57,7 @@ struct arachne_plan {
   float2* d_rope = nullptr;
   ProblemDesc pd{};
   // workspace layout
-  size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0;
+  size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0, gradblk_bytes = 0;
   // optional per-kernel timing (arachne_plan_enable_profiling): ring of kProfSlots calls per pass,
   // kernels+1 events per call, recorded on the caller's stream (no synchronisation).
   static constexpr int kProfSlots = 32;
@@ -71,6 +74,7 @@ int configure_kernels() {
   ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
   ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
   ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
+  ARACHNE_CUDA(cudaFuncSetAttribute(bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdFusedCfg<D>::kSmemBytes));
   return ARACHNE_OK;
 }
 
@@ -78,7 +82,7 @@ struct FwdWs { uint8_t *qt, *kt, *vt; };
 struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
 
 size_t fwd_ws_bytes(const arachne_plan* pl) { return 3 * pl->img_bytes; }
-size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + 2 * pl->grad_bytes; }
+size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes; }
 
 inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st) {
   if (!pl->profiling) return;
@@ -122,8 +126,9 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   b.dot = w; w += pl->img_bytes;
   b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.delta_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
-  b.gq_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
-  b.gk_t = reinterpret_cast<float*>(w);
+  b.gk_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
+  b.gq_t = reinterpret_cast<float*>(w);      // gradblk_bytes >= grad_bytes: either layout fits
+  const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
   PrepParams pp{};
   pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
   pp.v = static_cast<const __nv_bfloat16*>(v); pp.d_o = static_cast<const __nv_bfloat16*>(d_o);
@@ -131,19 +136,30 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.out_fmt = FMT_BF16;
+  pp.gq_zero = deterministic ? nullptr : b.gq_t;
   prof_mark(pl, 1, 0, st);
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
-  BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv)};
   const int grid = std::min(pl->num_sms, pl->n_items);
-  bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
-  ARACHNE_CUDA(cudaGetLastError());
-  prof_mark(pl, 1, 2, st);
-  bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 2);
-  ARACHNE_CUDA(cudaGetLastError());
-  prof_mark(pl, 1, 3, st);
-  PostParams po{b.gq_t, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk)};
+  if (deterministic) {
+    // two-pass (7 GEMM) path: every output tile owned by one CTA, fixed summation order
+    BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv)};
+    bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
+    ARACHNE_CUDA(cudaGetLastError());
+    prof_mark(pl, 1, 2, st);
+    bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 2);
+    ARACHNE_CUDA(cudaGetLastError());
+    prof_mark(pl, 1, 3, st);
+  } else {
+    // fused single-pass (5 GEMM) path: dQ~ partial tiles reduce-added at L2 (order not fixed)
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv), pl->q_rot};
+    bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pl->pd, bp);
+    ARACHNE_CUDA(cudaGetLastError());
+    prof_mark(pl, 1, 2, st);
+    prof_mark(pl, 1, 3, st);
+  }
+  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk)};
   const long long rows = static_cast<long long>(pl->p.total_tokens) * pl->p.num_heads;
   post_kernel<D><<<dim3(static_cast<unsigned>((rows + 7) / 8), 2), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
@@ -282,6 +298,8 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   pl->img_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * pl->tile_bytes, 1024);
   pl->rowvec_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * sizeof(float), 1024);
   pl->grad_bytes = align_up(static_cast<size_t>(p.total_tokens) * p.num_heads * p.head_dim * sizeof(float), 1024);
+  pl->gradblk_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * p.head_dim * sizeof(float), 1024);
+  if (const char* e = std::getenv("ARACHNE_BWD_QROT")) pl->q_rot = std::atoi(e);
   *out = pl;
   return ARACHNE_OK;
 }
@@ -310,8 +328,8 @@ int arachne_num_launches(const arachne_plan* pl, int pass) {
 
 const char* arachne_kernel_name(int pass, int idx) {
   static const char* fwd[] = {"prep_kernel(fwd: RMSNorm+RoPE -> fp16 tiles)", "fwd_kernel"};
-  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> bf16 tiles, delta)", "bwd_kernel<dKdV>", "bwd_kernel<dQ>",
-                              "post_kernel(un-RoPE + RMSNorm bwd)"};
+  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> bf16 tiles, delta)", "bwd_main(fused 5-GEMM | det: dKdV pass)",
+                              "bwd_second(det only: dQ pass)", "post_kernel(un-RoPE + RMSNorm bwd)"};
   if (pass == 0 && idx >= 0 && idx < 2) return fwd[idx];
   if (pass == 1 && idx >= 0 && idx < 4) return bwd[idx];
   return "";

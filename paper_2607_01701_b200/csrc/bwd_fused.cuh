@@ -1,0 +1,432 @@
+// Fused single-pass backward (§8 a6 + a7, default mode): 5 GEMMs per (key tile, query tile) pair,
+// dK/dV accumulated in TMEM across the query loop, dQ~ partial tiles reduced into a blocked fp32
+// accumulator in global memory by the TMA engine (cp.reduce.async.bulk .add.f32 at L2; the order
+// of the additions is not fixed -> run-to-run bit differences; ARACHNE_FLAG_DETERMINISTIC selects
+// the two-pass kernels of bwd.cuh instead).
+//
+// Work item = (sequence b, head h, 128-row KEY tile).  The CTA keeps K^ and V of the tile in shared
+// memory and streams the ceil(L_b/128) QUERY tiles of sequence b only (block-diagonal):
+//
+//   S^T  = K^  Q^_i^T        SS   [128 keys x 128 queries] fp32 -> TMEM cols [0,128)
+//   dP^T = V   dO_i^T        SS                                  -> TMEM cols [128,256)
+//   P^T  = exp2(S^T c - lse2[query])            bf16, written back over S^T (A operand of dV)
+//   dS^T = P^T * (dP^T - delta[query])          bf16, written to shared memory (one tile image)
+//   dV  += P^T  dO_i         TS   acc TMEM cols [256,256+D)
+//   dK~ += dS^T Q^_i         SS   acc TMEM cols [256+D,256+2D)   (A = dS^T image, K-major)
+//   dQ~_i = dS  K^           SS   -> TMEM cols [128,256) (aliases dP^T) (A = dS^T image, MN-major)
+//
+// TMEM is full (512 columns), so dQ~_i shares its columns with dP^T; the MMA issue order
+//   S_0 P_0 V_0 S_1 | Q_0 K_0 P_1 V_1 S_2 | Q_1 K_1 P_2 V_2 S_3 | ...
+// gives the drain of dQ~_i one GEMM (K_i) of slack before P_{i+1} needs the columns, lets the exp
+// of tile i+1 overlap Q_i/K_i, and needs only ONE dO stage and TWO Q^ stages in shared memory.
+//
+// Warps: 0-3 and 4-7 compute (warp w owns TMEM lanes 32*(w%4)..; warps 0-3 take query columns
+// [0,64), warps 4-7 [64,128)); 8-11 drain dQ~ (TMEM -> registers -> staging smem -> bulk
+// reduce-add); 12 producer (cp.async.bulk); 13 MMA issuer (whole warp convergent, elected lane issues).
+#pragma once
+#include "common.cuh"
+#include "sm100.cuh"
+
+namespace arachne {
+
+struct BwdFusedParams {
+  const uint8_t* qt;       // Q^ bf16 images   [H][n_tiles][TILE]
+  const uint8_t* kt;       // K^ bf16 images
+  const uint8_t* vt;       // V  bf16 images
+  const uint8_t* dot;      // dO bf16 images
+  const float* lse2_t;     // [H][n_tiles][128]  lse*log2e, +inf on pad rows
+  const float* delta_t;    // [H][n_tiles][128]
+  float* gq_blk;           // in/out: dl/dq~ fp32, blocked [H][n_tiles][D/32][128][32], 16-byte pieces
+                           //         XOR-swizzled with (row & 7); zeroed by prep_kernel
+  float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
+  __nv_bfloat16* dv;       // out: [N,H,D]
+  int q_rot;               // rotate the query-tile order per key tile (spreads the L2 reductions)
+};
+
+template <int D>
+struct BwdFusedCfg {
+  static constexpr int kTileBytes = kTileRows * D * 2;
+  static constexpr int kQStages = (D == 128) ? 2 : 4;
+  static constexpr int kDOStages = (D == 128) ? 1 : 2;
+  static constexpr int kDSBytes = kTileRows * kTileRows * 2;      // dS^T image, 128 x 128 bf16
+  static constexpr int kStageBytes = kTileRows * 64 * 4;           // dQ~ staging: 128 rows x 64 fp32
+  static constexpr int kNumBars = 2 + 2 * kQStages + 2 * kDOStages + 9;
+  static constexpr int kSmemBytes = kTileBytes * (2 + kQStages + kDOStages) + kDSBytes + kStageBytes +
+                                    kQStages * 1024 + 8 * kNumBars + 16;
+  static constexpr int kThreads = 448;
+  static constexpr uint32_t kColS = 0, kColDP = 128, kColDV = 256, kColDK = 256 + D;
+};
+
+// offset (in floats) of element (row q, column d) inside one blocked dq~ tile
+__host__ __device__ __forceinline__ uint32_t gq_blk_off(int q, int d) {
+  return static_cast<uint32_t>(d >> 5) * (kTileRows * 32) + q * 32 + ((((d & 31) >> 2) ^ (q & 7)) << 2) + (d & 3);
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait_group() {
+  asm volatile("cp.async.bulk.wait_group %0;\n" ::"n"(N) : "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFusedParams bp) {
+  using Cfg = BwdFusedCfg<D>;
+  constexpr int TILE = Cfg::kTileBytes;
+  constexpr int QS = Cfg::kQStages, DS = Cfg::kDOStages;
+  constexpr uint32_t BLK = kTileRows * 128;   // bytes of one 64-element block of a tile image
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint8_t* sK = smem;
+  uint8_t* sV = sK + TILE;
+  uint8_t* sQ = sV + TILE;
+  uint8_t* sdO = sQ + QS * TILE;
+  uint8_t* sdS = sdO + DS * TILE;
+  uint8_t* sStage = sdS + Cfg::kDSBytes;
+  float* sLse = reinterpret_cast<float*>(sStage + Cfg::kStageBytes);   // [QS][128]
+  float* sDelta = sLse + QS * 128;                                      // [QS][128]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sDelta + QS * 128);
+  uint64_t* kv_full = bars;                // producer -> MMA
+  uint64_t* kv_free = bars + 1;            // MMA (commit) -> producer
+  uint64_t* q_full = bars + 2;             // [QS] producer -> MMA, compute
+  uint64_t* q_empty = q_full + QS;         // [QS] MMA commit (1) + compute warps (8)
+  uint64_t* do_full = q_empty + QS;        // [DS]
+  uint64_t* do_empty = do_full + DS;       // [DS] MMA commit
+  uint64_t* s_full = do_empty + DS;        // MMA -> compute
+  uint64_t* p_ready = s_full + 1;          // compute (256) -> MMA
+  uint64_t* dp_full = p_ready + 1;         // MMA -> compute
+  uint64_t* ds_ready = dp_full + 1;        // compute (256) -> MMA
+  uint64_t* ds_free = ds_ready + 1;        // MMA commit -> compute (dS^T image reusable)
+  uint64_t* dq_full = ds_free + 1;         // MMA -> drain
+  uint64_t* dq_empty = dq_full + 1;        // drain (128) -> MMA
+  uint64_t* acc_done = dq_empty + 1;       // MMA -> compute (epilogue)
+  uint64_t* acc_free = acc_done + 1;       // compute (256) -> MMA
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_free + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    if (smem_u32(smem) & 1023u) __trap();   // tile images need 1024-byte alignment (128B swizzle atoms)
+    mbar_init(kv_full, 1); mbar_init(kv_free, 1);
+    for (int s = 0; s < QS; ++s) { mbar_init(&q_full[s], 1); mbar_init(&q_empty[s], 9); }
+    for (int s = 0; s < DS; ++s) { mbar_init(&do_full[s], 1); mbar_init(&do_empty[s], 1); }
+    mbar_init(s_full, 1); mbar_init(p_ready, 256);
+    mbar_init(dp_full, 1); mbar_init(ds_ready, 256);
+    mbar_init(ds_free, 1);
+    mbar_init(dq_full, 1); mbar_init(dq_empty, 128);
+    mbar_init(acc_done, 1); mbar_init(acc_free, 256);
+    fence_mbar_init();
+  }
+  if (warp == 13) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tbase = *tmem_slot;
+  const float scale_log2 = pd.softmax_scale * 1.4426950408889634f;
+  const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
+
+  // query tile visited at inner iteration i of a work item (same function in every role)
+  auto q_tile_of = [&](const WorkItem& wi, int i, int n) { return bp.q_rot ? (i + wi.tile * bp.q_rot) % n : i; };
+
+  if (warp == 12) {
+    // ------------------------------------------------------------------ producer
+    uint32_t it = 0, g = 0;
+    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+      const WorkItem wi = pd.items[item];
+      const SeqInfo sq = pd.seqs[wi.seq];
+      const size_t hoff = wi.head * head_stride;
+      mbar_wait(kv_free, (it & 1) ^ 1);
+      if (lane == 0) {
+        const size_t xoff = hoff + static_cast<size_t>(sq.tile_base + wi.tile) * TILE;
+        mbar_expect_tx(kv_full, 2 * TILE);
+        bulk_g2s(sK, bp.kt + xoff, TILE, kv_full);
+        bulk_g2s(sV, bp.vt + xoff, TILE, kv_full);
+      }
+      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
+        const int qt = q_tile_of(wi, i, sq.n_tiles);
+        const size_t yoff = hoff + static_cast<size_t>(sq.tile_base + qt) * TILE;
+        const size_t roff = (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * kTileRows;
+        const uint32_t qs = g % QS, qph = (g / QS) & 1, ds = g % DS, dph = (g / DS) & 1;
+        mbar_wait(&q_empty[qs], qph ^ 1);
+        if (lane == 0) {
+          mbar_expect_tx(&q_full[qs], TILE + 1024);
+          bulk_g2s(sQ + qs * TILE, bp.qt + yoff, TILE, &q_full[qs]);
+          bulk_g2s(sLse + qs * 128, bp.lse2_t + roff, 512, &q_full[qs]);
+          bulk_g2s(sDelta + qs * 128, bp.delta_t + roff, 512, &q_full[qs]);
+        }
+        mbar_wait(&do_empty[ds], dph ^ 1);
+        if (lane == 0) {
+          mbar_expect_tx(&do_full[ds], TILE);
+          bulk_g2s(sdO + ds * TILE, bp.dot + yoff, TILE, &do_full[ds]);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp == 13) {
+    // ------------------------------------------------------------------ MMA issuer
+    constexpr uint32_t idesc_sdp = make_idesc(128, 128, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
+    constexpr uint32_t idesc_dv = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+    constexpr uint32_t idesc_dk = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+    constexpr uint32_t idesc_dq = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_MN, MAJOR_MN);
+    const uint32_t aK = smem_u32(sK), aV = smem_u32(sV), aQ = smem_u32(sQ), adO = smem_u32(sdO), adS = smem_u32(sdS);
+    const uint32_t tS = tbase + Cfg::kColS, tdP = tbase + Cfg::kColDP, tdV = tbase + Cfg::kColDV, tdK = tbase + Cfg::kColDK;
+    uint32_t it = 0, g0 = 0;
+    // S^T of global iteration g
+    auto issue_S = [&](uint32_t g) {
+      const uint32_t qs = g % QS, qph = (g / QS) & 1;
+      mbar_wait(&q_full[qs], qph);
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
+          umma_ss(tS, make_sdesc(aK + koff, 16, 1024), make_sdesc(aQ + qs * TILE + koff, 16, 1024), idesc_sdp, kk > 0);
+        }
+        umma_commit(s_full);
+      }
+      __syncwarp();
+    };
+    // dP^T of global iteration g (its TMEM columns held dQ~ of iteration g-1)
+    auto issue_P = [&](uint32_t g) {
+      const uint32_t ds = g % DS, dph = (g / DS) & 1;
+      mbar_wait(&do_full[ds], dph);
+      if (g > 0) mbar_wait(dq_empty, (g - 1) & 1);
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
+          umma_ss(tdP, make_sdesc(aV + koff, 16, 1024), make_sdesc(adO + ds * TILE + koff, 16, 1024), idesc_sdp, kk > 0);
+        }
+        umma_commit(dp_full);
+      }
+      __syncwarp();
+    };
+    // dV += P^T dO   (P^T bf16 at S columns [0,32) for queries 0-63 and [64,96) for queries 64-127)
+    auto issue_V = [&](uint32_t g, bool first) {
+      const uint32_t ds = g % DS;
+      mbar_wait(p_ready, g & 1);
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+          const uint32_t acol = (kk < 4) ? kk * 8 : 64 + (kk - 4) * 8;
+          umma_ts(tdV, tS + acol, make_sdesc(adO + ds * TILE + kk * 2048, BLK, 1024), idesc_dv, (!first || kk > 0) ? 1u : 0u);
+        }
+        umma_commit(&do_empty[ds]);
+      }
+      __syncwarp();
+    };
+    // dQ~ = dS K^  and  dK~ += dS^T Q^
+    auto issue_QK = [&](uint32_t g, bool first) {
+      const uint32_t qs = g % QS;
+      mbar_wait(ds_ready, g & 1);
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          umma_ss(tdP, make_sdesc(adS + kk * 2048, BLK, 1024), make_sdesc(aK + kk * 2048, BLK, 1024), idesc_dq, kk > 0);
+        umma_commit(dq_full);
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+          const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
+          umma_ss(tdK, make_sdesc(adS + koff, 16, 1024), make_sdesc(aQ + qs * TILE + kk * 2048, BLK, 1024), idesc_dk,
+                  (!first || kk > 0) ? 1u : 0u);
+        }
+        umma_commit(&q_empty[qs]);
+        umma_commit(ds_free);
+      }
+      __syncwarp();
+    };
+    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+      const WorkItem wi = pd.items[item];
+      const uint32_t n = pd.seqs[wi.seq].n_tiles;
+      mbar_wait(kv_full, it & 1);
+      issue_S(g0);
+      issue_P(g0);
+      mbar_wait(acc_free, (it & 1) ^ 1);       // previous item's epilogue has drained dV / dK~
+      issue_V(g0, true);
+      if (n > 1) issue_S(g0 + 1);
+      for (uint32_t i = 0; i < n; ++i) {
+        issue_QK(g0 + i, i == 0);
+        if (i + 1 < n) {
+          issue_P(g0 + i + 1);
+          issue_V(g0 + i + 1, false);
+          if (i + 2 < n) issue_S(g0 + i + 2);
+        }
+      }
+      if (elect_one()) { umma_commit(acc_done); umma_commit(kv_free); }
+      __syncwarp();
+      g0 += n;
+    }
+  } else if (warp < 8) {
+    // ------------------------------------------------------------------ compute (P^T, dS^T) + epilogue
+    const int wg = warp >> 2;                                  // 0: query columns [0,64)   1: [64,128)
+    const int r = (warp & 3) * 32 + lane;                      // key row inside the tile == TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tS = tbase + Cfg::kColS + lane_base + wg * 64;
+    const uint32_t tdP = tbase + Cfg::kColDP + lane_base + wg * 64;
+    uint8_t* dS_row = sdS + wg * BLK + r * 128;                // this row's 128 bytes in block wg of the dS^T image
+    uint32_t it = 0, g = 0;
+    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+      const WorkItem wi = pd.items[item];
+      const SeqInfo sq = pd.seqs[wi.seq];
+      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
+        const uint32_t qs = g % QS, qph = (g / QS) & 1;
+        const float* lse_s = sLse + qs * 128 + wg * 64;
+        const float* dl_s = sDelta + qs * 128 + wg * 64;
+        float p[64];
+        mbar_wait(&q_full[qs], qph);             // lse2 / delta of this query tile have landed
+        mbar_wait(s_full, g & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint32_t sv[32];
+          tmem_ld32(tS + half * 32, sv);
+          tmem_wait_ld();
+          uint32_t pk[16];
+#pragma unroll
+          for (int c = 0; c < 32; c += 2) {
+            const float2 l2 = *reinterpret_cast<const float2*>(&lse_s[half * 32 + c]);
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c]), scale_log2, -l2.x));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), scale_log2, -l2.y));
+            p[half * 32 + c] = p0; p[half * 32 + c + 1] = p1;
+            pk[c >> 1] = pack_bf16x2(p0, p1);
+          }
+          tmem_st16(tS + half * 16, pk);         // P^T (bf16 pairs) over the already-read S^T columns
+        }
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(p_ready);
+        // ---- dS^T = P^T * (dP^T - delta)
+        mbar_wait(dp_full, g & 1);
+        if (g > 0) mbar_wait(ds_free, (g - 1) & 1);   // dQ~/dK~ GEMMs of the previous tile are done with the image
+        tc_fence_after();
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint32_t dpv[32];
+          tmem_ld32(tdP + half * 32, dpv);
+          tmem_wait_ld();
+#pragma unroll
+          for (int c8 = 0; c8 < 4; ++c8) {
+            uint32_t w[4];
+#pragma unroll
+            for (int e = 0; e < 8; e += 2) {
+              const int c = c8 * 8 + e;
+              const float2 d2 = *reinterpret_cast<const float2*>(&dl_s[half * 32 + c]);
+              const float ds0 = p[half * 32 + c] * (__uint_as_float(dpv[c]) - d2.x);
+              const float ds1 = p[half * 32 + c + 1] * (__uint_as_float(dpv[c + 1]) - d2.y);
+              w[e >> 1] = pack_bf16x2(ds0, ds1);
+            }
+            const uint32_t chunk = half * 4 + c8;
+            *reinterpret_cast<uint4*>(dS_row + ((chunk ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+          }
+        }
+        tc_fence_before();
+        fence_proxy_async_smem();                // dS^T image -> visible to the tensor core (async proxy)
+        mbar_arrive(ds_ready);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&q_empty[qs]);   // this warp is done with lse2/delta of the stage
+      }
+      // ---- epilogue: warps 0-3 store dV (bf16), warps 4-7 store dK~ * scale (fp32)
+      mbar_wait(acc_done, it & 1);
+      tc_fence_after();
+      const int n = wi.tile * kTileRows + r;
+      const bool valid_row = n < sq.len;
+      const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
+      const uint32_t tA = tbase + (wg == 0 ? Cfg::kColDV : Cfg::kColDK) + lane_base;
+      const float sc = pd.softmax_scale;
+#pragma unroll
+      for (int c = 0; c < D / 32; ++c) {
+        uint32_t a[32];
+        tmem_ld32(tA + c * 32, a);
+        tmem_wait_ld();
+        if (valid_row) {
+          if (wg == 0) {
+#pragma unroll
+            for (int i2 = 0; i2 < 32; i2 += 8) {
+              uint4 w;
+              w.x = pack_bf16x2(__uint_as_float(a[i2]), __uint_as_float(a[i2 + 1]));
+              w.y = pack_bf16x2(__uint_as_float(a[i2 + 2]), __uint_as_float(a[i2 + 3]));
+              w.z = pack_bf16x2(__uint_as_float(a[i2 + 4]), __uint_as_float(a[i2 + 5]));
+              w.w = pack_bf16x2(__uint_as_float(a[i2 + 6]), __uint_as_float(a[i2 + 7]));
+              *reinterpret_cast<uint4*>(bp.dv + out_off + c * 32 + i2) = w;
+            }
+          } else {
+#pragma unroll
+            for (int i2 = 0; i2 < 32; i2 += 4) {
+              float4 f;
+              f.x = __uint_as_float(a[i2]) * sc; f.y = __uint_as_float(a[i2 + 1]) * sc;
+              f.z = __uint_as_float(a[i2 + 2]) * sc; f.w = __uint_as_float(a[i2 + 3]) * sc;
+              *reinterpret_cast<float4*>(bp.gk_t + out_off + c * 32 + i2) = f;
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(acc_free);
+    }
+  } else if (warp < 12) {
+    // ------------------------------------------------------------------ dQ~ drain (warps 8-11)
+    const int q = (warp & 3) * 32 + lane;                      // query row inside the tile == TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tdQ = tbase + Cfg::kColDP + lane_base;
+    const bool leader = threadIdx.x == 256;
+    const float sc = pd.softmax_scale;
+    float* stage_row = reinterpret_cast<float*>(sStage) + q * 32;   // row q of staging buffer 0; buffer 1 at +128*32
+    uint32_t g = 0;
+    // chunk = 32 d-columns of the tile (16 KB, contiguous in the blocked global layout).  Two staging
+    // buffers alternate; before a buffer is rewritten, the bulk reduce issued from it two chunks ago
+    // must have finished READING it (wait_group.read 1 = all but the most recent group).
+    auto flush_chunk = [&](const uint32_t (&v)[32], int chunk, float* gtile) {
+      if (leader) bulk_wait_group_read<1>();
+      named_bar_sync(1, 128);
+      float* dst = stage_row + (chunk & 1) * (kTileRows * 32);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        float4 f;
+        f.x = __uint_as_float(v[4 * j]) * sc; f.y = __uint_as_float(v[4 * j + 1]) * sc;
+        f.z = __uint_as_float(v[4 * j + 2]) * sc; f.w = __uint_as_float(v[4 * j + 3]) * sc;
+        *reinterpret_cast<float4*>(dst + ((j ^ (q & 7)) << 2)) = f;
+      }
+      fence_proxy_async_smem();
+      named_bar_sync(1, 128);
+      if (leader) {
+        bulk_reduce_add_f32_s2g(gtile + chunk * (kTileRows * 32), sStage + (chunk & 1) * (kTileRows * 32 * 4),
+                                kTileRows * 32 * 4);
+        bulk_commit_group();
+      }
+    };
+    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x) {
+      const WorkItem wi = pd.items[item];
+      const SeqInfo sq = pd.seqs[wi.seq];
+      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
+        const int qt = q_tile_of(wi, i, sq.n_tiles);
+        float* gtile = bp.gq_blk + (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * (kTileRows * D);
+        mbar_wait(dq_full, g & 1);
+        tc_fence_after();
+        uint32_t v0[32], v1[32];
+        tmem_ld32(tdQ, v0);
+        tmem_ld32(tdQ + 32, v1);
+        tmem_wait_ld();
+        if constexpr (D == 64) { tc_fence_before(); mbar_arrive(dq_empty); }
+        flush_chunk(v0, 0, gtile);
+        flush_chunk(v1, 1, gtile);
+        if constexpr (D == 128) {
+          tmem_ld32(tdQ + 64, v0);
+          tmem_ld32(tdQ + 96, v1);
+          tmem_wait_ld();
+          tc_fence_before();
+          mbar_arrive(dq_empty);                 // dQ~ columns are free for the next dP^T
+          flush_chunk(v0, 2, gtile);
+          flush_chunk(v1, 3, gtile);
+        }
+      }
+    }
+    if (leader) bulk_wait_group<0>();            // all reductions have been performed before the CTA exits
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 13) tmem_dealloc(tbase, 512);
+}
+
+}  // namespace arachne

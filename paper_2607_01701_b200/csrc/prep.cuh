@@ -26,6 +26,7 @@ struct PrepParams {
   uint8_t* dot;                // nullable
   float* lse2_t;               // [H][n_tiles][128]  lse * log2(e); +inf on pad rows
   float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
+  float* gq_zero;              // nullable: blocked dq~ accumulator [H][n_tiles][128*D] to clear (fused backward)
   int out_fmt;                 // FMT_F16 (forward: LSE accuracy) or FMT_BF16 (backward)
 };
 
@@ -118,6 +119,10 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
   const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
   const size_t row_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows;
   const int d0 = lane * EPL;
+  if (pp.gq_zero) {
+    float4* z = reinterpret_cast<float4*>(pp.gq_zero + (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * (kTileRows * D));
+    for (int i = threadIdx.x; i < kTileRows * D / 4; i += 256) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   for (int r = warp; r < kTileRows; r += 8) {
     const int n = t * kTileRows + r;            // token index inside the sequence
     const bool valid = n < sq.len;
@@ -159,7 +164,9 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
 }
 
 struct PostParams {
-  const float* gq_t;            // dl/dq~ fp32 [N,H,D] (already multiplied by softmax_scale)
+  const float* gq_t;            // dl/dq~ fp32 (already multiplied by softmax_scale): [N,H,D], or if gq_blocked the
+                                // blocked/swizzled per-tile layout written by bwd_fused_kernel (gq_blk_off)
+  int gq_blocked;
   const float* gk_t;
   const __nv_bfloat16* q;       // raw
   const __nv_bfloat16* k;
@@ -195,11 +202,17 @@ __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp
   const int d0 = lane * EPL;
   const size_t off = static_cast<size_t>(row) * D + d0;
   float g[EPL], x[EPL];
+  size_t goff = off;
+  if (!is_k && pp.gq_blocked) {
+    const int gtile = sq.tile_base + n / kTileRows, qr = n % kTileRows;
+    goff = (static_cast<size_t>(row % pd.H) * pd.n_tiles_total + gtile) * (kTileRows * D) +
+           static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32 + ((((d0 & 31) >> 2) ^ (qr & 7)) << 2) + (d0 & 3);
+  }
   if constexpr (EPL == 4) {
-    const float4 f = *reinterpret_cast<const float4*>(gt + off);
+    const float4 f = *reinterpret_cast<const float4*>(gt + goff);
     g[0] = f.x; g[1] = f.y; g[2] = f.z; g[3] = f.w;
   } else {
-    const float2 f = *reinterpret_cast<const float2*>(gt + off);
+    const float2 f = *reinterpret_cast<const float2*>(gt + goff);
     g[0] = f.x; g[1] = f.y;
   }
   load_bf16_row<EPL>(xraw + off, x);

@@ -87,8 +87,10 @@ def test_large_gamma_rescale_path(orc):
     got = pu.run_gpu(st, t, gamma_q=g, gamma_k=g)
     a = _np(t)
     ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], gamma_q=g, gamma_k=g)
-    # attention is nearly one-hot here; bf16 P/dS rounding dominates -> same gates
-    pu.check_full(st, got, ref)
+    # attention is nearly one-hot here; bf16 P/dS rounding dominates -> same gates, except LSE: the fp16
+    # rounding of q^, k^ perturbs every logit by ~|s|*2^-11, and |s| scales with gamma_q*gamma_k = 4, so the
+    # LSE gate (1e-3, stated for gamma = 1) is scaled by the same factor.
+    pu.check_full(st, got, ref, tol=dict(pu.TOL, LSE_abs=4e-3))
 
 
 # ------------------------------------------------------------------ block-diagonality on the GPU path
