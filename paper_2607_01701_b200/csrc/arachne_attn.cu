@@ -53,6 +53,8 @@ struct arachne_plan {
   SeqInfo* d_seqs = nullptr;
   int* d_tile_seq = nullptr;
   WorkItem* d_items = nullptr;
+  WorkItem* d_fwd_items = nullptr;
+  int n_fwd_items = 0;
   int* d_counter = nullptr;
   float2* d_rope = nullptr;
   ProblemDesc pd{};
@@ -106,8 +108,8 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
   FwdParams fp{f.qt, f.kt, f.vt, static_cast<__nv_bfloat16*>(o), lse};
-  const int grid = std::min(pl->num_sms, pl->n_items);
-  fwd_kernel<D><<<grid, 192, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
+  const int grid = std::min(pl->num_sms, pl->n_fwd_items);
+  fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
   if (pl->profiling) pl->prof_calls[0]++;
@@ -256,6 +258,13 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   for (int b : order)
     for (int h = 0; h < p.num_heads; ++h)
       for (int t = 0; t < pl->seqs[b].n_tiles; ++t) items.push_back(WorkItem{b, h, t, 0});
+  // forward items: pairs of adjacent query tiles (two tiles ping-pong on the tensor pipe), same group order
+  std::vector<WorkItem> fwd_items;
+  for (int b : order)
+    for (int h = 0; h < p.num_heads; ++h)
+      for (int t = 0; t < pl->seqs[b].n_tiles; t += 2)
+        fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].n_tiles - t)});
+  pl->n_fwd_items = static_cast<int>(fwd_items.size());
   // RoPE tables in fp64 -> fp32 (readings R4, R5)
   std::vector<float2> tab;
   RopeDesc rd{};
@@ -278,6 +287,7 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   PLAN_UP(pl->d_seqs, pl->seqs, SeqInfo)
   PLAN_UP(pl->d_tile_seq, tile_seq, int)
   PLAN_UP(pl->d_items, items, WorkItem)
+  PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_counter), 4 * sizeof(int))) != cudaSuccess) return fail(e, "cudaMalloc");
@@ -287,7 +297,7 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.sched_counter = pl->d_counter;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.sched_counter = pl->d_counter;
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -310,7 +320,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_counter); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_counter); cudaFree(pl->d_rope);
   delete pl;
 }
 

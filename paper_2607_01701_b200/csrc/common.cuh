@@ -25,7 +25,7 @@ struct WorkItem {
   int seq;
   int head;
   int tile;
-  int pad;
+  int pad;         // forward items: number of query tiles in the item (1 or 2)
 };
 
 // cos/sin tables of the 3D RoPE (readings R4-R6): entry (axis a, position x, pair p) at
@@ -40,6 +40,8 @@ struct ProblemDesc {
   const SeqInfo* seqs;
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
+  const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
+  int n_fwd_items;
   int* sched_counter;        // dynamic tile scheduler: next item to hand out
   int n_items;
   int n_tiles_total;
