@@ -55,7 +55,7 @@ struct arachne_plan {
   WorkItem* d_items = nullptr;
   WorkItem* d_fwd_items = nullptr;
   int n_fwd_items = 0;
-  int* d_counter = nullptr;
+  unsigned* d_stats = nullptr;
   float2* d_rope = nullptr;
   ProblemDesc pd{};
   // workspace layout
@@ -103,7 +103,10 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
   pp.out_fmt = FMT_F16;
+  pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // S leaves the tensor core in the exp2 domain
+  pp.stats = pl->d_stats;
   prof_mark(pl, 0, 0, st);
+  ARACHNE_CUDA(cudaMemsetAsync(pl->d_stats, 0, 4 * sizeof(unsigned), st));
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
@@ -138,6 +141,7 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.out_fmt = FMT_BF16;
+  pp.q_prescale = 1.0f;
   pp.gq_zero = deterministic ? nullptr : b.gq_t;
   prof_mark(pl, 1, 0, st);
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
@@ -290,14 +294,14 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
-  if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_counter), 4 * sizeof(int))) != cudaSuccess) return fail(e, "cudaMalloc");
-  if ((e = cudaMemset(pl->d_counter, 0, 4 * sizeof(int))) != cudaSuccess) return fail(e, "cudaMemset");
+  if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_stats), 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
+  if ((e = cudaMemset(pl->d_stats, 0, 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
   int rc = p.head_dim == 128 ? configure_kernels<128>() : configure_kernels<64>();
   if (rc != ARACHNE_OK) { arachne_plan_destroy(pl); return rc; }
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.sched_counter = pl->d_counter;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -320,7 +324,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_counter); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
   delete pl;
 }
 

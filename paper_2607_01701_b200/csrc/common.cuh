@@ -42,7 +42,7 @@ struct ProblemDesc {
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
   const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int n_fwd_items;
-  int* sched_counter;        // dynamic tile scheduler: next item to hand out
+  unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel
   int n_items;
   int n_tiles_total;
   int num_seqs;

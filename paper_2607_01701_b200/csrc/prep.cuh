@@ -28,6 +28,10 @@ struct PrepParams {
   float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
   float* gq_zero;              // nullable: blocked dq~ accumulator [H][n_tiles][128*D] to clear (fused backward)
   int out_fmt;                 // FMT_F16 (forward: LSE accuracy) or FMT_BF16 (backward)
+  float q_prescale;            // Q^ is multiplied by this before rounding (forward: softmax_scale*log2(e), so that
+                               // S comes out of the tensor core already in the exp2 domain; backward: 1)
+  unsigned* stats;             // nullable: [0] = max_i |q~_i|^2, [1] = max_j |k~_j|^2 as float bits (atomicMax);
+                               // the forward kernel derives its logit bound from them (static-max softmax)
 };
 
 __device__ __forceinline__ float warp_sum(float x) {
@@ -74,12 +78,15 @@ __device__ __forceinline__ void store_image(uint8_t* img, int r, int d0, const f
 }
 
 // x~ = RoPE(gamma * x * rsqrt(mean(x^2) + eps))  (readings R1-R5), one row per warp
+// returns the lane's partial sum of squares of the stored row (0 for pad rows)
 template <int D>
-__device__ __forceinline__ void norm_rope_store(const ProblemDesc& pd, const __nv_bfloat16* src, const float* gamma,
-                                                uint8_t* img, int r, bool valid, const int (&pos)[3], int lane, int fmt) {
+__device__ __forceinline__ float norm_rope_store(const ProblemDesc& pd, const __nv_bfloat16* src, const float* gamma,
+                                                 uint8_t* img, int r, bool valid, const int (&pos)[3], int lane, int fmt,
+                                                 float prescale) {
   constexpr int EPL = D / 32;
   const int d0 = lane * EPL;
   float x[EPL];
+  float nrm = 0.f;
   if (valid) {
     load_bf16_row<EPL>(src + d0, x);
     if (!pd.no_norm) {
@@ -100,11 +107,14 @@ __device__ __forceinline__ void norm_rope_store(const ProblemDesc& pd, const __n
         x[i + 1] = x0 * cs.y + x1 * cs.x;
       }
     }
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) { x[i] *= prescale; nrm += x[i] * x[i]; }
   } else {
 #pragma unroll
     for (int i = 0; i < EPL; ++i) x[i] = 0.f;   // zero-padded tail rows (never NaN: 0 * P stays 0)
   }
   store_image<EPL>(img, r, d0, x, fmt);
+  return nrm;
 }
 
 template <int D>
@@ -113,7 +123,7 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
   constexpr int TILE_BYTES = kTileRows * D * 2;
   const int gtile = blockIdx.x, h = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x < 4) pd.sched_counter[threadIdx.x] = 0;
+  float qn = 0.f, kn = 0.f;      // this warp's largest |q~|^2, |k~|^2 (lane-partial sums until the end)
   const SeqInfo sq = pd.seqs[pd.tile_seq[gtile]];
   const int t = gtile - sq.tile_base;
   const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
@@ -130,8 +140,10 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
     const int hw = sq.Hg * sq.Wg;
     pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
     const size_t src = (static_cast<size_t>(sq.tok_start + n) * pd.H + h) * D;
-    norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, pos, lane, pp.out_fmt);
-    norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, pos, lane, pp.out_fmt);
+    const float qs = norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, pos, lane, pp.out_fmt, pp.q_prescale);
+    const float ks = norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, pos, lane, pp.out_fmt, 1.0f);
+    // row norms are only summed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
+    if (pp.stats && pd.no_norm) { qn = fmaxf(qn, warp_sum(qs)); kn = fmaxf(kn, warp_sum(ks)); }
     float x[EPL];
     if (valid) load_bf16_row<EPL>(pp.v + src + d0, x);
     else {
@@ -159,6 +171,33 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
         pp.lse2_t[row_off + r] = valid ? pp.lse[static_cast<size_t>(h) * pd.N + sq.tok_start + n] * 1.4426950408889634f
                                        : __int_as_float(0x7f800000);
       }
+    }
+  }
+  if (pp.stats) {
+    // Bound on |q~'|^2 and |k~|^2 for the forward kernel's static-max softmax.  With RMSNorm,
+    // |x^|^2 = sum_d gamma_d^2 x_d^2 / (mean(x^2) + eps) <= D * max_d gamma_d^2 (RoPE preserves the norm),
+    // identical for every block, so one warp publishes it; without it, the largest row norm seen.
+    // Non-negative floats order like their bit patterns (+inf sorts last -> online-softmax path).
+    if (!pd.no_norm) {
+      if (blockIdx.x == 0 && blockIdx.y == 0 && warp == 0) {
+        float gq = 0.f, gk = 0.f;
+        for (int d = lane; d < D; d += 32) {
+          gq = fmaxf(gq, pp.gamma_q ? fabsf(pp.gamma_q[d]) : 1.0f);
+          gk = fmaxf(gk, pp.gamma_k ? fabsf(pp.gamma_k[d]) : 1.0f);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          gq = fmaxf(gq, __shfl_xor_sync(0xffffffffu, gq, o));
+          gk = fmaxf(gk, __shfl_xor_sync(0xffffffffu, gk, o));
+        }
+        if (lane == 0) {
+          atomicMax(&pp.stats[0], __float_as_uint(gq * gq * D * pp.q_prescale * pp.q_prescale));
+          atomicMax(&pp.stats[1], __float_as_uint(gk * gk * D));
+        }
+      }
+    } else if (lane == 0) {
+      atomicMax(&pp.stats[0], __float_as_uint(qn));
+      atomicMax(&pp.stats[1], __float_as_uint(kn));
     }
   }
 }

@@ -70,10 +70,12 @@ def test_debug_flags_and_scale(orc):
     a = _np(t)
     ref = orc.attention(a["q"], a["k"], a["v"], st2["cu_seqlens"], st2["grids"], dO=a["dO"], no_norm=True)
     pu.check_full(st2, got, ref)
-    # explicit softmax scale
+    # explicit softmax scale 0.2 = 1.6 x the default 1/sqrt(64): logits are 1.6 x larger, so is the fp16
+    # operand-rounding error of a logit, hence the LSE gate scales by 1.6 (reading R19; an fp64
+    # emulation of "fp16(q^ c) . fp16(k^)" on these bytes gives 1.15e-3, 7.3e-4 with c applied after the dot)
     got = pu.run_gpu(st2, t, plan_kw=dict(softmax_scale=0.2))
     ref = orc.attention(a["q"], a["k"], a["v"], st2["cu_seqlens"], st2["grids"], dO=a["dO"], scale=0.2)
-    pu.check_full(st2, got, ref)
+    pu.check_full(st2, got, ref, tol=dict(pu.TOL, LSE_abs=pu.TOL["LSE_abs"] * 0.2 / 0.125))
 
 
 def test_large_gamma_rescale_path(orc):
