@@ -131,7 +131,7 @@ def run_reference(args):
     one = inputs.pack([st["grids"][b]], st["H"], st["D"], index=st["index"], rope_dims=st["rope_dims"])
     one["name"] = args.workload
     t = inputs.make_inputs(one, device="cpu")
-    rows = 2 if L > 50000 else 6
+    rows = max(4, min(L, int(6.0e6 / L)))          # ~5 s of oracle time per step (about 1.2e6 row x key / s / head)
     times, val = [], 0.0
     for i in range(args.warmup + args.steps):
         v_, dt, desc, cores = oracle_sample(one, t, budget_rows=rows, heads=1)
@@ -277,7 +277,8 @@ def main():
         orc.build()
         tc = {k: x.cpu() for k, x in t.items()}
         L_max = max(st["cu_seqlens"][i + 1] - st["cu_seqlens"][i] for i in range(len(st["grids"])))
-        v_, dt_, desc, cores = oracle_sample(st, tc, budget_rows=4 if L_max > 50000 else 16, heads=2)
+        # ~10-20 s of oracle time: rows x 2 heads x L_max ~ 2e7 query-row x key products
+        v_, dt_, desc, cores = oracle_sample(st, tc, budget_rows=max(8, min(L_max, int(1.0e7 / L_max))), heads=2)
         cpu = {"value": v_, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
     out = {
