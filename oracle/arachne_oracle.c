@@ -20,7 +20,11 @@
  * with torch SDPA (fp64) when norm and RoPE are off, and with a torch fp64 autograd
  * composite when on; closed forms (L=1, Q==0); RMSNorm scale invariance; RoPE norm
  * preservation / shift invariance / axis distinguishability; sum_j dV_j = sum_i dO_i;
- * row-subset + masked-dO mode == full mode restricted.
+ * row-subset + masked-dO mode == full mode restricted.  Joint text tokens (R21): brute force
+ * with its own is-text switch, equality with the no-RoPE run when every token sits at the
+ * origin, torch autograd composite.  dgamma (R22): finite differences in gamma, torch
+ * autograd, and the invariant sum_d gq_d dGq_d == sum_d gk_d dGk_d (the loss is unchanged
+ * by gamma_q -> c gamma_q, gamma_k -> gamma_k / c).
  *
  * One function does one (sequence, head) problem on gathered fp64 arrays; the Python
  * wrapper (oracle/arachne_oracle.py) loops over sequences and heads.  OpenMP over rows /
@@ -62,7 +66,7 @@ static void token_pos(const oracle_cfg* c, const int grid[3], int n, int pos[3])
 
 /* R1-R5: x~ = RoPE(gamma * x / sqrt(mean(x^2) + eps)).  Returns r = 1/sqrt(mean+eps). */
 static double norm_rope_row(const oracle_cfg* c, const double* x, const double* gamma,
-                            const int pos[3], double* xt) {
+                            const int pos[3], int is_text, double* xt) {
   const int D = c->D;
   double r = 1.0;
   if (!c->no_norm) {
@@ -74,7 +78,7 @@ static double norm_rope_row(const oracle_cfg* c, const double* x, const double* 
   } else {
     for (int d = 0; d < D; ++d) xt[d] = x[d];
   }
-  if (!c->no_rope) {                      /* R3: norm, then RoPE                         */
+  if (!c->no_rope && !is_text) {          /* R3: norm, then RoPE; R21: text tokens are not rotated */
     int base = 0;
     for (int a = 0; a < 3; ++a) {         /* R4: contiguous axis slices, order t,h,w     */
       const int da = c->rope_dims[a];
@@ -94,13 +98,15 @@ static double norm_rope_row(const oracle_cfg* c, const double* x, const double* 
 /* Chain rule through norm_rope_row (R12): g~ = dl/dx~  ->  dl/dx.
  *   rotate each pair by -phi:  g0 = g~0 cos + g~1 sin ; g1 = -g~0 sin + g~1 cos
  *   u = gamma * g ;  dx_e = r u_e - r^3 x_e (sum_d u_d x_d) / D
- * (from x^_d = gamma_d x_d r, dr/dx_e = -r^3 x_e / D). */
+ * (from x^_d = gamma_d x_d r, dr/dx_e = -r^3 x_e / D).
+ * dx may be NULL (only the dgamma term wanted). */
 static void norm_rope_row_bwd(const oracle_cfg* c, const double* x, const double* gamma,
-                              const int pos[3], double r, const double* gt, double* dx) {
+                              const int pos[3], int is_text, double r, const double* gt, double* dx,
+                              double* dgamma_row) {
   const int D = c->D;
   double* g = (double*)malloc(sizeof(double) * (size_t)D);
   for (int d = 0; d < D; ++d) g[d] = gt[d];
-  if (!c->no_rope) {
+  if (!c->no_rope && !is_text) {
     int base = 0;
     for (int a = 0; a < 3; ++a) {
       const int da = c->rope_dims[a];
@@ -117,15 +123,25 @@ static void norm_rope_row_bwd(const oracle_cfg* c, const double* x, const double
   if (!c->no_norm) {
     double ux = 0.0;
     for (int d = 0; d < D; ++d) ux += gamma[d] * g[d] * x[d];
-    for (int d = 0; d < D; ++d)
+    if (dx) for (int d = 0; d < D; ++d)
       dx[d] = r * gamma[d] * g[d] - r * r * r * x[d] * ux / (double)D;
+    /* R22: x^_d = gamma_d x_d r  =>  this row's term of dl/dgamma_d is g_d x_d r */
+    if (dgamma_row) for (int d = 0; d < D; ++d) dgamma_row[d] = g[d] * x[d] * r;
   } else {
-    for (int d = 0; d < D; ++d) dx[d] = g[d];
+    if (dx) for (int d = 0; d < D; ++d) dx[d] = g[d];
+    if (dgamma_row) for (int d = 0; d < D; ++d) dgamma_row[d] = 0.0;   /* gamma unused */
   }
   free(g);
 }
 
 /* One (sequence, head) problem.
+ *   R21 (joint text tokens; "hybrid dual/single-stream", PAPER.md:201
+ *   text < 256 tokens): the sequence is the T*Hg*Wg video tokens of `grid` in row-major order followed by
+ *   n_text text tokens (L = T*Hg*Wg + n_text).  Text tokens get the same QK-RMSNorm but NO RoPE; attention
+ *   is full (bidirectional) over all L tokens.
+ *   R22 (dgamma, NEXT-1): dGq[d] / dGk[d] = sum over the query / key rows of this problem of
+ *   (R^T g~)_d x_d r, i.e. dl/dgamma_q, dl/dgamma_k restricted to this (sequence, head); the caller sums
+ *   over sequences and heads (gamma is shared by all heads, R1).  Either may be NULL.
  *   L keys/values (all tokens 0..L-1 of the sequence), R query rows with in-sequence
  *   token indices qidx[0..R) (R == L and qidx[i] == i for the full problem).
  *   q  [R][D] raw query rows,   k, v [L][D] raw keys / values,   dO [R][D] or NULL.
@@ -135,12 +151,15 @@ static void norm_rope_row_bwd(const oracle_cfg* c, const double* x, const double
  *   dK, dV [L][D] = contributions of the given R rows only (== exact when R == L; this is
  *   the "masked-dO" quantity when R < L: dO is zero outside the row set).
  * Returns 0, or -1 on allocation failure / bad arguments. */
-int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, const int* qidx,
-                        const double* q, const double* k, const double* v,
-                        const double* gamma_q, const double* gamma_k, const double* dO,
-                        double* O, double* LSE, double* P, double* dQ, double* dK, double* dV) {
+int arachne_oracle_head_joint(const oracle_cfg* c, const int grid[3], int n_text, int L, int R,
+                              const int* qidx, const double* q, const double* k, const double* v,
+                              const double* gamma_q, const double* gamma_k, const double* dO,
+                              double* O, double* LSE, double* P, double* dQ, double* dK, double* dV,
+                              double* dGq, double* dGk) {
   const int D = c->D;
-  if (L < 1 || R < 1 || grid[0] * grid[1] * grid[2] != L) return -1; /* R16: L_b >= 1 */
+  const int Lvid = grid[0] * grid[1] * grid[2];
+  if (L < 1 || R < 1 || n_text < 0 || grid[0] < 0 || grid[1] < 1 || grid[2] < 1 || Lvid + n_text != L)
+    return -1;                                        /* R16: L_b >= 1; a text-only sequence has T = 0 */
   const int need_bwd = (dO != NULL);
   double* kt = (double*)malloc(sizeof(double) * (size_t)L * D);   /* k~_j */
   double* rk = (double*)malloc(sizeof(double) * (size_t)L);
@@ -149,8 +168,12 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
   double* Pm = (double*)malloc(sizeof(double) * (size_t)R * L);   /* P_ij */
   double* dS = need_bwd ? (double*)malloc(sizeof(double) * (size_t)R * L) : NULL;
   double* Oi = (double*)malloc(sizeof(double) * (size_t)R * D);
-  if (!kt || !rk || !qt || !rq || !Pm || !Oi || (need_bwd && !dS)) {
-    free(kt); free(rk); free(qt); free(rq); free(Pm); free(dS); free(Oi);
+  /* per-row dgamma terms (summed serially afterwards: no cross-thread reduction) */
+  double* dgq_rows = (need_bwd && dGq) ? (double*)malloc(sizeof(double) * (size_t)R * D) : NULL;
+  double* dgk_rows = (need_bwd && dGk) ? (double*)malloc(sizeof(double) * (size_t)L * D) : NULL;
+  if (!kt || !rk || !qt || !rq || !Pm || !Oi || (need_bwd && !dS) || (need_bwd && dGq && !dgq_rows) ||
+      (need_bwd && dGk && !dgk_rows)) {
+    free(kt); free(rk); free(qt); free(rq); free(Pm); free(dS); free(Oi); free(dgq_rows); free(dgk_rows);
     return -1;
   }
 
@@ -159,7 +182,7 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
   for (int j = 0; j < L; ++j) {
     int pos[3];
     token_pos(c, grid, j, pos);
-    rk[j] = norm_rope_row(c, k + (size_t)j * D, gamma_k, pos, kt + (size_t)j * D);
+    rk[j] = norm_rope_row(c, k + (size_t)j * D, gamma_k, pos, j >= Lvid, kt + (size_t)j * D);
   }
 
   /* step 2: per query row — scores, softmax, LSE, O (R8, R9, R11: no mask inside a sequence) */
@@ -168,7 +191,7 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
     int pos[3];
     token_pos(c, grid, qidx[i], pos);
     double* qti = qt + (size_t)i * D;
-    rq[i] = norm_rope_row(c, q + (size_t)i * D, gamma_q, pos, qti);
+    rq[i] = norm_rope_row(c, q + (size_t)i * D, gamma_q, pos, qidx[i] >= Lvid, qti);
     double* Pi = Pm + (size_t)i * L;
     double m = -INFINITY;
     for (int j = 0; j < L; ++j) {
@@ -211,7 +234,9 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
         for (int d = 0; d < D; ++d) gq[d] += ds * ktj[d];
       }
       for (int d = 0; d < D; ++d) gq[d] *= c->scale;
-      if (dQ) norm_rope_row_bwd(c, q + (size_t)i * D, gamma_q, pos, rq[i], gq, dQ + (size_t)i * D);
+      if (dQ || dgq_rows)
+        norm_rope_row_bwd(c, q + (size_t)i * D, gamma_q, pos, qidx[i] >= Lvid, rq[i], gq,
+                          dQ ? dQ + (size_t)i * D : NULL, dgq_rows ? dgq_rows + (size_t)i * D : NULL);
       free(gq);
     }
   }
@@ -219,7 +244,7 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
   if (P) memcpy(P, Pm, sizeof(double) * (size_t)R * L);
 
   /* step 4: per key — dV_j = sum_i P_ij dO_i ; dk~_j = scale * sum_i dS_ij q~_i -> dK_j */
-  if (need_bwd && (dK || dV)) {
+  if (need_bwd && (dK || dV || dgk_rows)) {
 #pragma omp parallel for schedule(static)
     for (int j = 0; j < L; ++j) {
       double* gv = (double*)malloc(sizeof(double) * 2 * (size_t)D);
@@ -232,23 +257,42 @@ int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, co
         for (int d = 0; d < D; ++d) { gv[d] += p * doi[d]; gk[d] += ds * qti[d]; }
       }
       if (dV) memcpy(dV + (size_t)j * D, gv, sizeof(double) * (size_t)D);
-      if (dK) {
+      if (dK || dgk_rows) {
         int pos[3];
         token_pos(c, grid, j, pos);
         for (int d = 0; d < D; ++d) gk[d] *= c->scale;
-        norm_rope_row_bwd(c, k + (size_t)j * D, gamma_k, pos, rk[j], gk, dK + (size_t)j * D);
+        norm_rope_row_bwd(c, k + (size_t)j * D, gamma_k, pos, j >= Lvid, rk[j], gk,
+                          dK ? dK + (size_t)j * D : NULL, dgk_rows ? dgk_rows + (size_t)j * D : NULL);
       }
       free(gv);
     }
   }
-  free(kt); free(rk); free(qt); free(rq); free(Pm); free(dS); free(Oi);
+  /* R22: dl/dgamma = sum of the per-row terms, rows in index order */
+  if (dgq_rows) {
+    for (int d = 0; d < D; ++d) dGq[d] = 0.0;
+    for (int i = 0; i < R; ++i) for (int d = 0; d < D; ++d) dGq[d] += dgq_rows[(size_t)i * D + d];
+  }
+  if (dgk_rows) {
+    for (int d = 0; d < D; ++d) dGk[d] = 0.0;
+    for (int j = 0; j < L; ++j) for (int d = 0; d < D; ++d) dGk[d] += dgk_rows[(size_t)j * D + d];
+  }
+  free(kt); free(rk); free(qt); free(rq); free(Pm); free(dS); free(Oi); free(dgq_rows); free(dgk_rows);
   return 0;
+}
+
+/* The base problem of BASELINE.json north_star: video tokens only, no dgamma. */
+int arachne_oracle_head(const oracle_cfg* c, const int grid[3], int L, int R, const int* qidx,
+                        const double* q, const double* k, const double* v,
+                        const double* gamma_q, const double* gamma_k, const double* dO,
+                        double* O, double* LSE, double* P, double* dQ, double* dK, double* dV) {
+  return arachne_oracle_head_joint(c, grid, 0, L, R, qidx, q, k, v, gamma_q, gamma_k, dO, O, LSE, P,
+                                   dQ, dK, dV, NULL, NULL);
 }
 
 /* Debug hook for the RoPE / RMSNorm pins: x~ of one row. */
 int arachne_oracle_norm_rope(const oracle_cfg* c, const int pos[3], const double* x,
                              const double* gamma, double* xt) {
   int p[3] = {pos[0] + c->pos_offset[0], pos[1] + c->pos_offset[1], pos[2] + c->pos_offset[2]};
-  norm_rope_row(c, x, gamma, p, xt);
+  norm_rope_row(c, x, gamma, p, 0, xt);
   return 0;
 }

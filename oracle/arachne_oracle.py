@@ -55,6 +55,8 @@ def _load():
         ip = ctypes.POINTER(ctypes.c_int)
         lib.arachne_oracle_head.restype = ctypes.c_int
         lib.arachne_oracle_head.argtypes = [ctypes.POINTER(_Cfg), ip, ctypes.c_int, ctypes.c_int, ip] + [dp] * 12
+        lib.arachne_oracle_head_joint.restype = ctypes.c_int
+        lib.arachne_oracle_head_joint.argtypes = [ctypes.POINTER(_Cfg), ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ip] + [dp] * 14
         lib.arachne_oracle_norm_rope.restype = ctypes.c_int
         lib.arachne_oracle_norm_rope.argtypes = [ctypes.POINTER(_Cfg), ip, dp, dp, dp]
         lib.arachne_oracle_num_threads.restype = ctypes.c_int
@@ -106,9 +108,11 @@ def norm_rope(x, pos, gamma=None, **kw):
     return out
 
 
-def head(q_rows, k, v, grid, qidx=None, dO_rows=None, gamma_q=None, gamma_k=None, want_P=False, **kw):
+def head(q_rows, k, v, grid, qidx=None, dO_rows=None, gamma_q=None, gamma_k=None, want_P=False, n_text=0, **kw):
     """One (sequence, head) problem.  q_rows [R,D], k,v [L,D], grid=(T,Hg,Wg), qidx [R] in-sequence
-    token indices of the query rows (default: all L rows).  Returns a dict of fp64 arrays."""
+    token indices of the query rows (default: all L rows).  n_text: the last n_text of the L tokens are
+    text tokens (R21: normed, not rotated).  Returns a dict of fp64 arrays; with dO_rows also dGq, dGk [D]
+    (R22: this problem's terms of dl/dgamma_q, dl/dgamma_k)."""
     k = np.ascontiguousarray(k, dtype=np.float64)
     v = np.ascontiguousarray(v, dtype=np.float64)
     q_rows = np.ascontiguousarray(q_rows, dtype=np.float64)
@@ -125,70 +129,80 @@ def head(q_rows, k, v, grid, qidx=None, dO_rows=None, gamma_q=None, gamma_k=None
     if dO_rows is not None:
         dO = np.ascontiguousarray(dO_rows, dtype=np.float64)
         dQ, dK, dV = np.empty((R, D)), np.empty((L, D)), np.empty((L, D))
-    rc = _load().arachne_oracle_head(
-        ctypes.byref(_cfg(D, **kw)), _iptr(g), L, R, _iptr(qidx), _dptr(q_rows), _dptr(k), _dptr(v),
+        dGq, dGk = np.empty(D), np.empty(D)
+    else:
+        dGq = dGk = None
+    rc = _load().arachne_oracle_head_joint(
+        ctypes.byref(_cfg(D, **kw)), _iptr(g), int(n_text), L, R, _iptr(qidx), _dptr(q_rows), _dptr(k), _dptr(v),
         _dptr(gq), _dptr(gk), _dptr(dO), _dptr(out["O"]), _dptr(out["LSE"]), _dptr(P), _dptr(dQ),
-        _dptr(dK), _dptr(dV))
+        _dptr(dK), _dptr(dV), _dptr(dGq), _dptr(dGk))
     if rc != 0:
-        raise ValueError("arachne_oracle_head rejected its arguments (L>=1, grid product == L)")
+        raise ValueError("arachne_oracle_head rejected its arguments (L>=1, grid product + n_text == L)")
     if want_P:
         out["P"] = P
     if dO is not None:
-        out.update(dQ=dQ, dK=dK, dV=dV)
+        out.update(dQ=dQ, dK=dK, dV=dV, dGq=dGq, dGk=dGk)
     return out
 
 
-def _check_packing(cu_seqlens, grids, N):
+def _check_packing(cu_seqlens, grids, N, text_lens=None):
     cu = np.asarray(cu_seqlens, dtype=np.int64)
     grids = np.asarray(grids, dtype=np.int64).reshape(-1, 3)
+    text = np.zeros(len(cu) - 1, dtype=np.int64) if text_lens is None else np.asarray(text_lens, dtype=np.int64)
     assert cu[0] == 0 and np.all(np.diff(cu) >= 1) and cu[-1] == N, "bad cu_seqlens (R16: L_b >= 1)"
-    assert np.all(grids.prod(axis=1) == np.diff(cu)), "grid product != sequence length"
-    return cu, grids
+    assert np.all(text >= 0) and np.all(grids.prod(axis=1) + text == np.diff(cu)), "grid product + text != sequence length"
+    return cu, grids, text
 
 
-def attention(q, k, v, cu_seqlens, grids, dO=None, gamma_q=None, gamma_k=None, want_P=False, **kw):
+def attention(q, k, v, cu_seqlens, grids, dO=None, gamma_q=None, gamma_k=None, want_P=False, text_lens=None, **kw):
     """Full packed problem.  q,k,v (and dO) are [N,H,D] arrays of exact input values (any float
-    dtype; converted to fp64).  Returns O [N,H,D], LSE [H,N] and, if dO is given, dQ,dK,dV [N,H,D]."""
+    dtype; converted to fp64).  text_lens [B]: trailing text tokens of each sequence (R21; default none).
+    Returns O [N,H,D], LSE [H,N] and, if dO is given, dQ,dK,dV [N,H,D] and dGq,dGk [D] (R22: summed over
+    sequences and heads in index order)."""
     q, k, v = (np.asarray(a, dtype=np.float64) for a in (q, k, v))
     N, H, D = q.shape
-    cu, grids = _check_packing(cu_seqlens, grids, N)
+    cu, grids, text = _check_packing(cu_seqlens, grids, N, text_lens)
     res = {"O": np.empty((N, H, D)), "LSE": np.empty((H, N))}
     if dO is not None:
         dO = np.asarray(dO, dtype=np.float64)
-        res.update(dQ=np.empty((N, H, D)), dK=np.empty((N, H, D)), dV=np.empty((N, H, D)))
+        res.update(dQ=np.empty((N, H, D)), dK=np.empty((N, H, D)), dV=np.empty((N, H, D)), dGq=np.zeros(D), dGk=np.zeros(D))
     if want_P:
         res["P"] = {}
     for b in range(len(cu) - 1):
         s, e = int(cu[b]), int(cu[b + 1])
         for h in range(H):
             r = head(q[s:e, h], k[s:e, h], v[s:e, h], grids[b], dO_rows=None if dO is None else dO[s:e, h],
-                     gamma_q=gamma_q, gamma_k=gamma_k, want_P=want_P, **kw)
+                     gamma_q=gamma_q, gamma_k=gamma_k, want_P=want_P, n_text=int(text[b]), **kw)
             res["O"][s:e, h] = r["O"]
             res["LSE"][h, s:e] = r["LSE"]
             if dO is not None:
                 res["dQ"][s:e, h], res["dK"][s:e, h], res["dV"][s:e, h] = r["dQ"], r["dK"], r["dV"]
+                res["dGq"] += r["dGq"]
+                res["dGk"] += r["dGk"]
             if want_P:
                 res["P"][(b, h)] = r["P"]
     return res
 
 
-def attention_rows(q, k, v, cu_seqlens, grids, rows, dO=None, heads=None, gamma_q=None, gamma_k=None, **kw):
+def attention_rows(q, k, v, cu_seqlens, grids, rows, dO=None, heads=None, gamma_q=None, gamma_k=None,
+                   text_lens=None, **kw):
     """Sampled-row evaluation for configs too large for the O(L^2) run.
 
     rows : sorted global token indices (any subset).  heads : list of heads (default all).
     Returns O_rows [R,Hs,D], LSE_rows [Hs,R] exactly (a query row needs only its own row of S) and,
-    if dO is given, dQ_rows [R,Hs,D] exactly plus dK, dV [N,Hs,D] of the MASKED-dO problem (dO zero
-    outside `rows`), which the GPU can reproduce by running its backward on that masked dO.
+    if dO is given, dQ_rows [R,Hs,D] exactly plus dK, dV [N,Hs,D] and dGq, dGk [D] of the MASKED-dO
+    problem (dO zero outside `rows` and outside `heads`), which the GPU can reproduce by running its
+    backward on that masked dO.
     dO may be the full [N,H,D] tensor (only `rows` are read) or [R,H,D]."""
     N, H, D = q.shape
-    cu, grids = _check_packing(cu_seqlens, grids, N)
+    cu, grids, text = _check_packing(cu_seqlens, grids, N, text_lens)
     rows = np.asarray(rows, dtype=np.int64)
     assert np.all(np.diff(rows) > 0)
     heads = list(range(H)) if heads is None else list(heads)
     R, Hs = len(rows), len(heads)
     res = {"O": np.empty((R, Hs, D)), "LSE": np.empty((Hs, R)), "rows": rows, "heads": heads}
     if dO is not None:
-        res.update(dQ=np.empty((R, Hs, D)), dK=np.zeros((N, Hs, D)), dV=np.zeros((N, Hs, D)))
+        res.update(dQ=np.empty((R, Hs, D)), dK=np.zeros((N, Hs, D)), dV=np.zeros((N, Hs, D)), dGq=np.zeros(D), dGk=np.zeros(D))
         dO_is_full = dO.shape[0] == N and N != R
     for b in range(len(cu) - 1):
         s, e = int(cu[b]), int(cu[b + 1])
@@ -202,11 +216,13 @@ def attention_rows(q, k, v, cu_seqlens, grids, rows, dO=None, heads=None, gamma_
                 dO_rows = np.asarray(dO[rows[sel], h] if dO_is_full else dO[sel, h], dtype=np.float64)
             r = head(np.asarray(q[rows[sel], h], dtype=np.float64), np.asarray(k[s:e, h], dtype=np.float64),
                      np.asarray(v[s:e, h], dtype=np.float64), grids[b], qidx=qidx, dO_rows=dO_rows,
-                     gamma_q=gamma_q, gamma_k=gamma_k, **kw)
+                     gamma_q=gamma_q, gamma_k=gamma_k, n_text=int(text[b]), **kw)
             res["O"][sel, hi] = r["O"]
             res["LSE"][hi, sel] = r["LSE"]
             if dO is not None:
                 res["dQ"][sel, hi] = r["dQ"]
                 res["dK"][s:e, hi] = r["dK"]
                 res["dV"][s:e, hi] = r["dV"]
+                res["dGq"] += r["dGq"]      # masked-dO problem restricted to `heads`
+                res["dGk"] += r["dGk"]
     return res

@@ -15,7 +15,9 @@ import math
 import torch
 
 BASE_SEED = 260701701          # + 16*config_index + tensor_id  (0 structure, 1 Q, 2 K, 3 V, 4 dO)
-CONFIG_NAMES = ["tiny", "bucket256", "mixed480p", "long720p", "heavytail"]
+CONFIG_NAMES = ["tiny", "bucket256", "mixed480p", "long720p", "heavytail",
+                # SURVEY §8(f) NEXT-2 workloads (not BASELINE.json configs): joint video+text sequences
+                "joint720p", "cogvideox"]
 
 _M64 = (1 << 64) - 1
 
@@ -68,6 +70,7 @@ def structure(name: str, seed_offset: int = 0, order: str = "listed"):
     """Packing structure of a BASELINE.json config: dict(grids, cu_seqlens, H, D, rope_dims, index).
     order: 'listed' | 'reversed' | 'shuffled' (sequence order inside the pack)."""
     idx = CONFIG_NAMES.index(name)
+    text_lens = None
     if name == "tiny":
         grids, H, D = [(1, 8, 8), (2, 10, 10)], 2, 64
     elif name == "bucket256":
@@ -78,26 +81,40 @@ def structure(name: str, seed_offset: int = 0, order: str = "listed"):
         grids, H, D = [(33, 45, 80)], 24, 128
     elif name == "heavytail":
         grids, H, D = heavytail_structure(BASE_SEED + 16 * idx + seed_offset), 24, 128
+    elif name == "joint720p":
+        # the 720p long clip with its text prompt joined to the sequence (HunyuanVideo single-stream blocks,
+        # PAPER.md:322; "text ... < 256 tokens"), 24 heads x 128
+        grids, H, D, text_lens = [(33, 45, 80)], 24, 128, [256]
+    elif name == "cogvideox":
+        # CogVideoX-shaped batch: 30 heads x head_dim 64, 4 joint sequences of a 13-frame
+        # 30x45 latent grid plus a 226-token prompt each
+        grids, H, D, text_lens = [(13, 30, 45)] * 4, 30, 64, [226] * 4
     else:
         raise KeyError(name)
-    return pack(grids, H, D, order=order, seed=BASE_SEED + 16 * idx + seed_offset, index=idx)
+    return pack(grids, H, D, order=order, seed=BASE_SEED + 16 * idx + seed_offset, index=idx, text_lens=text_lens)
 
 
-def pack(grids, H, D, order="listed", seed=0, index=-1, rope_dims=None):
+def pack(grids, H, D, order="listed", seed=0, index=-1, rope_dims=None, text_lens=None):
+    """text_lens [B] (optional): text tokens appended after the video tokens of each sequence (reading R21)."""
     grids = [tuple(int(x) for x in g) for g in grids]
+    text = [0] * len(grids) if text_lens is None else [int(x) for x in text_lens]
+    assert len(text) == len(grids)
+    seqs = list(zip(grids, text))
     if order == "reversed":
-        grids = grids[::-1]
+        seqs = seqs[::-1]
     elif order == "shuffled":
         state = (seed ^ 0xA5A5A5A5) & _M64
-        for i in range(len(grids) - 1, 0, -1):
+        for i in range(len(seqs) - 1, 0, -1):
             state, r = _splitmix64(state)
             j = r % (i + 1)
-            grids[i], grids[j] = grids[j], grids[i]
+            seqs[i], seqs[j] = seqs[j], seqs[i]
+    grids, text = [g for g, _ in seqs], [x for _, x in seqs]
     cu = [0]
-    for t, hg, wg in grids:
-        cu.append(cu[-1] + t * hg * wg)
+    for (t, hg, wg), nt in seqs:
+        cu.append(cu[-1] + t * hg * wg + nt)
     return dict(grids=grids, cu_seqlens=cu, H=H, D=D, N=cu[-1],
-                rope_dims=tuple(rope_dims) if rope_dims else rope_dims_for(D), index=index)
+                rope_dims=tuple(rope_dims) if rope_dims else rope_dims_for(D), index=index,
+                text_lens=text if any(text) else None)
 
 
 def attention_flops(st) -> float:
