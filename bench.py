@@ -107,7 +107,8 @@ def oracle_sample(st, tensors_cpu, budget_rows=6, heads=2):
     q, k, v, dO = (tensors_cpu[n][sl].float().numpy() for n in ("q", "k", "v", "dO"))
     rows_local = [r - cu[b] for r in rows]
     t0 = time.perf_counter()
-    orc.attention_rows(q, k, v, [0, L], [st["grids"][b]], rows_local, dO=dO, heads=hs, rope_dims=st["rope_dims"])
+    text = None if not st.get("text_lens") else [st["text_lens"][b]]
+    orc.attention_rows(q, k, v, [0, L], [st["grids"][b]], rows_local, dO=dO, heads=hs, rope_dims=st["rope_dims"], text_lens=text)
     dt = time.perf_counter() - t0
     flops = 14.0 * st["D"] * len(rows) * L * len(hs)        # same convention, restricted to the sampled rows
     desc = (f"fp64 oracle fwd+bwd on {len(rows)} query rows x {len(hs)} heads of the longest sequence "
@@ -132,7 +133,8 @@ def run_reference(args):
     cu = st["cu_seqlens"]
     b = max(range(len(cu) - 1), key=lambda i: cu[i + 1] - cu[i])
     L = cu[b + 1] - cu[b]
-    one = inputs.pack([st["grids"][b]], st["H"], st["D"], index=st["index"], rope_dims=st["rope_dims"])
+    one = inputs.pack([st["grids"][b]], st["H"], st["D"], index=st["index"], rope_dims=st["rope_dims"],
+                      text_lens=None if not st.get("text_lens") else [st["text_lens"][b]])
     one["name"] = args.workload
     t = inputs.make_inputs(one, device="cpu")
     rows = max(4, min(L, int(6.0e6 / L)))          # ~5 s of oracle time per step (about 1.2e6 row x key / s / head)
@@ -158,7 +160,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="long720p", choices=["tiny", "bucket256", "mixed480p", "long720p", "heavytail"])
+    ap.add_argument("--workload", default="long720p", choices=["tiny", "bucket256", "mixed480p", "long720p", "heavytail", "joint720p", "cogvideox"])
     ap.add_argument("--impl", default="arachne", choices=["arachne", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -94,6 +94,16 @@ typedef struct arachne_plan arachne_plan;
  * Synchronous (uses cudaMalloc/cudaMemcpy). */
 int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params,
                         const int32_t* cu_seqlens_host, const int32_t* grids_host);
+/* Same, for JOINT sequences (the single-stream blocks of HunyuanVideo and CogVideoX's
+ * full attention run over video and text tokens together; text "< 256 tokens", PAPER.md:201;
+ * DESIGN.md reading R21): sequence b = its T*Hg*Wg video tokens in row-major (t,h,w) order FOLLOWED by
+ * text_lens_host[b] >= 0 text tokens, cu_seqlens[b+1]-cu_seqlens[b] == T*Hg*Wg + text_lens_host[b].  Text
+ * tokens get the same QK-RMSNorm but NO RoPE; attention is full over all tokens of the sequence.
+ *   text_lens_host : int32 [B] HOST, or NULL (= all zero, identical to arachne_plan_create)
+ * Errors: a negative text length is ARACHNE_ERR_BAD_SHAPE; a length mismatch ARACHNE_ERR_GRID_MISMATCH. */
+int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* params,
+                              const int32_t* cu_seqlens_host, const int32_t* grids_host,
+                              const int32_t* text_lens_host);
 void arachne_plan_destroy(arachne_plan* plan);
 
 /* Bytes of caller-owned device workspace needed by one call.  pass: 0 = fwd, 1 = bwd.
@@ -131,6 +141,20 @@ int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void*
                             const float* gamma_q, const float* gamma_k, const void* o,
                             const float* lse, const void* d_o, void* dq, void* dk, void* dv,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Backward that ALSO returns the gradients of the RMSNorm weights (DESIGN.md reading
+ * R22): dgamma_q[d] = sum over all tokens n and heads h of (R^T dq~)[n,h,d] * Q[n,h,d] * r_q[n,h], where
+ * dq~ is the gradient w.r.t. the normed + rotated query, R^T the inverse rotation and r = rsqrt(mean(x^2) +
+ * eps); likewise dgamma_k.  fp32 [D] DEVICE, fully overwritten; either may be NULL (not computed).  gamma is
+ * shared by all heads (R1), so the sum runs over heads too.  With ARACHNE_FLAG_NO_NORM both are zero.  The
+ * sum is taken in a fixed order (per-block partials, then block order), so given the same dq~/dk~ it is
+ * bit-reproducible.  Enqueues one more (tiny) kernel than arachne_varlen_attn_bwd; everything else is
+ * identical, and arachne_workspace_bytes(plan, 1) covers it. */
+int arachne_varlen_attn_bwd_dgamma(const arachne_plan* plan, const void* q, const void* k, const void* v,
+                                   const float* gamma_q, const float* gamma_k, const void* o,
+                                   const float* lse, const void* d_o, void* dq, void* dk, void* dv,
+                                   float* dgamma_q, float* dgamma_k,
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
  * memory, pinned or pageable): allocate device buffers, copy in, run on a private stream,

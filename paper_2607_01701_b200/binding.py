@@ -25,6 +25,7 @@ EXPORTS = [
     "arachne_varlen_attn_fwd", "arachne_varlen_attn_bwd", "arachne_varlen_attn_fwd_host",
     "arachne_varlen_attn_fwd_bwd_host", "arachne_status_string", "arachne_last_error_message",
     "arachne_kernel_name", "arachne_plan_enable_profiling", "arachne_plan_kernel_times",
+    "arachne_plan_create_joint", "arachne_varlen_attn_bwd_dgamma",
 ]
 
 
@@ -39,6 +40,8 @@ class AttnParams(ctypes.Structure):
 _vp, _i32p, _fp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_void_p
 _lib.arachne_plan_create.restype = ctypes.c_int
 _lib.arachne_plan_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p]
+_lib.arachne_plan_create_joint.restype = ctypes.c_int
+_lib.arachne_plan_create_joint.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p, _i32p]
 _lib.arachne_plan_destroy.restype = None
 _lib.arachne_plan_destroy.argtypes = [_vp]
 _lib.arachne_workspace_bytes.restype = ctypes.c_size_t
@@ -49,6 +52,8 @@ _lib.arachne_varlen_attn_fwd.restype = ctypes.c_int
 _lib.arachne_varlen_attn_fwd.argtypes = [_vp] * 8 + [_vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_bwd.restype = ctypes.c_int
 _lib.arachne_varlen_attn_bwd.argtypes = [_vp] * 12 + [_vp, ctypes.c_size_t, _vp]
+_lib.arachne_varlen_attn_bwd_dgamma.restype = ctypes.c_int
+_lib.arachne_varlen_attn_bwd_dgamma.argtypes = [_vp] * 14 + [_vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_fwd_host.restype = ctypes.c_int
 _lib.arachne_varlen_attn_fwd_host.argtypes = [_vp] * 8
 _lib.arachne_varlen_attn_fwd_bwd_host.restype = ctypes.c_int
@@ -83,10 +88,11 @@ def _ptr(t):
 
 
 class Plan:
-    """arachne_plan_create / arachne_plan_destroy."""
+    """arachne_plan_create[_joint] / arachne_plan_destroy.  text_lens [B] (optional): trailing text tokens of
+    each sequence (arachne_plan_create_joint)."""
 
     def __init__(self, cu_seqlens, grids, num_heads, head_dim, rope_dims, rope_theta=10000.0, rms_eps=1e-6,
-                 softmax_scale=0.0, flags=0):
+                 softmax_scale=0.0, flags=0, text_lens=None):
         cu = [int(x) for x in cu_seqlens]
         gr = [int(x) for g in grids for x in g]
         self.params = AttnParams()
@@ -102,7 +108,12 @@ class Plan:
         self._h = _vp()
         cu_arr = (ctypes.c_int32 * len(cu))(*cu)
         gr_arr = (ctypes.c_int32 * max(len(gr), 1))(*gr)
-        _check(_lib.arachne_plan_create(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr))
+        if text_lens is None:
+            _check(_lib.arachne_plan_create(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr))
+        else:
+            tl = [int(x) for x in text_lens]
+            tl_arr = (ctypes.c_int32 * max(len(tl), 1))(*tl)
+            _check(_lib.arachne_plan_create_joint(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr))
         self.N, self.H, self.D = self.params.total_tokens, num_heads, head_dim
 
     def workspace_bytes(self, bwd: bool) -> int:
@@ -154,6 +165,15 @@ def arachne_varlen_attn_bwd(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, worksp
                                         workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
 
 
+def arachne_varlen_attn_bwd_dgamma(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, workspace,
+                                   gamma_q=None, gamma_k=None, stream=None):
+    """As arachne_varlen_attn_bwd, plus dgamma_q, dgamma_k: fp32 CUDA [D] (either may be None)."""
+    _check(_lib.arachne_varlen_attn_bwd_dgamma(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
+                                               _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(dgamma_q),
+                                               _ptr(dgamma_k), _ptr(workspace),
+                                               workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
 def arachne_varlen_attn_fwd_host(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None):
     """Same as fwd but every tensor is a HOST (CPU, preferably pinned) tensor; copies are inside the call."""
     _check(_lib.arachne_varlen_attn_fwd_host(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k),
@@ -167,7 +187,8 @@ def arachne_varlen_attn_fwd_bwd_host(plan: Plan, q, k, v, d_o, o, lse, dq, dk, d
 
 # ---- convenience wrappers that allocate outputs / workspace with torch (plumbing only)
 def plan_for(st, flags=0, **kw) -> Plan:
-    return Plan(st["cu_seqlens"], st["grids"], st["H"], st["D"], st["rope_dims"], flags=flags, **kw)
+    return Plan(st["cu_seqlens"], st["grids"], st["H"], st["D"], st["rope_dims"], flags=flags,
+                text_lens=st.get("text_lens"), **kw)
 
 
 def forward(plan: Plan, q, k, v, gamma_q=None, gamma_k=None, workspace=None):
@@ -178,8 +199,14 @@ def forward(plan: Plan, q, k, v, gamma_q=None, gamma_k=None, workspace=None):
     return o, lse
 
 
-def backward(plan: Plan, q, k, v, o, lse, d_o, gamma_q=None, gamma_k=None, workspace=None):
+def backward(plan: Plan, q, k, v, o, lse, d_o, gamma_q=None, gamma_k=None, workspace=None, with_dgamma=False):
+    """Returns (dq, dk, dv) or, with_dgamma, (dq, dk, dv, dgamma_q, dgamma_k)."""
     dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
     ws = workspace if workspace is not None else torch.empty(plan.workspace_bytes(True), dtype=torch.uint8, device=q.device)
-    arachne_varlen_attn_bwd(plan, q, k, v, o, lse, d_o, dq, dk, dv, ws, gamma_q, gamma_k)
-    return dq, dk, dv
+    if not with_dgamma:
+        arachne_varlen_attn_bwd(plan, q, k, v, o, lse, d_o, dq, dk, dv, ws, gamma_q, gamma_k)
+        return dq, dk, dv
+    dgq = torch.empty(plan.D, dtype=torch.float32, device=q.device)
+    dgk = torch.empty(plan.D, dtype=torch.float32, device=q.device)
+    arachne_varlen_attn_bwd_dgamma(plan, q, k, v, o, lse, d_o, dq, dk, dv, dgq, dgk, ws, gamma_q, gamma_k)
+    return dq, dk, dv, dgq, dgk

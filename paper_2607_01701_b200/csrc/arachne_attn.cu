@@ -59,7 +59,8 @@ struct arachne_plan {
   float2* d_rope = nullptr;
   ProblemDesc pd{};
   // workspace layout
-  size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0, gradblk_bytes = 0;
+  size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0, gradblk_bytes = 0, dgpart_bytes = 0;
+  int post_blocks = 0;   // post_kernel grid.x (grid-stride over the N*H rows); fixes the dgamma summation order
   // optional per-kernel timing (arachne_plan_enable_profiling): ring of kProfSlots calls per pass,
   // kernels+1 events per call, recorded on the caller's stream (no synchronisation).
   static constexpr int kProfSlots = 32;
@@ -84,7 +85,7 @@ struct FwdWs { uint8_t *qt, *kt, *vt; };
 struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
 
 size_t fwd_ws_bytes(const arachne_plan* pl) { return 3 * pl->img_bytes; }
-size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes; }
+size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
 
 inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st) {
   if (!pl->profiling) return;
@@ -121,8 +122,8 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
 
 template <int D>
 int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
-               const void* o, const float* lse, const void* d_o, void* dq, void* dk, void* dv, void* ws,
-               cudaStream_t st) {
+               const void* o, const float* lse, const void* d_o, void* dq, void* dk, void* dv, float* dgq, float* dgk,
+               void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
   BwdWs b{};
   b.qt = w; w += pl->img_bytes;
@@ -132,7 +133,8 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.delta_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.gk_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
-  b.gq_t = reinterpret_cast<float*>(w);      // gradblk_bytes >= grad_bytes: either layout fits
+  b.gq_t = reinterpret_cast<float*>(w); w += pl->gradblk_bytes;     // gradblk_bytes >= grad_bytes: either layout fits
+  float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
   PrepParams pp{};
   pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
@@ -165,10 +167,13 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
     prof_mark(pl, 1, 2, st);
     prof_mark(pl, 1, 3, st);
   }
-  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk)};
-  const long long rows = static_cast<long long>(pl->p.total_tokens) * pl->p.num_heads;
-  post_kernel<D><<<dim3(static_cast<unsigned>((rows + 7) / 8), 2), 256, 0, st>>>(pl->pd, po);
+  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk), dgpart};
+  post_kernel<D><<<dim3(pl->post_blocks, 2), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
+  if (dgpart) {
+    dgamma_reduce_kernel<D><<<2, 256, 0, st>>>(dgpart, pl->post_blocks, dgq, dgk);
+    ARACHNE_CUDA(cudaGetLastError());
+  }
   prof_mark(pl, 1, 4, st);
   if (pl->profiling) pl->prof_calls[1]++;
   return ARACHNE_OK;
@@ -200,6 +205,11 @@ const char* arachne_status_string(int s) {
 const char* arachne_last_error_message(void) { return g_last_error.c_str(); }
 
 int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids) {
+  return arachne_plan_create_joint(out, params, cu, grids, nullptr);
+}
+
+int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
+                              const int32_t* text_lens) {
   if (!out || !params || !cu || !grids) return ARACHNE_ERR_NULL_POINTER;
   *out = nullptr;
   const arachne_attn_params& p = *params;
@@ -221,7 +231,9 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   for (int b = 0; b < p.num_seqs; ++b) {
     const int32_t* g = grids + 3 * b;
     if (g[0] <= 0 || g[1] <= 0 || g[2] <= 0) return ARACHNE_ERR_GRID_MISMATCH;
-    if (static_cast<long long>(g[0]) * g[1] * g[2] != static_cast<long long>(cu[b + 1] - cu[b])) return ARACHNE_ERR_GRID_MISMATCH;
+    const long long nt = text_lens ? text_lens[b] : 0;      // R21: trailing text tokens
+    if (nt < 0) return ARACHNE_ERR_BAD_SHAPE;
+    if (static_cast<long long>(g[0]) * g[1] * g[2] + nt != static_cast<long long>(cu[b + 1] - cu[b])) return ARACHNE_ERR_GRID_MISMATCH;
   }
   int dev = 0;
   cudaDeviceProp prop{};
@@ -242,6 +254,7 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
     s.tok_start = cu[b]; s.len = cu[b + 1] - cu[b];
     s.tile_base = tile_base; s.n_tiles = (s.len + kTileRows - 1) / kTileRows;
     s.T = grids[3 * b]; s.Hg = grids[3 * b + 1]; s.Wg = grids[3 * b + 2];
+    s.n_video = s.T * s.Hg * s.Wg;
     tile_base += s.n_tiles;
     for (int a = 0; a < 3; ++a) ext[a] = std::max(ext[a], grids[3 * b + a]);
     pl->seqs.push_back(s);
@@ -313,6 +326,11 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
   pl->rowvec_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * sizeof(float), 1024);
   pl->grad_bytes = align_up(static_cast<size_t>(p.total_tokens) * p.num_heads * p.head_dim * sizeof(float), 1024);
   pl->gradblk_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * p.head_dim * sizeof(float), 1024);
+  {
+    const long long rows = static_cast<long long>(p.total_tokens) * p.num_heads;
+    pl->post_blocks = static_cast<int>(std::min<long long>((rows + 7) / 8, static_cast<long long>(pl->num_sms) * 8));
+    pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
+  }
   if (const char* e = std::getenv("ARACHNE_BWD_QROT")) pl->q_rot = std::atoi(e);
   *out = pl;
   return ARACHNE_OK;
@@ -394,16 +412,22 @@ int arachne_varlen_attn_fwd(const arachne_plan* pl, const void* q, const void* k
 int arachne_varlen_attn_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
                             const float* gamma_k, const void* o, const float* lse, const void* d_o, void* dq, void* dk,
                             void* dv, void* ws, size_t ws_bytes, void* stream) {
+  return arachne_varlen_attn_bwd_dgamma(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, nullptr, nullptr, ws, ws_bytes, stream);
+}
+
+int arachne_varlen_attn_bwd_dgamma(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
+                                   const float* gamma_k, const void* o, const float* lse, const void* d_o, void* dq, void* dk,
+                                   void* dv, float* dgamma_q, float* dgamma_k, void* ws, size_t ws_bytes, void* stream) {
   if (!pl || !q || !k || !v || !o || !lse || !d_o || !dq || !dk || !dv || !ws) return ARACHNE_ERR_NULL_POINTER;
   if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(d_o) ||
       misaligned(dq) || misaligned(dk) || misaligned(dv) || misaligned(ws) || (gamma_q && misaligned(gamma_q)) ||
-      (gamma_k && misaligned(gamma_k)))
+      (gamma_k && misaligned(gamma_k)) || (dgamma_q && misaligned(dgamma_q)) || (dgamma_k && misaligned(dgamma_k)))
     return ARACHNE_ERR_MISALIGNED;
   if (ws_bytes < bwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   return pl->p.head_dim == 128
-             ? launch_bwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, ws, st)
-             : launch_bwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, ws, st);
+             ? launch_bwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, ws, st)
+             : launch_bwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, ws, st);
 }
 
 // ---------------------------------------------------------------- host-buffer convenience calls

@@ -15,7 +15,8 @@ struct SeqInfo {
   int tile_base;   // index of the sequence's first 128-token tile in the tiled workspace
   int n_tiles;     // ceil(L_b / 128)
   int T, Hg, Wg;   // latent grid; token n -> (n / (Hg*Wg), (n / Wg) % Hg, n % Wg)   (reading R7)
-  int pad;
+  int n_video;     // T*Hg*Wg: tokens [0, n_video) are video tokens (rotated); [n_video, len) are text tokens,
+                   // normed but NOT rotated (reading R21)
 };
 
 // One unit of work for every persistent kernel: (sequence, head, 128-token tile of that sequence).

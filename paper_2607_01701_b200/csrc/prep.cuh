@@ -81,8 +81,8 @@ __device__ __forceinline__ void store_image(uint8_t* img, int r, int d0, const f
 // returns the lane's partial sum of squares of the stored row (0 for pad rows)
 template <int D>
 __device__ __forceinline__ float norm_rope_store(const ProblemDesc& pd, const __nv_bfloat16* src, const float* gamma,
-                                                 uint8_t* img, int r, bool valid, const int (&pos)[3], int lane, int fmt,
-                                                 float prescale) {
+                                                 uint8_t* img, int r, bool valid, bool rotate, const int (&pos)[3], int lane,
+                                                 int fmt, float prescale) {
   constexpr int EPL = D / 32;
   const int d0 = lane * EPL;
   float x[EPL];
@@ -98,7 +98,7 @@ __device__ __forceinline__ float norm_rope_store(const ProblemDesc& pd, const __
 #pragma unroll
       for (int i = 0; i < EPL; ++i) x[i] *= rinv * (gamma ? __ldg(&gamma[d0 + i]) : 1.0f);
     }
-    if (!pd.no_rope) {
+    if (rotate) {
 #pragma unroll
       for (int i = 0; i < EPL; i += 2) {
         const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
@@ -136,12 +136,13 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
   for (int r = warp; r < kTileRows; r += 8) {
     const int n = t * kTileRows + r;            // token index inside the sequence
     const bool valid = n < sq.len;
+    const bool rotate = !pd.no_rope && n < sq.n_video;   // R21: trailing text tokens are normed, not rotated
     int pos[3];
     const int hw = sq.Hg * sq.Wg;
-    pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
+    pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;   // only read when rotate
     const size_t src = (static_cast<size_t>(sq.tok_start + n) * pd.H + h) * D;
-    const float qs = norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, pos, lane, pp.out_fmt, pp.q_prescale);
-    const float ks = norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, pos, lane, pp.out_fmt, 1.0f);
+    const float qs = norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, pp.q_prescale);
+    const float ks = norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, 1.0f);
     // row norms are only summed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, warp_sum(qs)); kn = fmaxf(kn, warp_sum(ks)); }
     float x[EPL];
@@ -213,81 +214,128 @@ struct PostParams {
   const float* gamma_k;
   __nv_bfloat16* dq;
   __nv_bfloat16* dk;
+  float* dgamma_part;           // nullable: [2][gridDim.x][D] per-block partial sums of dl/dgamma_q, dl/dgamma_k (R22)
 };
 
 // dx = r*u - r^3 * x * (sum_d u_d x_d)/D,  u = gamma * R^T g~   (§8 a8; oracle: norm_rope_row_bwd)
+// dl/dgamma_d += (R^T g~)_d * x_d * r                            (reading R22)
+// Grid (nblk, 2): y = 0 -> dQ, y = 1 -> dK.  Warps walk the (token, head) rows with a grid stride, so a
+// warp's dgamma partial stays in registers (lane l owns elements [l*D/32, ...)) until the end; the
+// per-block partials are then summed in block order by dgamma_reduce_kernel (fixed order: run-to-run
+// bit-reproducible for a given plan, whichever backward produced g~).
 template <int D>
 __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp) {
   constexpr int EPL = D / 32;
-  const int lane = threadIdx.x & 31;
-  const long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5);   // (token, head)
-  if (row >= static_cast<long long>(pd.N) * pd.H) return;
-  const int tok = static_cast<int>(row / pd.H);
+  __shared__ float s_part[8][D];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool is_k = blockIdx.y == 1;
   const float* gt = is_k ? pp.gk_t : pp.gq_t;
   const __nv_bfloat16* xraw = is_k ? pp.k : pp.q;
   const float* gamma = is_k ? pp.gamma_k : pp.gamma_q;
   __nv_bfloat16* out = is_k ? pp.dk : pp.dq;
-  // sequence of this token: binary search over cu_seqlens (num_seqs is small)
-  int lo = 0, hi = pd.num_seqs - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (pd.seqs[mid].tok_start <= tok) lo = mid; else hi = mid - 1;
-  }
-  const SeqInfo sq = pd.seqs[lo];
-  const int n = tok - sq.tok_start;
-  int pos[3];
-  pos[0] = n / (sq.Hg * sq.Wg); pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
   const int d0 = lane * EPL;
-  const size_t off = static_cast<size_t>(row) * D + d0;
-  float g[EPL], x[EPL];
-  size_t goff = off;
-  if (!is_k && pp.gq_blocked) {
-    const int gtile = sq.tile_base + n / kTileRows, qr = n % kTileRows;
-    goff = (static_cast<size_t>(row % pd.H) * pd.n_tiles_total + gtile) * (kTileRows * D) +
-           static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32 + ((((d0 & 31) >> 2) ^ (qr & 7)) << 2) + (d0 & 3);
-  }
-  if constexpr (EPL == 4) {
-    const float4 f = *reinterpret_cast<const float4*>(gt + goff);
-    g[0] = f.x; g[1] = f.y; g[2] = f.z; g[3] = f.w;
-  } else {
-    const float2 f = *reinterpret_cast<const float2*>(gt + goff);
-    g[0] = f.x; g[1] = f.y;
-  }
-  load_bf16_row<EPL>(xraw + off, x);
-  if (!pd.no_rope) {
+  float gam[EPL], dgam[EPL];
 #pragma unroll
-    for (int i = 0; i < EPL; i += 2) {
-      const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
-      const float g0 = g[i], g1 = g[i + 1];
-      g[i] = g0 * cs.x + g1 * cs.y;          // rotate by -phi
-      g[i + 1] = -g0 * cs.y + g1 * cs.x;
+  for (int i = 0; i < EPL; ++i) { gam[i] = gamma ? __ldg(&gamma[d0 + i]) : 1.0f; dgam[i] = 0.f; }
+  const long long n_rows = static_cast<long long>(pd.N) * pd.H;
+  const long long stride = static_cast<long long>(gridDim.x) * 8;
+  for (long long row = static_cast<long long>(blockIdx.x) * 8 + warp; row < n_rows; row += stride) {   // (token, head)
+    const int tok = static_cast<int>(row / pd.H);
+    // sequence of this token: binary search over cu_seqlens (num_seqs is small)
+    int lo = 0, hi = pd.num_seqs - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (pd.seqs[mid].tok_start <= tok) lo = mid; else hi = mid - 1;
+    }
+    const SeqInfo sq = pd.seqs[lo];
+    const int n = tok - sq.tok_start;
+    const bool rotate = !pd.no_rope && n < sq.n_video;     // R21: text tokens were not rotated
+    int pos[3];
+    pos[0] = n / (sq.Hg * sq.Wg); pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
+    const size_t off = static_cast<size_t>(row) * D + d0;
+    float g[EPL], x[EPL];
+    size_t goff = off;
+    if (!is_k && pp.gq_blocked) {
+      const int gtile = sq.tile_base + n / kTileRows, qr = n % kTileRows;
+      goff = (static_cast<size_t>(row % pd.H) * pd.n_tiles_total + gtile) * (kTileRows * D) +
+             static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32 + ((((d0 & 31) >> 2) ^ (qr & 7)) << 2) + (d0 & 3);
+    }
+    if constexpr (EPL == 4) {
+      const float4 f = *reinterpret_cast<const float4*>(gt + goff);
+      g[0] = f.x; g[1] = f.y; g[2] = f.z; g[3] = f.w;
+    } else {
+      const float2 f = *reinterpret_cast<const float2*>(gt + goff);
+      g[0] = f.x; g[1] = f.y;
+    }
+    load_bf16_row<EPL>(xraw + off, x);
+    if (rotate) {
+#pragma unroll
+      for (int i = 0; i < EPL; i += 2) {
+        const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
+        const float g0 = g[i], g1 = g[i + 1];
+        g[i] = g0 * cs.x + g1 * cs.y;          // rotate by -phi
+        g[i + 1] = -g0 * cs.y + g1 * cs.x;
+      }
+    }
+    float y[EPL];
+    if (!pd.no_norm) {
+      float ss = 0.f, ux = 0.f;
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) {
+        ss += x[i] * x[i];
+        ux += gam[i] * g[i] * x[i];
+      }
+      ss = warp_sum(ss);
+      ux = warp_sum(ux);
+      const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
+      const float c = rinv * rinv * rinv * ux * (1.0f / D);
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) {
+        y[i] = rinv * gam[i] * g[i] - c * x[i];
+        dgam[i] += g[i] * x[i] * rinv;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < EPL; ++i) y[i] = g[i];      // gamma unused: dgamma = 0
+    }
+    if constexpr (EPL == 4) {
+      uint2 u; u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]);
+      *reinterpret_cast<uint2*>(out + off) = u;
+    } else {
+      *reinterpret_cast<uint32_t*>(out + off) = pack_bf16x2(y[0], y[1]);
     }
   }
-  float y[EPL];
-  if (!pd.no_norm) {
-    float ss = 0.f, ux = 0.f;
+  if (pp.dgamma_part) {
 #pragma unroll
-    for (int i = 0; i < EPL; ++i) {
-      g[i] *= gamma ? __ldg(&gamma[d0 + i]) : 1.0f;     // u = gamma * g
-      ss += x[i] * x[i];
-      ux += g[i] * x[i];
+    for (int i = 0; i < EPL; ++i) s_part[warp][d0 + i] = dgam[i];
+    __syncthreads();
+    if (threadIdx.x < D) {
+      float a = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) a += s_part[w][threadIdx.x];
+      pp.dgamma_part[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * D + threadIdx.x] = a;
     }
-    ss = warp_sum(ss);
-    ux = warp_sum(ux);
-    const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
-    const float c = rinv * rinv * rinv * ux * (1.0f / D);
-#pragma unroll
-    for (int i = 0; i < EPL; ++i) y[i] = rinv * g[i] - c * x[i];
-  } else {
-#pragma unroll
-    for (int i = 0; i < EPL; ++i) y[i] = g[i];
   }
-  if constexpr (EPL == 4) {
-    uint2 u; u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]);
-    *reinterpret_cast<uint2*>(out + off) = u;
-  } else {
-    *reinterpret_cast<uint32_t*>(out + off) = pack_bf16x2(y[0], y[1]);
+}
+
+// dgamma[d] = sum over the post_kernel blocks, in block order.  Grid 2 (0: gamma_q, 1: gamma_k), 256 threads:
+// thread (s, d) with s = tid / D sums the blocks b == s (mod 256/D); the 256/D slices are then added in order.
+template <int D>
+__global__ void __launch_bounds__(256) dgamma_reduce_kernel(const float* part, int nblk, float* dgamma_q, float* dgamma_k) {
+  constexpr int S = 256 / D;
+  __shared__ float s[S][D];
+  const int d = threadIdx.x % D, sl = threadIdx.x / D;
+  const float* p = part + static_cast<size_t>(blockIdx.x) * nblk * D;
+  float a = 0.f;
+  for (int b = sl; b < nblk; b += S) a += p[static_cast<size_t>(b) * D + d];
+  s[sl][d] = a;
+  __syncthreads();
+  float* out = blockIdx.x == 0 ? dgamma_q : dgamma_k;
+  if (sl == 0 && out) {
+    float t = 0.f;
+#pragma unroll
+    for (int i = 0; i < S; ++i) t += s[i][d];
+    out[d] = t;
   }
 }
 

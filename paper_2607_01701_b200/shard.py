@@ -50,8 +50,9 @@ def shard_structure(st: dict, rank: int, world_size: int) -> dict:
     lcu = [0]
     for b in mine:
         lcu.append(lcu[-1] + lengths[b])
+    text = st.get("text_lens")
     return dict(grids=grids, cu_seqlens=lcu, H=st["H"], D=st["D"], N=lcu[-1], rope_dims=st["rope_dims"],
-                index=st.get("index", -1), seq_ids=mine, token_index=[(cu[b], cu[b + 1]) for b in mine])
+                text_lens=[text[b] for b in mine] if text else None, index=st.get("index", -1), seq_ids=mine, token_index=[(cu[b], cu[b + 1]) for b in mine])
 
 
 def max_over_ranks(value: float, device=None) -> float:

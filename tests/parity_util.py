@@ -6,6 +6,9 @@ import torch
 
 # tolerances stated by BASELINE.json north_star
 TOL = dict(O_rel=1e-2, O_abs=2e-2, LSE_abs=1e-3, dQ_rel=2e-2, dK_rel=2e-2, dV_rel=2e-2)
+# dgamma_q / dgamma_k (reading R22) are sums of dQ^ / dK^ terms: north_star states no gate
+# for them, so they are held to the gradient gate (rel-L2 over the [D] vector), DESIGN.md §6
+TOL_DGAMMA = 2e-2
 
 
 def rel_l2(a, b):
@@ -14,7 +17,7 @@ def rel_l2(a, b):
     return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a - b))
 
 
-def run_gpu(st, t, flags=0, gamma_q=None, gamma_k=None, with_bwd=True, plan_kw=None):
+def run_gpu(st, t, flags=0, gamma_q=None, gamma_k=None, with_bwd=True, plan_kw=None, with_dgamma=False):
     from paper_2607_01701_b200 import binding
 
     plan = binding.plan_for(st, flags=flags, **(plan_kw or {}))
@@ -23,8 +26,10 @@ def run_gpu(st, t, flags=0, gamma_q=None, gamma_k=None, with_bwd=True, plan_kw=N
     o, lse = binding.forward(plan, t["q"], t["k"], t["v"], gq, gk)
     out = {"O": o, "LSE": lse, "plan": plan}
     if with_bwd:
-        dq, dk, dv = binding.backward(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], gq, gk)
-        out.update(dQ=dq, dK=dk, dV=dv)
+        r = binding.backward(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], gq, gk, with_dgamma=with_dgamma)
+        out.update(dQ=r[0], dK=r[1], dV=r[2])
+        if with_dgamma:
+            out.update(dGq=r[3], dGk=r[4])
     torch.cuda.synchronize()
     return out
 
@@ -52,6 +57,14 @@ def check_full(st, got, ref, with_bwd=True, tol=TOL):
         worst["LSE_abs"] = max(worst.get("LSE_abs", 0.0), la)
         assert la <= tol["LSE_abs"], f"LSE max-abs {la:.3e} in sequence {b}"
     return worst
+
+
+def check_dgamma(got, ref, tol=TOL_DGAMMA):
+    w = {}
+    for k in ("dGq", "dGk"):
+        w[k + "_rel"] = rel_l2(to_np(got[k]), ref[k])
+        assert w[k + "_rel"] <= tol, f"{k} rel-L2 {w[k + '_rel']:.3e} > {tol}"
+    return w
 
 
 def check_rows(st, got, ref, rows, tol=TOL):

@@ -1,0 +1,138 @@
+"""GPU parity for the SURVEY §8(f) rows built after the base path: NEXT-1 (gamma != 1 with dgamma_q /
+dgamma_k outputs, reading R22) and NEXT-2 (joint video + text sequences, reading R21; CogVideoX shape
+30 heads x head_dim 64).  Same bar as test_gpu_parity.py: CUDA path through the C ABI vs the
+fp64 oracle on the same seeded bytes, north_star's tolerances per tensor and per sequence."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_01701_b200 import inputs
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+def _np(t):
+    return {k: v.float().cpu().numpy().astype(np.float64) for k, v in t.items()}
+
+
+def _gammas(D, seed=5):
+    rng = np.random.default_rng(seed)
+    return (0.5 + rng.random(D)).astype(np.float32), (0.5 + rng.random(D)).astype(np.float32)
+
+
+def _full(orc, st, flags=0, gamma=True, oracle_kw=None):
+    t = inputs.make_inputs(st, device="cuda")
+    gq, gk = _gammas(st["D"]) if gamma else (None, None)
+    got = pu.run_gpu(st, t, flags=flags, gamma_q=gq, gamma_k=gk, with_dgamma=True)
+    a = _np(t)
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], gamma_q=gq, gamma_k=gk,
+                        rope_dims=st["rope_dims"], text_lens=st["text_lens"], **(oracle_kw or {}))
+    w = pu.check_full(st, got, ref)
+    w.update(pu.check_dgamma(got, ref))
+    return w, got, t, ref
+
+
+@pytest.mark.parametrize("grids,text,H,D", [
+    ([(2, 9, 11), (1, 8, 8), (1, 1, 1)], [37, 0, 200], 2, 128),    # 235 (text crosses a tile edge), 64, 201
+    ([(1, 16, 16), (3, 10, 13)], [128, 6], 3, 64),                 # text = exactly one tile; text fills the tail
+    ([(1, 2, 3)] * 5, [1, 0, 250, 3, 0], 2, 128),                  # tiny grids, mostly-text sequences
+])
+def test_joint_text_tokens_and_dgamma_full(orc, grids, text, H, D):
+    w, _, _, _ = _full(orc, inputs.pack(grids, H, D, index=5, text_lens=text))
+    print(grids, text, w)
+
+
+def test_dgamma_video_only_and_deterministic_mode(orc):
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(2, 16, 20), (1, 5, 7), (5, 9, 11)], 4, 128, index=1)
+    w, got, t, ref = _full(orc, st)
+    print(w)
+    # the deterministic (two-pass) backward feeds the same post kernel: same dgamma gate, and bit-reproducible
+    gq, gk = _gammas(128)
+    a = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC, gamma_q=gq, gamma_k=gk, with_dgamma=True)
+    b = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC, gamma_q=gq, gamma_k=gk, with_dgamma=True)
+    pu.check_dgamma(a, ref)
+    for k in ("dQ", "dK", "dV", "dGq", "dGk"):
+        assert torch.equal(a[k], b[k]), k
+    # gamma = None (ones) through the dgamma entry point: dgamma is still defined (d/dgamma at gamma = 1)
+    g1 = pu.run_gpu(st, t, with_dgamma=True)
+    aa = _np(t)
+    r1 = orc.attention(aa["q"], aa["k"], aa["v"], st["cu_seqlens"], st["grids"], dO=aa["dO"], rope_dims=st["rope_dims"])
+    pu.check_dgamma(g1, r1)
+    # either output may be NULL
+    ws = torch.empty(got["plan"].workspace_bytes(True), dtype=torch.uint8, device="cuda")
+    dq, dk, dv = (torch.empty_like(t["q"]) for _ in range(3))
+    only_k = torch.full((128,), float("nan"), device="cuda")
+    binding.arachne_varlen_attn_bwd_dgamma(g1["plan"], t["q"], t["k"], t["v"], g1["O"], g1["LSE"], t["dO"], dq, dk, dv,
+                                           None, only_k, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(only_k, g1["dGk"]) or pu.rel_l2(pu.to_np(only_k), pu.to_np(g1["dGk"])) <= 1e-3
+
+
+def test_dgamma_is_zero_without_norm(orc):
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(2, 9, 11)], 2, 64, index=2, text_lens=[9])
+    t = inputs.make_inputs(st, device="cuda")
+    t = {k: (v.float() * (0.5 if k in ("q", "k") else 1.0)).to(torch.bfloat16) for k, v in t.items()}
+    got = pu.run_gpu(st, t, flags=binding.FLAG_NO_NORM, with_dgamma=True)
+    a = _np(t)
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], no_norm=True, text_lens=st["text_lens"])
+    pu.check_full(st, got, ref)
+    assert not got["dGq"].any() and not got["dGk"].any() and not ref["dGq"].any()
+
+
+def test_plan_create_joint_validation():
+    from paper_2607_01701_b200 import binding
+    with pytest.raises(binding.ArachneError) as e:
+        binding.Plan([0, 70], [(1, 8, 8)], 2, 64, (16, 24, 24), text_lens=[5])      # 64 + 5 != 70
+    assert e.value.status == 5
+    with pytest.raises(binding.ArachneError) as e:
+        binding.Plan([0, 63], [(1, 8, 8)], 2, 64, (16, 24, 24), text_lens=[-1])
+    assert e.value.status == 11
+    binding.Plan([0, 70], [(1, 8, 8)], 2, 64, (16, 24, 24), text_lens=[6]).close()
+
+
+def _large_joint(orc, name, heads, per_seq):
+    """Full-size NEXT-2 workloads in bench.py's launch configuration: sampled query rows (always including
+    text rows) exact per row, masked-dO dK / dV / dgamma exact for all key rows."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.structure(name)
+    t = inputs.make_inputs(st, device="cuda")
+    gq, gk = _gammas(st["D"], seed=9)
+    got = pu.run_gpu(st, t, gamma_q=gq, gamma_k=gk, with_dgamma=True)
+    cu = st["cu_seqlens"]
+    rows = set(inputs.sample_rows(st, per_seq=per_seq, seed=11))
+    for b in range(len(cu) - 1):                       # first / middle / last text token of every sequence
+        nt = st["text_lens"][b]
+        rows.update({cu[b + 1] - nt, cu[b + 1] - nt // 2, cu[b + 1] - 1, cu[b + 1] - nt - 1})
+    rows = sorted(rows)
+    ridx = torch.as_tensor(rows, device="cuda")
+    tc = {k: v.cpu() for k, v in t.items()}
+    q, k, v, dO = (tc[n].float().numpy() for n in ("q", "k", "v", "dO"))
+    ref = orc.attention_rows(q, k, v, cu, st["grids"], rows, dO=dO, heads=heads, gamma_q=gq, gamma_k=gk,
+                             rope_dims=st["rope_dims"], text_lens=st["text_lens"])
+    w = pu.check_rows(st, got, ref, rows)
+    dOm = torch.zeros_like(t["dO"])
+    hidx = torch.as_tensor(heads, device="cuda")
+    dOm[ridx[:, None], hidx[None, :]] = t["dO"][ridx[:, None], hidx[None, :]]      # masked in rows AND heads
+    g_q = torch.as_tensor(gq, device="cuda"); g_k = torch.as_tensor(gk, device="cuda")
+    dqm, dkm, dvm, dgq, dgk = binding.backward(got["plan"], t["q"], t["k"], t["v"], got["O"], got["LSE"], dOm, g_q, g_k,
+                                               with_dgamma=True)
+    torch.cuda.synchronize()
+    w.update(pu.check_masked_kv(st, {"dK": dkm, "dV": dvm}, ref))
+    w.update(pu.check_dgamma({"dGq": dgq, "dGk": dgk}, ref))
+    for b in range(len(cu) - 1):
+        s, e = cu[b], cu[b + 1]
+        lhs, rhs = got["dV"][s:e].float().sum(0), t["dO"][s:e].float().sum(0)
+        assert float(torch.linalg.vector_norm(lhs - rhs) / torch.linalg.vector_norm(rhs)) <= 2e-2, b
+    print(name, w)
+
+
+def test_cogvideox_shape_full_size(orc):
+    _large_joint(orc, "cogvideox", heads=[0, 14, 29], per_seq=24)
+
+
+def test_joint720p_full_size(orc):
+    _large_joint(orc, "joint720p", heads=[5, 23], per_seq=24)
