@@ -56,7 +56,8 @@ typedef enum {
   ARACHNE_ERR_BAD_ARCH = 9,          /* current device is not compute capability 10.x       */
   ARACHNE_ERR_CUDA = 10,             /* CUDA runtime error; text in arachne_last_error_message */
   ARACHNE_ERR_BAD_SHAPE = 11,        /* num_seqs/num_heads/total_tokens <= 0, or too large  */
-  ARACHNE_ERR_BAD_PARAM = 12         /* non-finite / non-positive theta, eps < 0, bad flags */
+  ARACHNE_ERR_BAD_PARAM = 12,        /* non-finite / non-positive theta, eps < 0, bad flags */
+  ARACHNE_ERR_BAD_SHARDING = 13      /* see arachne_plan_create_sharded; or a sharded plan passed to a plain call */
 } arachne_status;
 
 enum {
@@ -104,6 +105,27 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params,
 int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* params,
                               const int32_t* cu_seqlens_host, const int32_t* grids_host,
                               const int32_t* text_lens_host);
+/* Plan for Ulysses sequence parallelism with the All-to-All FUSED into the kernels (
+ * PAPER.md:84 "Ulysses SP partitions along the attention-head dimension ... All-to-All"; the SP degree k is what
+ * Arachne tunes per cascade).  The packed batch of N tokens is split BY TOKEN RANGE into
+ * num_shards buffers (one per SP rank): shard r is a [n_r, total_heads, D] bf16 tensor holding the global tokens
+ * [shard_starts_host[r], shard_starts_host[r+1]) with ALL heads — exactly what rank r has before Ulysses'
+ * first All-to-All.  This process computes heads [head_offset, head_offset + params->num_heads) of EVERY
+ * token: the *_sharded calls read Q, K, V (and O, dO) rows of those heads straight out of all shards and write
+ * O (dQ, dK, dV) rows of those heads straight into them.  A shard pointer may be local memory or a peer GPU's
+ * memory mapped into this process (CUDA IPC / symmetric memory over NVLink-NVSwitch): the gather IS the first
+ * All-to-All and the scatter IS the second, with no staging buffer, overlapped with the tensor-core kernels.
+ * The caller orders the ranks (all shards written before any rank's call starts; all calls finished before a
+ * shard is read): paper_2607_01701_b200/ulysses.py does it with torch.distributed barriers.
+ *   params->num_heads : LOCAL head count;  total_heads : heads in the raw tensors;  cu_seqlens / grids / text_lens
+ *   describe the GLOBAL pack (sequences may straddle shard boundaries);  1 <= num_shards <= 8;  shard_starts_host
+ *   int32 [num_shards+1] HOST, [0] = 0, non-decreasing, [num_shards] = N (NULL allowed iff num_shards == 1).
+ * lse, the workspace, gamma and dgamma are LOCAL: lse fp32 [num_heads, N]; dgamma is this rank's partial sum over
+ * its heads (all-reduce it across the SP group).  Errors: ARACHNE_ERR_BAD_SHARDING. */
+int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* params,
+                                const int32_t* cu_seqlens_host, const int32_t* grids_host,
+                                const int32_t* text_lens_host, int32_t num_shards,
+                                const int32_t* shard_starts_host, int32_t total_heads, int32_t head_offset);
 void arachne_plan_destroy(arachne_plan* plan);
 
 /* Bytes of caller-owned device workspace needed by one call.  pass: 0 = fwd, 1 = bwd.
@@ -155,6 +177,22 @@ int arachne_varlen_attn_bwd_dgamma(const arachne_plan* plan, const void* q, cons
                                    const float* lse, const void* d_o, void* dq, void* dk, void* dv,
                                    float* dgamma_q, float* dgamma_k,
                                    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Forward / backward on token-range-sharded tensors (plan from arachne_plan_create_sharded; a plan from
+ * arachne_plan_create[_joint] is the 1-shard case and is accepted too).  Every `const void* const* x` is a HOST
+ * array of num_shards DEVICE pointers, x[r] = base of shard r ([n_r, total_heads, D] bf16, 16-byte aligned;
+ * may be NULL iff shard r is empty).  Same semantics, workspace and stream rules as the plain calls;
+ * dgamma_q / dgamma_k may be NULL. */
+int arachne_varlen_attn_fwd_sharded(const arachne_plan* plan, const void* const* q, const void* const* k,
+                                    const void* const* v, const float* gamma_q, const float* gamma_k,
+                                    void* const* o, float* lse, void* workspace, size_t workspace_bytes,
+                                    void* cuda_stream);
+int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const* q, const void* const* k,
+                                    const void* const* v, const float* gamma_q, const float* gamma_k,
+                                    const void* const* o, const float* lse, const void* const* d_o,
+                                    void* const* dq, void* const* dk, void* const* dv,
+                                    float* dgamma_q, float* dgamma_k,
+                                    void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
  * memory, pinned or pageable): allocate device buffers, copy in, run on a private stream,

@@ -26,6 +26,7 @@ EXPORTS = [
     "arachne_varlen_attn_fwd_bwd_host", "arachne_status_string", "arachne_last_error_message",
     "arachne_kernel_name", "arachne_plan_enable_profiling", "arachne_plan_kernel_times",
     "arachne_plan_create_joint", "arachne_varlen_attn_bwd_dgamma",
+    "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
 ]
 
 
@@ -42,6 +43,9 @@ _lib.arachne_plan_create.restype = ctypes.c_int
 _lib.arachne_plan_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p]
 _lib.arachne_plan_create_joint.restype = ctypes.c_int
 _lib.arachne_plan_create_joint.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p, _i32p]
+_lib.arachne_plan_create_sharded.restype = ctypes.c_int
+_lib.arachne_plan_create_sharded.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p, _i32p,
+                                             ctypes.c_int32, _i32p, ctypes.c_int32, ctypes.c_int32]
 _lib.arachne_plan_destroy.restype = None
 _lib.arachne_plan_destroy.argtypes = [_vp]
 _lib.arachne_workspace_bytes.restype = ctypes.c_size_t
@@ -54,6 +58,12 @@ _lib.arachne_varlen_attn_bwd.restype = ctypes.c_int
 _lib.arachne_varlen_attn_bwd.argtypes = [_vp] * 12 + [_vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_bwd_dgamma.restype = ctypes.c_int
 _lib.arachne_varlen_attn_bwd_dgamma.argtypes = [_vp] * 14 + [_vp, ctypes.c_size_t, _vp]
+_vpp = ctypes.POINTER(ctypes.c_void_p)
+_lib.arachne_varlen_attn_fwd_sharded.restype = ctypes.c_int
+_lib.arachne_varlen_attn_fwd_sharded.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vp, _vpp, _vp, _vp, ctypes.c_size_t, _vp]
+_lib.arachne_varlen_attn_bwd_sharded.restype = ctypes.c_int
+_lib.arachne_varlen_attn_bwd_sharded.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vp, _vpp, _vp, _vpp, _vpp, _vpp, _vpp,
+                                                 _vp, _vp, _vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_fwd_host.restype = ctypes.c_int
 _lib.arachne_varlen_attn_fwd_host.argtypes = [_vp] * 8
 _lib.arachne_varlen_attn_fwd_bwd_host.restype = ctypes.c_int
@@ -89,10 +99,12 @@ def _ptr(t):
 
 class Plan:
     """arachne_plan_create[_joint] / arachne_plan_destroy.  text_lens [B] (optional): trailing text tokens of
-    each sequence (arachne_plan_create_joint)."""
+    each sequence (arachne_plan_create_joint).  shard_starts [k+1] (+ total_heads, head_offset): token-range
+    sharding of the raw tensors for the fused-All-to-All Ulysses calls (arachne_plan_create_sharded); num_heads
+    is then the LOCAL head count."""
 
     def __init__(self, cu_seqlens, grids, num_heads, head_dim, rope_dims, rope_theta=10000.0, rms_eps=1e-6,
-                 softmax_scale=0.0, flags=0, text_lens=None):
+                 softmax_scale=0.0, flags=0, text_lens=None, shard_starts=None, total_heads=None, head_offset=0):
         cu = [int(x) for x in cu_seqlens]
         gr = [int(x) for g in grids for x in g]
         self.params = AttnParams()
@@ -108,7 +120,18 @@ class Plan:
         self._h = _vp()
         cu_arr = (ctypes.c_int32 * len(cu))(*cu)
         gr_arr = (ctypes.c_int32 * max(len(gr), 1))(*gr)
-        if text_lens is None:
+        self.num_shards = 1
+        if shard_starts is not None:
+            ss = [int(x) for x in shard_starts]
+            self.num_shards = len(ss) - 1
+            ss_arr = (ctypes.c_int32 * len(ss))(*ss)
+            tl_arr = None
+            if text_lens is not None:
+                tl = [int(x) for x in text_lens]
+                tl_arr = (ctypes.c_int32 * max(len(tl), 1))(*tl)
+            _check(_lib.arachne_plan_create_sharded(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr,
+                                                    self.num_shards, ss_arr, int(total_heads or num_heads), int(head_offset)))
+        elif text_lens is None:
             _check(_lib.arachne_plan_create(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr))
         else:
             tl = [int(x) for x in text_lens]
@@ -172,6 +195,32 @@ def arachne_varlen_attn_bwd_dgamma(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv,
                                                _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(dgamma_q),
                                                _ptr(dgamma_k), _ptr(workspace),
                                                workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
+def _ptr_array(shards, n):
+    """HOST array of n device pointers from a list of CUDA tensors / integer addresses / None (empty shard)."""
+    assert len(shards) == n, f"expected {n} shards, got {len(shards)}"
+    vals = [None if s is None else (int(s) if isinstance(s, int) else s.data_ptr()) for s in shards]
+    return (ctypes.c_void_p * n)(*vals)
+
+
+def arachne_varlen_attn_fwd_sharded(plan: Plan, q, k, v, o, lse, workspace, gamma_q=None, gamma_k=None, stream=None):
+    """q, k, v, o: lists of plan.num_shards bf16 CUDA tensors [n_r, total_heads, D] (or raw device addresses of peer
+    memory); lse: LOCAL fp32 [num_heads, N]."""
+    n = plan.num_shards
+    _check(_lib.arachne_varlen_attn_fwd_sharded(plan._h, _ptr_array(q, n), _ptr_array(k, n), _ptr_array(v, n),
+                                                _ptr(gamma_q), _ptr(gamma_k), _ptr_array(o, n), _ptr(lse), _ptr(workspace),
+                                                workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
+def arachne_varlen_attn_bwd_sharded(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, workspace, dgamma_q=None, dgamma_k=None,
+                                    gamma_q=None, gamma_k=None, stream=None):
+    n = plan.num_shards
+    _check(_lib.arachne_varlen_attn_bwd_sharded(plan._h, _ptr_array(q, n), _ptr_array(k, n), _ptr_array(v, n),
+                                                _ptr(gamma_q), _ptr(gamma_k), _ptr_array(o, n), _ptr(lse),
+                                                _ptr_array(d_o, n), _ptr_array(dq, n), _ptr_array(dk, n), _ptr_array(dv, n),
+                                                _ptr(dgamma_q), _ptr(dgamma_k), _ptr(workspace),
+                                                workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
 
 
 def arachne_varlen_attn_fwd_host(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None):

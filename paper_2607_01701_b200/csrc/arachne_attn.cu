@@ -48,6 +48,7 @@ struct arachne_plan {
   int n_items = 0;
   int num_sms = 0;
   int device = 0;
+  Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
   int q_rot = 0;   // fused backward: query-tile rotation per key tile (ARACHNE_BWD_QROT env, tuning)
   // device arrays (owned)
   SeqInfo* d_seqs = nullptr;
@@ -94,13 +95,12 @@ inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st
 }
 
 template <int D>
-int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
-               void* o, float* lse, void* ws, cudaStream_t st) {
+int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k, const ShardedPtr& v, const float* gq,
+               const float* gk, const ShardedPtr& o, float* lse, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
   FwdWs f{w, w + pl->img_bytes, w + 2 * pl->img_bytes};
   PrepParams pp{};
-  pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
-  pp.v = static_cast<const __nv_bfloat16*>(v);
+  pp.q = q; pp.k = k; pp.v = v;
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
   pp.out_fmt = FMT_F16;
@@ -111,7 +111,7 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
-  FwdParams fp{f.qt, f.kt, f.vt, static_cast<__nv_bfloat16*>(o), lse};
+  FwdParams fp{f.qt, f.kt, f.vt, o, lse};
   const int grid = std::min(pl->num_sms, pl->n_fwd_items);
   fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
   ARACHNE_CUDA(cudaGetLastError());
@@ -121,9 +121,9 @@ int launch_fwd(const arachne_plan* pl, const void* q, const void* k, const void*
 }
 
 template <int D>
-int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gq, const float* gk,
-               const void* o, const float* lse, const void* d_o, void* dq, void* dk, void* dv, float* dgq, float* dgk,
-               void* ws, cudaStream_t st) {
+int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k, const ShardedPtr& v, const float* gq,
+               const float* gk, const ShardedPtr& o, const float* lse, const ShardedPtr& d_o, const ShardedPtr& dq,
+               const ShardedPtr& dk, const ShardedPtr& dv, float* dgq, float* dgk, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
   BwdWs b{};
   b.qt = w; w += pl->img_bytes;
@@ -137,9 +137,7 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
   PrepParams pp{};
-  pp.q = static_cast<const __nv_bfloat16*>(q); pp.k = static_cast<const __nv_bfloat16*>(k);
-  pp.v = static_cast<const __nv_bfloat16*>(v); pp.d_o = static_cast<const __nv_bfloat16*>(d_o);
-  pp.o = static_cast<const __nv_bfloat16*>(o); pp.lse = lse;
+  pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse; pp.backward = 1;
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.out_fmt = FMT_BF16;
@@ -152,7 +150,7 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
   const int grid = std::min(pl->num_sms, pl->n_items);
   if (deterministic) {
     // two-pass (7 GEMM) path: every output tile owned by one CTA, fixed summation order
-    BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv)};
+    BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv};
     bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
@@ -161,13 +159,13 @@ int launch_bwd(const arachne_plan* pl, const void* q, const void* k, const void*
     prof_mark(pl, 1, 3, st);
   } else {
     // fused single-pass (5 GEMM) path: dQ~ partial tiles reduce-added at L2 (order not fixed)
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, static_cast<__nv_bfloat16*>(dv), pl->q_rot};
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, pl->q_rot};
     bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pl->pd, bp);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
     prof_mark(pl, 1, 3, st);
   }
-  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, pp.q, pp.k, gq, gk, static_cast<__nv_bfloat16*>(dq), static_cast<__nv_bfloat16*>(dk), dgpart};
+  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, q, k, gq, gk, dq, dk, dgpart};
   post_kernel<D><<<dim3(pl->post_blocks, 2), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
@@ -198,6 +196,7 @@ const char* arachne_status_string(int s) {
     case ARACHNE_ERR_CUDA: return "CUDA runtime error";
     case ARACHNE_ERR_BAD_SHAPE: return "bad shape";
     case ARACHNE_ERR_BAD_PARAM: return "bad parameter";
+    case ARACHNE_ERR_BAD_SHARDING: return "bad sharding (1..8 shards, starts 0..N non-decreasing, head_offset + num_heads <= total_heads)";
     default: return "unknown status";
   }
 }
@@ -210,7 +209,21 @@ int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, c
 
 int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
                               const int32_t* text_lens) {
+  return arachne_plan_create_sharded(out, params, cu, grids, text_lens, 1, nullptr, params ? params->num_heads : 0, 0);
+}
+
+int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
+                                const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts,
+                                int32_t total_heads, int32_t head_offset) {
   if (!out || !params || !cu || !grids) return ARACHNE_ERR_NULL_POINTER;
+  if (num_shards < 1 || num_shards > kMaxShards || (num_shards > 1 && !shard_starts)) return ARACHNE_ERR_BAD_SHARDING;
+  if (head_offset < 0 || params->num_heads <= 0 || static_cast<long long>(head_offset) + params->num_heads > total_heads)
+    return ARACHNE_ERR_BAD_SHARDING;
+  if (shard_starts) {
+    if (shard_starts[0] != 0 || shard_starts[num_shards] != params->total_tokens) return ARACHNE_ERR_BAD_SHARDING;
+    for (int r = 0; r < num_shards; ++r)
+      if (shard_starts[r + 1] < shard_starts[r]) return ARACHNE_ERR_BAD_SHARDING;      // empty shards are allowed
+  }
   *out = nullptr;
   const arachne_attn_params& p = *params;
   if (p.head_dim != 64 && p.head_dim != 128) return ARACHNE_ERR_BAD_HEAD_DIM;
@@ -321,6 +334,12 @@ int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* par
   pd.no_norm = (p.flags & ARACHNE_FLAG_NO_NORM) ? 1 : 0;
   pd.no_rope = (p.flags & ARACHNE_FLAG_NO_ROPE) ? 1 : 0;
   pd.rope = rd;
+  pl->sh.n_shards = num_shards;
+  for (int r = 0; r <= kMaxShards; ++r)
+    pl->sh.start[r] = (shard_starts && r <= num_shards) ? shard_starts[r] : (r == 0 ? 0 : p.total_tokens);
+  pl->sh.H_total = total_heads;
+  pl->sh.head_offset = head_offset;
+  pd.sh = pl->sh;
   pl->tile_bytes = static_cast<size_t>(kTileRows) * p.head_dim * 2;
   pl->img_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * pl->tile_bytes, 1024);
   pl->rowvec_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * sizeof(float), 1024);
@@ -397,16 +416,53 @@ int arachne_plan_kernel_times(const arachne_plan* pl, int pass, float* ms_sum, i
   return ARACHNE_OK;
 }
 
+namespace {
+ShardedPtr one_shard(const void* p) {
+  ShardedPtr s{};
+  s.p[0] = const_cast<void*>(p);
+  return s;
+}
+// copies a host array of num_shards device pointers; empty shards may be NULL; others must be 16-byte aligned
+int gather_shards(const arachne_plan* pl, const void* const* arr, ShardedPtr& out) {
+  out = ShardedPtr{};
+  if (!arr) return ARACHNE_ERR_NULL_POINTER;
+  for (int r = 0; r < pl->sh.n_shards; ++r) {
+    const bool empty = pl->sh.start[r + 1] == pl->sh.start[r];
+    if (!arr[r] && !empty) return ARACHNE_ERR_NULL_POINTER;
+    if (misaligned(arr[r])) return ARACHNE_ERR_MISALIGNED;
+    out.p[r] = const_cast<void*>(arr[r]);
+  }
+  return ARACHNE_OK;
+}
+bool row_pitch_misaligned(const arachne_plan* pl) {   // every (token, head) row must start on a 16-byte boundary
+  return (static_cast<size_t>(pl->p.head_dim) * 2 * pl->sh.H_total) % 16 != 0;
+}
+}  // namespace
+
 int arachne_varlen_attn_fwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
                             const float* gamma_k, void* o, float* lse, void* ws, size_t ws_bytes, void* stream) {
+  if (!pl || !q || !k || !v || !o) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;      // a sharded plan needs the _sharded entry points
+  const void* qa[1] = {q}; const void* ka[1] = {k}; const void* va[1] = {v}; void* oa[1] = {o};
+  return arachne_varlen_attn_fwd_sharded(pl, qa, ka, va, gamma_q, gamma_k, oa, lse, ws, ws_bytes, stream);
+}
+
+int arachne_varlen_attn_fwd_sharded(const arachne_plan* pl, const void* const* q, const void* const* k, const void* const* v,
+                                    const float* gamma_q, const float* gamma_k, void* const* o, float* lse, void* ws,
+                                    size_t ws_bytes, void* stream) {
   if (!pl || !q || !k || !v || !o || !lse || !ws) return ARACHNE_ERR_NULL_POINTER;
-  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(ws) ||
-      (gamma_q && misaligned(gamma_q)) || (gamma_k && misaligned(gamma_k)))
+  ShardedPtr sq, sk, sv, so;
+  int rc;
+  if ((rc = gather_shards(pl, q, sq)) || (rc = gather_shards(pl, k, sk)) || (rc = gather_shards(pl, v, sv)) ||
+      (rc = gather_shards(pl, o, so)))
+    return rc;
+  if (misaligned(lse) || misaligned(ws) || (gamma_q && misaligned(gamma_q)) || (gamma_k && misaligned(gamma_k)) ||
+      row_pitch_misaligned(pl))
     return ARACHNE_ERR_MISALIGNED;
   if (ws_bytes < fwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  return pl->p.head_dim == 128 ? launch_fwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, ws, st)
-                               : launch_fwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, ws, st);
+  return pl->p.head_dim == 128 ? launch_fwd<128>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, ws, st)
+                               : launch_fwd<64>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, ws, st);
 }
 
 int arachne_varlen_attn_bwd(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
@@ -418,16 +474,33 @@ int arachne_varlen_attn_bwd(const arachne_plan* pl, const void* q, const void* k
 int arachne_varlen_attn_bwd_dgamma(const arachne_plan* pl, const void* q, const void* k, const void* v, const float* gamma_q,
                                    const float* gamma_k, const void* o, const float* lse, const void* d_o, void* dq, void* dk,
                                    void* dv, float* dgamma_q, float* dgamma_k, void* ws, size_t ws_bytes, void* stream) {
+  if (!pl || !q || !k || !v || !o || !d_o || !dq || !dk || !dv) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;
+  const void* qa[1] = {q}; const void* ka[1] = {k}; const void* va[1] = {v}; const void* oa[1] = {o};
+  const void* ga[1] = {d_o}; void* dqa[1] = {dq}; void* dka[1] = {dk}; void* dva[1] = {dv};
+  return arachne_varlen_attn_bwd_sharded(pl, qa, ka, va, gamma_q, gamma_k, oa, lse, ga, dqa, dka, dva, dgamma_q, dgamma_k,
+                                         ws, ws_bytes, stream);
+}
+
+int arachne_varlen_attn_bwd_sharded(const arachne_plan* pl, const void* const* q, const void* const* k, const void* const* v,
+                                    const float* gamma_q, const float* gamma_k, const void* const* o, const float* lse,
+                                    const void* const* d_o, void* const* dq, void* const* dk, void* const* dv,
+                                    float* dgamma_q, float* dgamma_k, void* ws, size_t ws_bytes, void* stream) {
   if (!pl || !q || !k || !v || !o || !lse || !d_o || !dq || !dk || !dv || !ws) return ARACHNE_ERR_NULL_POINTER;
-  if (misaligned(q) || misaligned(k) || misaligned(v) || misaligned(o) || misaligned(lse) || misaligned(d_o) ||
-      misaligned(dq) || misaligned(dk) || misaligned(dv) || misaligned(ws) || (gamma_q && misaligned(gamma_q)) ||
-      (gamma_k && misaligned(gamma_k)) || (dgamma_q && misaligned(dgamma_q)) || (dgamma_k && misaligned(dgamma_k)))
+  ShardedPtr sq, sk, sv, so, sg, sdq, sdk, sdv;
+  int rc;
+  if ((rc = gather_shards(pl, q, sq)) || (rc = gather_shards(pl, k, sk)) || (rc = gather_shards(pl, v, sv)) ||
+      (rc = gather_shards(pl, o, so)) || (rc = gather_shards(pl, d_o, sg)) || (rc = gather_shards(pl, dq, sdq)) ||
+      (rc = gather_shards(pl, dk, sdk)) || (rc = gather_shards(pl, dv, sdv)))
+    return rc;
+  if (misaligned(lse) || misaligned(ws) || (gamma_q && misaligned(gamma_q)) || (gamma_k && misaligned(gamma_k)) ||
+      (dgamma_q && misaligned(dgamma_q)) || (dgamma_k && misaligned(dgamma_k)) || row_pitch_misaligned(pl))
     return ARACHNE_ERR_MISALIGNED;
   if (ws_bytes < bwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   return pl->p.head_dim == 128
-             ? launch_bwd<128>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, ws, st)
-             : launch_bwd<64>(pl, q, k, v, gamma_q, gamma_k, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, ws, st);
+             ? launch_bwd<128>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, sdk, sdv, dgamma_q, dgamma_k, ws, st)
+             : launch_bwd<64>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, sdk, sdv, dgamma_q, dgamma_k, ws, st);
 }
 
 // ---------------------------------------------------------------- host-buffer convenience calls

@@ -35,7 +35,7 @@ struct BwdParams {
   const float* delta_t;    // [H][n_tiles][128]
   float* gq_t;             // out: dl/dq~ fp32 [N,H,D]
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
-  __nv_bfloat16* dv;       // out: [N,H,D]
+  ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
 };
 
 template <int D>
@@ -249,6 +249,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
       const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
       const uint32_t tA0 = tbase + Cfg::kColAcc0 + lane_base, tA1 = tbase + Cfg::kColAcc1 + lane_base;
       const float sc = pd.softmax_scale;
+      __nv_bfloat16* dv_row = valid_row ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
       float* gout = (kIsDQ ? bp.gq_t : bp.gk_t) + out_off;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
               w.y = pack_bf16x2(__uint_as_float(a[i + 2]), __uint_as_float(a[i + 3]));
               w.z = pack_bf16x2(__uint_as_float(a[i + 4]), __uint_as_float(a[i + 5]));
               w.w = pack_bf16x2(__uint_as_float(a[i + 6]), __uint_as_float(a[i + 7]));
-              *reinterpret_cast<uint4*>(bp.dv + out_off + c * 32 + i) = w;
+              *reinterpret_cast<uint4*>(dv_row + c * 32 + i) = w;
             }
           }
         }

@@ -39,7 +39,7 @@ struct BwdFusedParams {
   float* gq_blk;           // in/out: dl/dq~ fp32, blocked [H][n_tiles][D/32][128][32], 16-byte pieces
                            //         XOR-swizzled with (row & 7); zeroed by prep_kernel
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
-  __nv_bfloat16* dv;       // out: [N,H,D]
+  ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
   int q_rot;               // rotate the query-tile order per key tile (spreads the L2 reductions)
 };
 
@@ -335,6 +335,7 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
       const uint32_t tA = tbase + (wg == 0 ? Cfg::kColDV : Cfg::kColDK) + lane_base;
       const float sc = pd.softmax_scale;
+      __nv_bfloat16* dv_row = (valid_row && wg == 0) ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
         uint32_t a[32];
@@ -349,7 +350,7 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
               w.y = pack_bf16x2(__uint_as_float(a[i2 + 2]), __uint_as_float(a[i2 + 3]));
               w.z = pack_bf16x2(__uint_as_float(a[i2 + 4]), __uint_as_float(a[i2 + 5]));
               w.w = pack_bf16x2(__uint_as_float(a[i2 + 6]), __uint_as_float(a[i2 + 7]));
-              *reinterpret_cast<uint4*>(bp.dv + out_off + c * 32 + i2) = w;
+              *reinterpret_cast<uint4*>(dv_row + c * 32 + i2) = w;
             }
           } else {
 #pragma unroll

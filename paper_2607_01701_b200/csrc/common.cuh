@@ -37,6 +37,51 @@ struct RopeDesc {
   int half[3];   // d_a / 2
 };
 
+// Raw [tokens, heads, D] tensors may be SHARDED BY TOKEN RANGE across up to kMaxShards buffers (Ulysses sequence
+// parallelism): shard r holds the global tokens [start[r], start[r+1]) with ALL
+// H_total heads, [n_r, H_total, D]; this process computes heads [head_offset, head_offset + H).  The buffers are any
+// device-accessible memory (local, or peer memory mapped over NVLink), so the All-to-All of Ulysses is the prep
+// kernel's gather (loads) and the epilogues' scatter (stores) — no staging copy.  n_shards = 1, start = {0, N},
+// H_total = H, head_offset = 0 is the plain single-tensor case.
+constexpr int kMaxShards = 8;
+struct Sharding {
+  int n_shards;
+  int start[kMaxShards + 1];
+  int H_total;
+  int head_offset;
+};
+struct ShardedPtr {
+  void* p[kMaxShards];
+};
+// element offset of (global token tok, local head h, 0) inside its shard; r_out = the shard
+__device__ __forceinline__ size_t raw_off(const Sharding& sh, int tok, int h, int D, int& r_out) {
+  int r = 0;
+  if (sh.n_shards > 1) {      // uniform branch: the plain single-tensor case pays nothing
+#pragma unroll
+    for (int i = 1; i < kMaxShards; ++i)
+      if (i < sh.n_shards && tok >= sh.start[i]) r = i;
+  }
+  r_out = r;
+  return (static_cast<size_t>(tok - sh.start[r]) * sh.H_total + sh.head_offset + h) * D;
+}
+// t.p[r] with constant indices only (a dynamic index would make ptxas copy the kernel parameter to local memory)
+template <typename T>
+__device__ __forceinline__ T* shard_base(const ShardedPtr& t, int r) {
+  void* b = t.p[0];
+  if (r > 0) {
+#pragma unroll
+    for (int i = 1; i < kMaxShards; ++i)
+      if (r == i) b = t.p[i];
+  }
+  return static_cast<T*>(b);
+}
+template <typename T>
+__device__ __forceinline__ T* raw_row(const Sharding& sh, const ShardedPtr& t, int tok, int h, int D) {
+  int r;
+  const size_t off = raw_off(sh, tok, h, D, r);
+  return shard_base<T>(t, r) + off;
+}
+
 struct ProblemDesc {
   const SeqInfo* seqs;
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
@@ -52,6 +97,7 @@ struct ProblemDesc {
   float softmax_scale;
   int no_norm, no_rope;
   RopeDesc rope;
+  Sharding sh;
 };
 
 }  // namespace arachne

@@ -27,7 +27,7 @@ struct FwdParams {
   const uint8_t* qt;      // [H][n_tiles][TILE_BYTES]  Q^ fp16 images
   const uint8_t* kt;      // K^ fp16 images
   const uint8_t* vt;      // V bf16 images
-  __nv_bfloat16* o;       // [N,H,D]
+  ShardedPtr o;           // [N,H_total,D] bf16, possibly sharded by token range (common.cuh)
   float* lse;             // [H,N]
 };
 
@@ -305,7 +305,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
       const int n = (wi.tile + t) * kTileRows + row;     // token inside the sequence
       const bool valid_row = n < sq.len;
       const float inv_l = 1.0f / l;
-      __nv_bfloat16* orow = fp.o + (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
+      __nv_bfloat16* orow = valid_row ? raw_row<__nv_bfloat16>(pd.sh, fp.o, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32];

@@ -12,11 +12,9 @@
 namespace arachne {
 
 struct PrepParams {
-  const __nv_bfloat16* q;
-  const __nv_bfloat16* k;
-  const __nv_bfloat16* v;
-  const __nv_bfloat16* d_o;    // nullable (forward)
-  const __nv_bfloat16* o;      // nullable (forward)
+  ShardedPtr q, k, v;          // raw bf16 [N, H_total, D], possibly sharded by token range (common.cuh)
+  ShardedPtr d_o, o;           // backward only
+  int backward;                // 0 forward, 1 backward (d_o, o, lse valid)
   const float* lse;            // nullable (forward)
   const float* gamma_q;        // nullable => ones
   const float* gamma_k;
@@ -140,24 +138,27 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
     int pos[3];
     const int hw = sq.Hg * sq.Wg;
     pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;   // only read when rotate
-    const size_t src = (static_cast<size_t>(sq.tok_start + n) * pd.H + h) * D;
-    const float qs = norm_rope_store<D>(pd, pp.q + src, pp.gamma_q, pp.qt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, pp.q_prescale);
-    const float ks = norm_rope_store<D>(pd, pp.k + src, pp.gamma_k, pp.kt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, 1.0f);
+    int shard = 0;
+    const size_t src = valid ? raw_off(pd.sh, sq.tok_start + n, h, D, shard) : 0;
+    const __nv_bfloat16* qsrc = shard_base<const __nv_bfloat16>(pp.q, shard) + src;
+    const __nv_bfloat16* ksrc = shard_base<const __nv_bfloat16>(pp.k, shard) + src;
+    const float qs = norm_rope_store<D>(pd, qsrc, pp.gamma_q, pp.qt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, pp.q_prescale);
+    const float ks = norm_rope_store<D>(pd, ksrc, pp.gamma_k, pp.kt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, 1.0f);
     // row norms are only summed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, warp_sum(qs)); kn = fmaxf(kn, warp_sum(ks)); }
     float x[EPL];
-    if (valid) load_bf16_row<EPL>(pp.v + src + d0, x);
+    if (valid) load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.v, shard) + src + d0, x);
     else {
 #pragma unroll
       for (int i = 0; i < EPL; ++i) x[i] = 0.f;
     }
     store_image<EPL>(pp.vt + img_off, r, d0, x, FMT_BF16);     // bf16 -> bf16 is exact
-    if (pp.dot) {
+    if (pp.backward) {
       float g[EPL], oo[EPL];
       float dsum = 0.f;
       if (valid) {
-        load_bf16_row<EPL>(pp.d_o + src + d0, g);
-        load_bf16_row<EPL>(pp.o + src + d0, oo);
+        load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src + d0, g);
+        load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.o, shard) + src + d0, oo);
 #pragma unroll
         for (int i = 0; i < EPL; ++i) dsum += g[i] * oo[i];
       } else {
@@ -208,12 +209,10 @@ struct PostParams {
                                 // blocked/swizzled per-tile layout written by bwd_fused_kernel (gq_blk_off)
   int gq_blocked;
   const float* gk_t;
-  const __nv_bfloat16* q;       // raw
-  const __nv_bfloat16* k;
+  ShardedPtr q, k;              // raw bf16, possibly sharded (common.cuh)
   const float* gamma_q;
   const float* gamma_k;
-  __nv_bfloat16* dq;
-  __nv_bfloat16* dk;
+  ShardedPtr dq, dk;            // out bf16, same sharding
   float* dgamma_part;           // nullable: [2][gridDim.x][D] per-block partial sums of dl/dgamma_q, dl/dgamma_k (R22)
 };
 
@@ -230,9 +229,9 @@ __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool is_k = blockIdx.y == 1;
   const float* gt = is_k ? pp.gk_t : pp.gq_t;
-  const __nv_bfloat16* xraw = is_k ? pp.k : pp.q;
+  const ShardedPtr& xraw_s = is_k ? pp.k : pp.q;
   const float* gamma = is_k ? pp.gamma_k : pp.gamma_q;
-  __nv_bfloat16* out = is_k ? pp.dk : pp.dq;
+  const ShardedPtr& out_s = is_k ? pp.dk : pp.dq;
   const int d0 = lane * EPL;
   float gam[EPL], dgam[EPL];
 #pragma unroll
@@ -252,7 +251,11 @@ __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp
     const bool rotate = !pd.no_rope && n < sq.n_video;     // R21: text tokens were not rotated
     int pos[3];
     pos[0] = n / (sq.Hg * sq.Wg); pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
-    const size_t off = static_cast<size_t>(row) * D + d0;
+    const size_t off = static_cast<size_t>(row) * D + d0;      // local fp32 workspace [N, H, D]
+    int shard;
+    const size_t roff = raw_off(pd.sh, tok, static_cast<int>(row % pd.H), D, shard) + d0;
+    const __nv_bfloat16* xraw = shard_base<const __nv_bfloat16>(xraw_s, shard) + roff;
+    __nv_bfloat16* out = shard_base<__nv_bfloat16>(out_s, shard) + roff;
     float g[EPL], x[EPL];
     size_t goff = off;
     if (!is_k && pp.gq_blocked) {
@@ -267,7 +270,7 @@ __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp
       const float2 f = *reinterpret_cast<const float2*>(gt + goff);
       g[0] = f.x; g[1] = f.y;
     }
-    load_bf16_row<EPL>(xraw + off, x);
+    load_bf16_row<EPL>(xraw, x);
     if (rotate) {
 #pragma unroll
       for (int i = 0; i < EPL; i += 2) {
@@ -300,9 +303,9 @@ __global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp
     }
     if constexpr (EPL == 4) {
       uint2 u; u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]);
-      *reinterpret_cast<uint2*>(out + off) = u;
+      *reinterpret_cast<uint2*>(out) = u;
     } else {
-      *reinterpret_cast<uint32_t*>(out + off) = pack_bf16x2(y[0], y[1]);
+      *reinterpret_cast<uint32_t*>(out) = pack_bf16x2(y[0], y[1]);
     }
   }
   if (pp.dgamma_part) {

@@ -31,7 +31,7 @@ def test_status_strings_and_validation_without_device():
     from paper_2607_01701_b200 import binding
 
     lib = binding._lib
-    for s in range(0, 13):
+    for s in range(0, 14):
         assert lib.arachne_status_string(s).decode() not in ("", "unknown status")
     assert lib.arachne_status_string(99).decode() == "unknown status"
     assert lib.arachne_workspace_bytes(None, 0) == 0
