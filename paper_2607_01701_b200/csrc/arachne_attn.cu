@@ -53,6 +53,7 @@ struct arachne_plan {
   // device arrays (owned)
   SeqInfo* d_seqs = nullptr;
   int* d_tile_seq = nullptr;
+  TokInfo* d_tok_info = nullptr;
   WorkItem* d_items = nullptr;
   WorkItem* d_fwd_items = nullptr;
   int n_fwd_items = 0;
@@ -244,6 +245,7 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   for (int b = 0; b < p.num_seqs; ++b) {
     const int32_t* g = grids + 3 * b;
     if (g[0] <= 0 || g[1] <= 0 || g[2] <= 0) return ARACHNE_ERR_GRID_MISMATCH;
+    if (g[1] > 65535 || g[2] > 65535) return ARACHNE_ERR_BAD_SHAPE;      // TokInfo packs h, w into 16 bits each
     const long long nt = text_lens ? text_lens[b] : 0;      // R21: trailing text tokens
     if (nt < 0) return ARACHNE_ERR_BAD_SHAPE;
     if (static_cast<long long>(g[0]) * g[1] * g[2] + nt != static_cast<long long>(cu[b + 1] - cu[b])) return ARACHNE_ERR_GRID_MISMATCH;
@@ -316,6 +318,22 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   if ((e = cudaMemcpy(dptr, (vec).data(), (vec).size() * sizeof(T), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e, "cudaMemcpy");
   PLAN_UP(pl->d_seqs, pl->seqs, SeqInfo)
   PLAN_UP(pl->d_tile_seq, tile_seq, int)
+  {
+    std::vector<TokInfo> ti(static_cast<size_t>(p.total_tokens));
+    for (int b = 0; b < p.num_seqs; ++b) {
+      const SeqInfo& s = pl->seqs[b];
+      for (int n = 0; n < s.len; ++n) {
+        TokInfo& x = ti[static_cast<size_t>(s.tok_start) + n];
+        const bool text = n >= s.n_video;                       // R21
+        const int hw = s.Hg * s.Wg;
+        x.t_flag = text ? 0x80000000u : static_cast<uint32_t>(n / hw);
+        x.hw = text ? 0u : (static_cast<uint32_t>((n / s.Wg) % s.Hg) << 16) | static_cast<uint32_t>(n % s.Wg);
+        x.blkrow = static_cast<uint32_t>((s.tile_base + n / kTileRows) * kTileRows + n % kTileRows);
+        x.seq = static_cast<uint32_t>(b);
+      }
+    }
+    PLAN_UP(pl->d_tok_info, ti, TokInfo)
+  }
   PLAN_UP(pl->d_items, items, WorkItem)
   PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
   PLAN_UP(pl->d_rope, tab, float2)
@@ -327,7 +345,7 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -347,7 +365,8 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   pl->gradblk_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * p.head_dim * sizeof(float), 1024);
   {
     const long long rows = static_cast<long long>(p.total_tokens) * p.num_heads;
-    pl->post_blocks = static_cast<int>(std::min<long long>((rows + 7) / 8, static_cast<long long>(pl->num_sms) * 8));
+    const int rpb = 8 * (32 / (p.head_dim / 8));          // rows per post_kernel block and step (8 warps x RPW)
+    pl->post_blocks = static_cast<int>(std::min<long long>((rows + rpb - 1) / rpb, static_cast<long long>(pl->num_sms) * 8));
     pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
   }
   if (const char* e = std::getenv("ARACHNE_BWD_QROT")) pl->q_rot = std::atoi(e);
@@ -361,7 +380,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
   delete pl;
 }
 

@@ -19,6 +19,15 @@ struct SeqInfo {
                    // normed but NOT rotated (reading R21)
 };
 
+// Per-token lookup built by the plan (host): position on the latent grid and place in the tiled workspace, so the
+// elementwise kernels need neither integer divisions nor a search over cu_seqlens.
+struct TokInfo {
+  uint32_t t_flag;   // t (bits 0..30) | bit 31: text token (normed, not rotated: reading R21)
+  uint32_t hw;       // h << 16 | w      (grid extents <= 65535, checked by the plan)
+  uint32_t blkrow;   // (tile_base + n / 128) * 128 + n % 128: the token's row in the tiled workspace
+  uint32_t seq;      // sequence index
+};
+
 // One unit of work for every persistent kernel: (sequence, head, 128-token tile of that sequence).
 // Forward / dQ kernels read it as a QUERY tile, the dK/dV kernel as a KEY tile.  The host orders
 // the list longest-processing-time-first by (sequence, head) group, tiles of a group adjacent.
@@ -85,6 +94,7 @@ __device__ __forceinline__ T* raw_row(const Sharding& sh, const ShardedPtr& t, i
 struct ProblemDesc {
   const SeqInfo* seqs;
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
+  const TokInfo* tok_info;   // [N]
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
   const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int n_fwd_items;

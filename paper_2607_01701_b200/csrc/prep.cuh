@@ -1,10 +1,13 @@
 // Elementwise (HBM-bound) kernels around the tensor-core kernels:
 //   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> 16-bit operand tile images;
 //                 V, dO -> tile images (zero-padded tails); D_i = rowsum(dO*O); LSE*log2e padded.
-//   post_kernel : §8 a8.  dq~, dk~ (fp32) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK.
-// One warp owns one (token, head) row; lane l owns the D/32 contiguous elements [l*D/32, ...),
-// so both elements of every RoPE pair (2p, 2p+1) sit in the same lane and the only cross-lane
-// work is the sum of squares.  All loads/stores are whole 128/256-byte row segments.
+//   post_kernel : §8 a8.  dq~, dk~ (fp32) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK (+ dgamma partials, R22).
+// Thread mapping: a lane owns 8 contiguous elements (one 16-byte bf16 load / store, one swizzle chunk of a tile
+// image), so a (token, head) row takes LPR = D/8 lanes and a warp works on RPW = 32/LPR rows at once (2 at D = 128,
+// 4 at D = 64).  Both elements of every RoPE pair (2p, 2p+1) sit in the same lane; the only cross-lane work is the
+// sum over the LPR lanes of a row.  Token positions come from the plan's per-token table (TokInfo) — no integer
+// divisions and no search over cu_seqlens on the device.  These kernels were instruction-issue-bound with 8-byte
+// accesses and per-row index arithmetic; see profiles/r1_notes.md §7.
 #pragma once
 #include "common.cuh"
 #include "sm100.cuh"
@@ -32,145 +35,142 @@ struct PrepParams {
                                // the forward kernel derives its logit bound from them (static-max softmax)
 };
 
-__device__ __forceinline__ float warp_sum(float x) {
+// sum over the LPR consecutive lanes that share a row
+template <int LPR>
+__device__ __forceinline__ float seg_sum(float x) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  for (int o = LPR / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
   return x;
 }
 
-template <int EPL>
-__device__ __forceinline__ void load_bf16_row(const __nv_bfloat16* p, float (&x)[EPL]) {
-  if constexpr (EPL == 4) {
-    const uint2 u = *reinterpret_cast<const uint2*>(p);
-    x[0] = __uint_as_float(u.x << 16); x[1] = __uint_as_float(u.x & 0xffff0000u);
-    x[2] = __uint_as_float(u.y << 16); x[3] = __uint_as_float(u.y & 0xffff0000u);
+__device__ __forceinline__ void unpack_bf16x8(const uint4& u, float (&x)[8]) {
+  x[0] = __uint_as_float(u.x << 16); x[1] = __uint_as_float(u.x & 0xffff0000u);
+  x[2] = __uint_as_float(u.y << 16); x[3] = __uint_as_float(u.y & 0xffff0000u);
+  x[4] = __uint_as_float(u.z << 16); x[5] = __uint_as_float(u.z & 0xffff0000u);
+  x[6] = __uint_as_float(u.w << 16); x[7] = __uint_as_float(u.w & 0xffff0000u);
+}
+__device__ __forceinline__ uint4 pack8(const float (&y)[8], int fmt) {
+  uint4 u;
+  if (fmt == FMT_F16) {
+    u.x = pack_f16x2(y[0], y[1]); u.y = pack_f16x2(y[2], y[3]); u.z = pack_f16x2(y[4], y[5]); u.w = pack_f16x2(y[6], y[7]);
   } else {
-    const uint32_t u = *reinterpret_cast<const uint32_t*>(p);
-    x[0] = __uint_as_float(u << 16); x[1] = __uint_as_float(u & 0xffff0000u);
+    u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]); u.z = pack_bf16x2(y[4], y[5]); u.w = pack_bf16x2(y[6], y[7]);
+  }
+  return u;
+}
+
+// (cos, sin) of the 4 RoPE pairs of elements [d0, d0+8) at the token position packed in ti (identity when the token
+// is not rotated: text token, R21, or no_rope)
+__device__ __forceinline__ void rope_cs4(const RopeDesc& rp, int d0, const TokInfo& ti, bool rotate, float2 (&cs)[4]) {
+  const int pos[3] = {static_cast<int>(ti.t_flag & 0x7fffffffu), static_cast<int>(ti.hw >> 16), static_cast<int>(ti.hw & 0xffffu)};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    int a = 0, p = (d0 >> 1) + i;
+    if (p >= rp.half[0]) { p -= rp.half[0]; a = 1; if (p >= rp.half[1]) { p -= rp.half[1]; a = 2; } }
+    cs[i] = rotate ? __ldg(&rp.tab[rp.off[a] + pos[a] * rp.half[a] + p]) : make_float2(1.f, 0.f);
   }
 }
 
-// (cos, sin) of the RoPE pair `pp` (0..D/2-1) at grid position pos[]
-__device__ __forceinline__ float2 rope_cs(const RopeDesc& rp, int pp, const int (&pos)[3]) {
-  int a = 0, p = pp;
-  if (p >= rp.half[0]) { p -= rp.half[0]; a = 1; if (p >= rp.half[1]) { p -= rp.half[1]; a = 2; } }
-  return __ldg(&rp.tab[rp.off[a] + pos[a] * rp.half[a] + p]);
+// byte offset of the 16-byte chunk holding elements [d0, d0+8) of row r inside a [128][D] tile image
+__device__ __forceinline__ uint32_t image_off(int r, int d0) {
+  return static_cast<uint32_t>(d0 >> 6) * (kTileRows * 128) + swz_off(r, (d0 & 63) >> 3);
 }
 
-// byte offset of element d of row r inside a [128][D] tile image
-__device__ __forceinline__ uint32_t image_off(int r, int d) {
-  return static_cast<uint32_t>(d >> 6) * (kTileRows * 128) + swz_off(r, (d & 63) >> 3) + (d & 7) * 2;
-}
-
-template <int EPL>
-__device__ __forceinline__ void store_image(uint8_t* img, int r, int d0, const float (&y)[EPL], int fmt) {
-  uint8_t* dst = img + image_off(r, d0);
-  if constexpr (EPL == 4) {
-    uint2 u;
-    if (fmt == FMT_F16) { u.x = pack_f16x2(y[0], y[1]); u.y = pack_f16x2(y[2], y[3]); }
-    else                { u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]); }
-    *reinterpret_cast<uint2*>(dst) = u;
-  } else {
-    *reinterpret_cast<uint32_t*>(dst) = fmt == FMT_F16 ? pack_f16x2(y[0], y[1]) : pack_bf16x2(y[0], y[1]);
-  }
-}
-
-// x~ = RoPE(gamma * x * rsqrt(mean(x^2) + eps))  (readings R1-R5), one row per warp
-// returns the lane's partial sum of squares of the stored row (0 for pad rows)
+// x~ = RoPE(gamma * x * rsqrt(mean(x^2) + eps)) * prescale  (readings R1-R5) on this lane's 8 elements;
+// returns the lane's partial |x~|^2
 template <int D>
-__device__ __forceinline__ float norm_rope_store(const ProblemDesc& pd, const __nv_bfloat16* src, const float* gamma,
-                                                 uint8_t* img, int r, bool valid, bool rotate, const int (&pos)[3], int lane,
-                                                 int fmt, float prescale) {
-  constexpr int EPL = D / 32;
-  const int d0 = lane * EPL;
-  float x[EPL];
-  float nrm = 0.f;
-  if (valid) {
-    load_bf16_row<EPL>(src + d0, x);
-    if (!pd.no_norm) {
-      float ss = 0.f;
+__device__ __forceinline__ float norm_rope8(float (&x)[8], const float (&gam)[8], const float2 (&cs)[4], bool no_norm,
+                                            float eps, float prescale) {
+  constexpr int LPR = D / 8;
+  if (!no_norm) {
+    float ss = 0.f;
 #pragma unroll
-      for (int i = 0; i < EPL; ++i) ss += x[i] * x[i];
-      ss = warp_sum(ss);
-      const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
+    for (int i = 0; i < 8; ++i) ss += x[i] * x[i];
+    ss = seg_sum<LPR>(ss);
+    const float rinv = rsqrtf(ss * (1.0f / D) + eps);
 #pragma unroll
-      for (int i = 0; i < EPL; ++i) x[i] *= rinv * (gamma ? __ldg(&gamma[d0 + i]) : 1.0f);
-    }
-    if (rotate) {
-#pragma unroll
-      for (int i = 0; i < EPL; i += 2) {
-        const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
-        const float x0 = x[i], x1 = x[i + 1];
-        x[i] = x0 * cs.x - x1 * cs.y;
-        x[i + 1] = x0 * cs.y + x1 * cs.x;
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < EPL; ++i) { x[i] *= prescale; nrm += x[i] * x[i]; }
-  } else {
-#pragma unroll
-    for (int i = 0; i < EPL; ++i) x[i] = 0.f;   // zero-padded tail rows (never NaN: 0 * P stays 0)
+    for (int i = 0; i < 8; ++i) x[i] *= rinv * gam[i];
   }
-  store_image<EPL>(img, r, d0, x, fmt);
+  float nrm = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; i += 2) {
+    const float2 c = cs[i >> 1];
+    const float x0 = x[i], x1 = x[i + 1];
+    x[i] = (x0 * c.x - x1 * c.y) * prescale;
+    x[i + 1] = (x0 * c.y + x1 * c.x) * prescale;
+    nrm += x[i] * x[i] + x[i + 1] * x[i + 1];
+  }
   return nrm;
 }
 
 template <int D>
-__global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp) {
-  constexpr int EPL = D / 32;
+__global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams pp) {
+  constexpr int LPR = D / 8, RPW = 32 / LPR;
   constexpr int TILE_BYTES = kTileRows * D * 2;
   const int gtile = blockIdx.x, h = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  float qn = 0.f, kn = 0.f;      // this warp's largest |q~|^2, |k~|^2 (lane-partial sums until the end)
+  const int sub = lane / LPR, d0 = (lane % LPR) * 8;
+  float qn = 0.f, kn = 0.f;      // largest |q~|^2, |k~|^2 seen by this lane's rows (no_norm only)
   const SeqInfo sq = pd.seqs[pd.tile_seq[gtile]];
   const int t = gtile - sq.tile_base;
   const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
   const size_t row_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows;
-  const int d0 = lane * EPL;
   if (pp.gq_zero) {
     float4* z = reinterpret_cast<float4*>(pp.gq_zero + (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * (kTileRows * D));
     for (int i = threadIdx.x; i < kTileRows * D / 4; i += 256) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
-  for (int r = warp; r < kTileRows; r += 8) {
+  float gq[8], gk[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    gq[i] = pp.gamma_q ? __ldg(&pp.gamma_q[d0 + i]) : 1.0f;
+    gk[i] = pp.gamma_k ? __ldg(&pp.gamma_k[d0 + i]) : 1.0f;
+  }
+  const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll 1
+  for (int r = warp * RPW + sub; r < kTileRows; r += 8 * RPW) {
     const int n = t * kTileRows + r;            // token index inside the sequence
     const bool valid = n < sq.len;
-    const bool rotate = !pd.no_rope && n < sq.n_video;   // R21: trailing text tokens are normed, not rotated
-    int pos[3];
-    const int hw = sq.Hg * sq.Wg;
-    pos[0] = n / hw; pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;   // only read when rotate
+    const int tok = sq.tok_start + (valid ? n : 0);
+    const TokInfo ti = pd.tok_info[tok];
+    const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);   // R21: trailing text tokens are normed, not rotated
     int shard = 0;
-    const size_t src = valid ? raw_off(pd.sh, sq.tok_start + n, h, D, shard) : 0;
-    const __nv_bfloat16* qsrc = shard_base<const __nv_bfloat16>(pp.q, shard) + src;
-    const __nv_bfloat16* ksrc = shard_base<const __nv_bfloat16>(pp.k, shard) + src;
-    const float qs = norm_rope_store<D>(pd, qsrc, pp.gamma_q, pp.qt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, pp.q_prescale);
-    const float ks = norm_rope_store<D>(pd, ksrc, pp.gamma_k, pp.kt + img_off, r, valid, rotate, pos, lane, pp.out_fmt, 1.0f);
-    // row norms are only summed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
-    if (pp.stats && pd.no_norm) { qn = fmaxf(qn, warp_sum(qs)); kn = fmaxf(kn, warp_sum(ks)); }
-    float x[EPL];
-    if (valid) load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.v, shard) + src + d0, x);
-    else {
-#pragma unroll
-      for (int i = 0; i < EPL; ++i) x[i] = 0.f;
-    }
-    store_image<EPL>(pp.vt + img_off, r, d0, x, FMT_BF16);     // bf16 -> bf16 is exact
-    if (pp.backward) {
-      float g[EPL], oo[EPL];
-      float dsum = 0.f;
-      if (valid) {
-        load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src + d0, g);
-        load_bf16_row<EPL>(shard_base<const __nv_bfloat16>(pp.o, shard) + src + d0, oo);
-#pragma unroll
-        for (int i = 0; i < EPL; ++i) dsum += g[i] * oo[i];
-      } else {
-#pragma unroll
-        for (int i = 0; i < EPL; ++i) g[i] = 0.f;
+    const size_t src = raw_off(pd.sh, tok, h, D, shard) + d0;
+    uint4 uq = zero4, uk = zero4, uv = zero4, ug = zero4, uo = zero4;
+    if (valid) {
+      uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
+      uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src);
+      uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);
+      if (pp.backward) {
+        ug = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src);
+        uo = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.o, shard) + src);
       }
-      store_image<EPL>(pp.dot + img_off, r, d0, g, FMT_BF16);
-      dsum = warp_sum(dsum);                                    // D_i = sum_d dO*O   (§8 a5)
-      if (lane == 0) {
+    }
+    float2 cs[4];
+    rope_cs4(pd.rope, d0, ti, rotate, cs);
+    float xq[8], xk[8];
+    unpack_bf16x8(uq, xq);
+    unpack_bf16x8(uk, xk);
+    const float qs = norm_rope8<D>(xq, gq, cs, pd.no_norm != 0, pd.eps, pp.q_prescale);
+    const float ks = norm_rope8<D>(xk, gk, cs, pd.no_norm != 0, pd.eps, 1.0f);
+    const uint32_t ioff = image_off(r, d0);
+    *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, pp.out_fmt) : zero4;   // (eps = 0: 0 * inf)
+    *reinterpret_cast<uint4*>(pp.kt + img_off + ioff) = valid ? pack8(xk, pp.out_fmt) : zero4;
+    *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
+    // row norms are only needed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
+    if (pp.stats && pd.no_norm) { qn = fmaxf(qn, seg_sum<LPR>(qs)); kn = fmaxf(kn, seg_sum<LPR>(ks)); }
+    if (pp.backward) {
+      *reinterpret_cast<uint4*>(pp.dot + img_off + ioff) = ug;
+      float g[8], oo[8];
+      unpack_bf16x8(ug, g);
+      unpack_bf16x8(uo, oo);
+      float dsum = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) dsum += g[i] * oo[i];
+      dsum = seg_sum<LPR>(dsum);                                // D_i = sum_d dO*O   (§8 a5)
+      if (d0 == 0) {
         pp.delta_t[row_off + r] = valid ? dsum : 0.f;
         // pad rows get +inf so that P = exp2(s - inf) = 0 for them in the backward kernels
-        pp.lse2_t[row_off + r] = valid ? pp.lse[static_cast<size_t>(h) * pd.N + sq.tok_start + n] * 1.4426950408889634f
+        pp.lse2_t[row_off + r] = valid ? pp.lse[static_cast<size_t>(h) * pd.N + tok] * 1.4426950408889634f
                                        : __int_as_float(0x7f800000);
       }
     }
@@ -182,24 +182,31 @@ __global__ void __launch_bounds__(256) prep_kernel(ProblemDesc pd, PrepParams pp
     // Non-negative floats order like their bit patterns (+inf sorts last -> online-softmax path).
     if (!pd.no_norm) {
       if (blockIdx.x == 0 && blockIdx.y == 0 && warp == 0) {
-        float gq = 0.f, gk = 0.f;
+        float mq = 0.f, mk = 0.f;
         for (int d = lane; d < D; d += 32) {
-          gq = fmaxf(gq, pp.gamma_q ? fabsf(pp.gamma_q[d]) : 1.0f);
-          gk = fmaxf(gk, pp.gamma_k ? fabsf(pp.gamma_k[d]) : 1.0f);
+          mq = fmaxf(mq, pp.gamma_q ? fabsf(pp.gamma_q[d]) : 1.0f);
+          mk = fmaxf(mk, pp.gamma_k ? fabsf(pp.gamma_k[d]) : 1.0f);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-          gq = fmaxf(gq, __shfl_xor_sync(0xffffffffu, gq, o));
-          gk = fmaxf(gk, __shfl_xor_sync(0xffffffffu, gk, o));
+          mq = fmaxf(mq, __shfl_xor_sync(0xffffffffu, mq, o));
+          mk = fmaxf(mk, __shfl_xor_sync(0xffffffffu, mk, o));
         }
         if (lane == 0) {
-          atomicMax(&pp.stats[0], __float_as_uint(gq * gq * D * pp.q_prescale * pp.q_prescale));
-          atomicMax(&pp.stats[1], __float_as_uint(gk * gk * D));
+          atomicMax(&pp.stats[0], __float_as_uint(mq * mq * D * pp.q_prescale * pp.q_prescale));
+          atomicMax(&pp.stats[1], __float_as_uint(mk * mk * D));
         }
       }
-    } else if (lane == 0) {
-      atomicMax(&pp.stats[0], __float_as_uint(qn));
-      atomicMax(&pp.stats[1], __float_as_uint(kn));
+    } else {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        qn = fmaxf(qn, __shfl_xor_sync(0xffffffffu, qn, o));
+        kn = fmaxf(kn, __shfl_xor_sync(0xffffffffu, kn, o));
+      }
+      if (lane == 0) {
+        atomicMax(&pp.stats[0], __float_as_uint(qn));
+        atomicMax(&pp.stats[1], __float_as_uint(kn));
+      }
     }
   }
 }
@@ -218,104 +225,94 @@ struct PostParams {
 
 // dx = r*u - r^3 * x * (sum_d u_d x_d)/D,  u = gamma * R^T g~   (§8 a8; oracle: norm_rope_row_bwd)
 // dl/dgamma_d += (R^T g~)_d * x_d * r                            (reading R22)
-// Grid (nblk, 2): y = 0 -> dQ, y = 1 -> dK.  Warps walk the (token, head) rows with a grid stride, so a
-// warp's dgamma partial stays in registers (lane l owns elements [l*D/32, ...)) until the end; the
-// per-block partials are then summed in block order by dgamma_reduce_kernel (fixed order: run-to-run
-// bit-reproducible for a given plan, whichever backward produced g~).
+// Grid (nblk, 2): y = 0 -> dQ, y = 1 -> dK.  Warps walk the (token, head) rows with a grid stride, RPW rows per
+// warp and step, so a lane's dgamma partial stays in registers until the end; the per-block partials are then
+// summed in block order by dgamma_reduce_kernel (fixed order: run-to-run bit-reproducible for a given plan,
+// whichever backward produced g~).
 template <int D>
-__global__ void __launch_bounds__(256) post_kernel(ProblemDesc pd, PostParams pp) {
-  constexpr int EPL = D / 32;
-  __shared__ float s_part[8][D];
+__global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams pp) {
+  constexpr int LPR = D / 8, RPW = 32 / LPR;
+  __shared__ float s_part[8 * RPW][D];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int sub = lane / LPR, d0 = (lane % LPR) * 8;
   const bool is_k = blockIdx.y == 1;
   const float* gt = is_k ? pp.gk_t : pp.gq_t;
   const ShardedPtr& xraw_s = is_k ? pp.k : pp.q;
   const float* gamma = is_k ? pp.gamma_k : pp.gamma_q;
   const ShardedPtr& out_s = is_k ? pp.dk : pp.dq;
-  const int d0 = lane * EPL;
-  float gam[EPL], dgam[EPL];
+  const bool blocked = !is_k && pp.gq_blocked;
+  float gam[8], dgam[8];
 #pragma unroll
-  for (int i = 0; i < EPL; ++i) { gam[i] = gamma ? __ldg(&gamma[d0 + i]) : 1.0f; dgam[i] = 0.f; }
-  const long long n_rows = static_cast<long long>(pd.N) * pd.H;
-  const long long stride = static_cast<long long>(gridDim.x) * 8;
-  for (long long row = static_cast<long long>(blockIdx.x) * 8 + warp; row < n_rows; row += stride) {   // (token, head)
-    const int tok = static_cast<int>(row / pd.H);
-    // sequence of this token: binary search over cu_seqlens (num_seqs is small)
-    int lo = 0, hi = pd.num_seqs - 1;
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (pd.seqs[mid].tok_start <= tok) lo = mid; else hi = mid - 1;
-    }
-    const SeqInfo sq = pd.seqs[lo];
-    const int n = tok - sq.tok_start;
-    const bool rotate = !pd.no_rope && n < sq.n_video;     // R21: text tokens were not rotated
-    int pos[3];
-    pos[0] = n / (sq.Hg * sq.Wg); pos[1] = (n / sq.Wg) % sq.Hg; pos[2] = n % sq.Wg;
-    const size_t off = static_cast<size_t>(row) * D + d0;      // local fp32 workspace [N, H, D]
+  for (int i = 0; i < 8; ++i) { gam[i] = gamma ? __ldg(&gamma[d0 + i]) : 1.0f; dgam[i] = 0.f; }
+  const int n_rows = pd.N * pd.H;                              // < 2^31 (checked by the plan)
+  const int stride = gridDim.x * 8 * RPW;
+#pragma unroll 2
+  for (int row0 = (blockIdx.x * 8 + warp) * RPW; row0 < n_rows; row0 += stride) {   // warp-uniform trip count
+    const bool live = row0 + sub < n_rows;                     // ragged end: the lane keeps shuffling, stores nothing
+    const int row = live ? row0 + sub : n_rows - 1;            // (token, head)
+    const int tok = row / pd.H, h = row - tok * pd.H;
+    const TokInfo ti = pd.tok_info[tok];
+    const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);     // R21: text tokens were not rotated
     int shard;
-    const size_t roff = raw_off(pd.sh, tok, static_cast<int>(row % pd.H), D, shard) + d0;
-    const __nv_bfloat16* xraw = shard_base<const __nv_bfloat16>(xraw_s, shard) + roff;
-    __nv_bfloat16* out = shard_base<__nv_bfloat16>(out_s, shard) + roff;
-    float g[EPL], x[EPL];
-    size_t goff = off;
-    if (!is_k && pp.gq_blocked) {
-      const int gtile = sq.tile_base + n / kTileRows, qr = n % kTileRows;
-      goff = (static_cast<size_t>(row % pd.H) * pd.n_tiles_total + gtile) * (kTileRows * D) +
-             static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32 + ((((d0 & 31) >> 2) ^ (qr & 7)) << 2) + (d0 & 3);
-    }
-    if constexpr (EPL == 4) {
-      const float4 f = *reinterpret_cast<const float4*>(gt + goff);
-      g[0] = f.x; g[1] = f.y; g[2] = f.z; g[3] = f.w;
+    const size_t roff = raw_off(pd.sh, tok, h, D, shard) + d0;
+    const uint4 ux = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(xraw_s, shard) + roff);
+    float4 f0, f1;
+    if (blocked) {
+      // blocked layout [H][tile][D/32][128 rows][32], 16-byte pieces XOR-swizzled with (row & 7) (bwd_fused.cuh)
+      const int qr = ti.blkrow & (kTileRows - 1);
+      const float* base = gt + (static_cast<size_t>(h) * pd.n_tiles_total + (ti.blkrow >> 7)) * (kTileRows * D) +
+                          static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32;
+      const int j = (d0 & 31) >> 2;
+      f0 = *reinterpret_cast<const float4*>(base + ((j ^ (qr & 7)) << 2));
+      f1 = *reinterpret_cast<const float4*>(base + (((j + 1) ^ (qr & 7)) << 2));
     } else {
-      const float2 f = *reinterpret_cast<const float2*>(gt + goff);
-      g[0] = f.x; g[1] = f.y;
+      const float* base = gt + static_cast<size_t>(row) * D + d0;      // local fp32 workspace [N, H, D]
+      f0 = *reinterpret_cast<const float4*>(base);
+      f1 = *reinterpret_cast<const float4*>(base + 4);
     }
-    load_bf16_row<EPL>(xraw, x);
-    if (rotate) {
+    float g[8] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w};
+    float x[8];
+    unpack_bf16x8(ux, x);
+    float2 cs[4];
+    rope_cs4(pd.rope, d0, ti, rotate, cs);
 #pragma unroll
-      for (int i = 0; i < EPL; i += 2) {
-        const float2 cs = rope_cs(pd.rope, (d0 + i) >> 1, pos);
-        const float g0 = g[i], g1 = g[i + 1];
-        g[i] = g0 * cs.x + g1 * cs.y;          // rotate by -phi
-        g[i + 1] = -g0 * cs.y + g1 * cs.x;
-      }
+    for (int i = 0; i < 8; i += 2) {
+      const float2 c = cs[i >> 1];
+      const float g0 = g[i], g1 = g[i + 1];
+      g[i] = g0 * c.x + g1 * c.y;          // rotate by -phi
+      g[i + 1] = -g0 * c.y + g1 * c.x;
     }
-    float y[EPL];
+    float y[8];
     if (!pd.no_norm) {
-      float ss = 0.f, ux = 0.f;
+      float ss = 0.f, uxs = 0.f;
 #pragma unroll
-      for (int i = 0; i < EPL; ++i) {
+      for (int i = 0; i < 8; ++i) {
         ss += x[i] * x[i];
-        ux += gam[i] * g[i] * x[i];
+        uxs += gam[i] * g[i] * x[i];
       }
-      ss = warp_sum(ss);
-      ux = warp_sum(ux);
+      ss = seg_sum<LPR>(ss);
+      uxs = seg_sum<LPR>(uxs);
       const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
-      const float c = rinv * rinv * rinv * ux * (1.0f / D);
+      const float c = rinv * rinv * rinv * uxs * (1.0f / D);
 #pragma unroll
-      for (int i = 0; i < EPL; ++i) {
+      for (int i = 0; i < 8; ++i) {
         y[i] = rinv * gam[i] * g[i] - c * x[i];
-        dgam[i] += g[i] * x[i] * rinv;
+        if (live) dgam[i] += g[i] * x[i] * rinv;
       }
     } else {
 #pragma unroll
-      for (int i = 0; i < EPL; ++i) y[i] = g[i];      // gamma unused: dgamma = 0
+      for (int i = 0; i < 8; ++i) y[i] = g[i];      // gamma unused: dgamma = 0
     }
-    if constexpr (EPL == 4) {
-      uint2 u; u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]);
-      *reinterpret_cast<uint2*>(out) = u;
-    } else {
-      *reinterpret_cast<uint32_t*>(out) = pack_bf16x2(y[0], y[1]);
-    }
+    if (live) *reinterpret_cast<uint4*>(shard_base<__nv_bfloat16>(out_s, shard) + roff) = pack8(y, FMT_BF16);
   }
   if (pp.dgamma_part) {
 #pragma unroll
-    for (int i = 0; i < EPL; ++i) s_part[warp][d0 + i] = dgam[i];
+    for (int i = 0; i < 8; ++i) s_part[warp * RPW + sub][d0 + i] = dgam[i];
     __syncthreads();
     if (threadIdx.x < D) {
       float a = 0.f;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) a += s_part[w][threadIdx.x];
+      for (int w = 0; w < 8 * RPW; ++w) a += s_part[w][threadIdx.x];
       pp.dgamma_part[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * D + threadIdx.x] = a;
     }
   }
