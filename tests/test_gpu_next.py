@@ -136,3 +136,47 @@ def test_cogvideox_shape_full_size(orc):
 
 def test_joint720p_full_size(orc):
     _large_joint(orc, "joint720p", heads=[5, 23], per_seq=24)
+
+
+def test_guard_bands_no_out_of_bounds_writes(orc):
+    """compute-sanitizer is closed on this pool, so out-of-bounds WRITES are looked for directly: every output
+    tensor and the workspace sit inside a larger allocation whose margins hold a sentinel; after forward + backward
+    (fused and deterministic, with dgamma, ragged tails, text tokens) the margins must be untouched."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(1, 10, 13), (2, 9, 11), (1, 1, 1)], 3, 128, index=4, text_lens=[5, 0, 60])   # 135, 198, 61
+    t = inputs.make_inputs(st, device="cuda")
+    N, H, D = st["N"], st["H"], st["D"]
+    G = 4096                                                   # guard elements on each side
+
+    def guarded(numel, dtype, fill):
+        buf = torch.full((numel + 2 * G,), fill, dtype=dtype, device="cuda")
+        return buf, buf[G:G + numel]
+
+    for flags in (0, binding.FLAG_DETERMINISTIC):
+        plan = binding.plan_for(st, flags=flags)
+        bufs = {}
+        for name in ("o", "dq", "dk", "dv"):
+            bufs[name] = guarded(N * H * D, torch.bfloat16, 3.0)
+        bufs["lse"] = guarded(H * N, torch.float32, 3.0)
+        bufs["dgq"] = guarded(D, torch.float32, 3.0)
+        bufs["dgk"] = guarded(D, torch.float32, 3.0)
+        wsb = max(plan.workspace_bytes(False), plan.workspace_bytes(True))
+        bufs["ws"] = guarded(wsb, torch.uint8, 0x5A)
+        v = {k: b[1] for k, b in bufs.items()}
+        o, lse = v["o"].view(N, H, D), v["lse"].view(H, N)
+        binding.arachne_varlen_attn_fwd(plan, t["q"], t["k"], t["v"], o, lse, v["ws"])
+        binding.arachne_varlen_attn_bwd_dgamma(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], v["dq"].view(N, H, D),
+                                               v["dk"].view(N, H, D), v["dv"].view(N, H, D), v["dgq"], v["dgk"], v["ws"])
+        torch.cuda.synchronize()
+        for name, (buf, view) in bufs.items():
+            fill = 0x5A if name == "ws" else 3.0
+            assert bool((buf[:G] == fill).all()) and bool((buf[G + view.numel():] == fill).all()), (name, flags)
+        # and the guarded run computes the right thing
+        a = _np(t)
+        ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], rope_dims=st["rope_dims"],
+                            text_lens=st["text_lens"])
+        got = {"O": o, "LSE": lse, "dQ": v["dq"].view(N, H, D), "dK": v["dk"].view(N, H, D), "dV": v["dv"].view(N, H, D),
+               "dGq": v["dgq"], "dGk": v["dgk"]}
+        pu.check_full(st, got, ref)
+        pu.check_dgamma(got, ref)
+        plan.close()
