@@ -11,7 +11,7 @@ import os
 
 import torch
 
-_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libarachne_attn.so")
+_LIB_PATH = os.environ.get("ARACHNE_ATTN_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "libarachne_attn.so")
 if not os.path.exists(_LIB_PATH):
     raise ImportError(
         f"{_LIB_PATH} is missing: build it with `python -m paper_2607_01701_b200.build` "

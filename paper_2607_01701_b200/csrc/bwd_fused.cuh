@@ -53,7 +53,7 @@ struct BwdFusedCfg {
   static constexpr int kNumBars = 2 + 2 * kQStages + 2 * kDOStages + 9;
   static constexpr int kSmemBytes = kTileBytes * (2 + kQStages + kDOStages) + kDSBytes + kStageBytes +
                                     kQStages * 1024 + 8 * kNumBars + 16;
-  static constexpr int kThreads = 448;
+  static constexpr int kThreads = 512;   // 4 warpgroups: compute, compute, dQ~ drain, {producer, MMA, 2 idle warps}
   static constexpr uint32_t kColS = 0, kColDP = 128, kColDV = 256, kColDK = 256 + D;
 };
 
@@ -65,13 +65,25 @@ __host__ __device__ __forceinline__ uint32_t gq_blk_off(int q, int d) {
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
 }
+// Register re-allocation between warpgroups (512 threads x 128 = the whole register file): the producer / MMA
+// warpgroup gives registers back and the drain warpgroup takes them (no spills anywhere in the kernel).  Holding a
+// whole 128 x D fp32 dQ~ tile in registers to release the TMEM columns before staging was tried and is slower
+// (profiles/r1_notes.md §8): the dQ~ columns are not what the tensor pipe waits for.
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() {
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(N));
+}
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() {
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(N));
+}
 template <int N>
 __device__ __forceinline__ void bulk_wait_group() {
   asm volatile("cp.async.bulk.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
 template <int D>
-__global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFusedParams bp) {
+__global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFusedParams bp) {
   using Cfg = BwdFusedCfg<D>;
   constexpr int TILE = Cfg::kTileBytes;
   constexpr int QS = Cfg::kQStages, DS = Cfg::kDOStages;
@@ -129,6 +141,7 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
 
   if (warp == 12) {
     // ------------------------------------------------------------------ producer
+    setmaxnreg_dec<56>();
     uint32_t it = 0, g = 0;
     for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
       const WorkItem wi = pd.items[item];
@@ -163,6 +176,7 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     }
   } else if (warp == 13) {
     // ------------------------------------------------------------------ MMA issuer
+    setmaxnreg_dec<56>();
     constexpr uint32_t idesc_sdp = make_idesc(128, 128, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
     constexpr uint32_t idesc_dv = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
     constexpr uint32_t idesc_dk = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
@@ -368,6 +382,7 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     }
   } else if (warp < 12) {
     // ------------------------------------------------------------------ dQ~ drain (warps 8-11)
+    setmaxnreg_inc<200>();
     const int q = (warp & 3) * 32 + lane;                      // query row inside the tile == TMEM lane
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tdQ = tbase + Cfg::kColDP + lane_base;
@@ -424,6 +439,8 @@ __global__ void __launch_bounds__(448, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       }
     }
     if (leader) bulk_wait_group<0>();            // all reductions have been performed before the CTA exits
+  } else {
+    setmaxnreg_dec<56>();                        // warps 14-15: only there to complete the fourth warpgroup
   }
   tc_fence_before();
   __syncthreads();
