@@ -195,9 +195,11 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const*
                                     void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
- * memory, pinned or pageable): allocate device buffers, copy in, run on a private stream,
- * copy the results back, free, and return after everything has completed.  These are the
- * calls bench.py times for its "e2e" figure. */
+ * memory; pinned for the copies to overlap the kernels, pageable works but serialises): copy in,
+ * run, copy the results back, and return after everything has completed.  Device buffers and two
+ * private streams are created by the first host call on a plan and kept until arachne_plan_destroy;
+ * dO is uploaded while the forward runs and O, LSE are downloaded while the backward runs.  Not
+ * re-entrant per plan.  These are the calls bench.py times for its "e2e" figure. */
 int arachne_varlen_attn_fwd_host(const arachne_plan* plan, const void* q_host, const void* k_host,
                                  const void* v_host, const float* gamma_q_host,
                                  const float* gamma_k_host, void* o_host, float* lse_host);

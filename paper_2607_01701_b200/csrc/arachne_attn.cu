@@ -40,6 +40,9 @@ bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) !
 
 }  // namespace
 
+struct arachne_host_ctx;
+static void arachne_host_ctx_free(arachne_host_ctx*);
+
 struct arachne_plan {
   arachne_attn_params p;
   std::vector<int32_t> cu;
@@ -48,6 +51,7 @@ struct arachne_plan {
   int n_items = 0;
   int num_sms = 0;
   int device = 0;
+  mutable struct arachne_host_ctx* host = nullptr;   // lazily created by the *_host calls (device buffers, streams)
   Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
   int q_rot = 0;   // fused backward: query-tile rotation per key tile (ARACHNE_BWD_QROT env, tuning)
   // device arrays (owned)
@@ -376,6 +380,7 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
 
 void arachne_plan_destroy(arachne_plan* pl) {
   if (!pl) return;
+  arachne_host_ctx_free(pl->host);
   for (auto& pass : pl->prof_ev)
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
@@ -523,59 +528,103 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* pl, const void* const* q
 }
 
 // ---------------------------------------------------------------- host-buffer convenience calls
-namespace {
-struct DevBufs {
-  std::vector<void*> ptrs;
-  ~DevBufs() { for (void* p : ptrs) cudaFree(p); }
-  int alloc(void** p, size_t bytes) {
-    cudaError_t e = cudaMalloc(p, bytes);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
-    ptrs.push_back(*p);
-    return ARACHNE_OK;
+// Device buffers and the two streams are created on the first host call and cached in the plan (freed by
+// arachne_plan_destroy).  Copies overlap the kernels: dO goes up while the forward runs, O and LSE come down while
+// the backward runs; PCIe is full duplex, so only Q,K,V in front and dQ,dK,dV at the end are exposed.
+struct arachne_host_ctx {
+  void *q = nullptr, *k = nullptr, *v = nullptr, *o = nullptr, *lse = nullptr, *ws = nullptr, *d_o = nullptr, *dq = nullptr,
+       *dk = nullptr, *dv = nullptr, *gq = nullptr, *gk = nullptr;
+  size_t ws_bytes = 0;
+  bool has_bwd = false;
+  cudaStream_t compute = nullptr, copy = nullptr;
+  cudaEvent_t ev_do_up = nullptr, ev_fwd = nullptr, ev_o_down = nullptr, ev_dv = nullptr;
+  ~arachne_host_ctx() {
+    for (void* p : {q, k, v, o, lse, ws, d_o, dq, dk, dv, gq, gk}) cudaFree(p);
+    for (cudaEvent_t e : {ev_do_up, ev_fwd, ev_o_down, ev_dv}) if (e) cudaEventDestroy(e);
+    if (compute) cudaStreamDestroy(compute);
+    if (copy) cudaStreamDestroy(copy);
   }
 };
-}  // namespace
+
+}  // extern "C"
+static void arachne_host_ctx_free(arachne_host_ctx* c) { delete c; }
+extern "C" {
+
+static int host_ctx(const arachne_plan* pl, bool with_bwd, arachne_host_ctx** out) {
+  const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
+  const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
+  const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
+  arachne_host_ctx* c = pl->host;
+  if (!c) {
+    c = new (std::nothrow) arachne_host_ctx();
+    if (!c) { g_last_error = "out of host memory"; return ARACHNE_ERR_CUDA; }
+    pl->host = c;
+    ARACHNE_CUDA(cudaStreamCreateWithFlags(&c->compute, cudaStreamNonBlocking));
+    ARACHNE_CUDA(cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking));
+    for (cudaEvent_t* e : {&c->ev_do_up, &c->ev_fwd, &c->ev_o_down, &c->ev_dv})
+      ARACHNE_CUDA(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    ARACHNE_CUDA(cudaMalloc(&c->q, nb)); ARACHNE_CUDA(cudaMalloc(&c->k, nb)); ARACHNE_CUDA(cudaMalloc(&c->v, nb));
+    ARACHNE_CUDA(cudaMalloc(&c->o, nb)); ARACHNE_CUDA(cudaMalloc(&c->lse, lb));
+    ARACHNE_CUDA(cudaMalloc(&c->gq, gb)); ARACHNE_CUDA(cudaMalloc(&c->gk, gb));
+  }
+  const size_t wsb = std::max(fwd_ws_bytes(pl), with_bwd ? bwd_ws_bytes(pl) : size_t(0));
+  if (c->ws_bytes < wsb) {
+    ARACHNE_CUDA(cudaFree(c->ws)); c->ws = nullptr; c->ws_bytes = 0;
+    ARACHNE_CUDA(cudaMalloc(&c->ws, wsb)); c->ws_bytes = wsb;
+  }
+  if (with_bwd && !c->has_bwd) {
+    ARACHNE_CUDA(cudaMalloc(&c->d_o, nb)); ARACHNE_CUDA(cudaMalloc(&c->dq, nb));
+    ARACHNE_CUDA(cudaMalloc(&c->dk, nb)); ARACHNE_CUDA(cudaMalloc(&c->dv, nb));
+    c->has_bwd = true;
+  }
+  *out = c;
+  return ARACHNE_OK;
+}
 
 static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, const void* k_h, const void* v_h,
                     const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h, void* dq_h,
                     void* dk_h, void* dv_h) {
   if (!pl || !q_h || !k_h || !v_h || !o_h || !lse_h) return ARACHNE_ERR_NULL_POINTER;
   if (with_bwd && (!do_h || !dq_h || !dk_h || !dv_h)) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;
   const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
   const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
   const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
-  DevBufs bufs;
-  void *q, *k, *v, *o, *lse, *ws, *d_o = nullptr, *dq = nullptr, *dk = nullptr, *dv = nullptr, *gq = nullptr, *gk = nullptr;
-  int rc;
-  const size_t wsb = std::max(fwd_ws_bytes(pl), with_bwd ? bwd_ws_bytes(pl) : size_t(0));
-  if ((rc = bufs.alloc(&q, nb)) || (rc = bufs.alloc(&k, nb)) || (rc = bufs.alloc(&v, nb)) || (rc = bufs.alloc(&o, nb)) ||
-      (rc = bufs.alloc(&lse, lb)) || (rc = bufs.alloc(&ws, wsb)))
-    return rc;
-  if (gq_h && (rc = bufs.alloc(&gq, gb))) return rc;
-  if (gk_h && (rc = bufs.alloc(&gk, gb))) return rc;
-  if (with_bwd && ((rc = bufs.alloc(&d_o, nb)) || (rc = bufs.alloc(&dq, nb)) || (rc = bufs.alloc(&dk, nb)) || (rc = bufs.alloc(&dv, nb))))
-    return rc;
-  cudaStream_t st;
-  ARACHNE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
-  struct StreamGuard { cudaStream_t s; ~StreamGuard() { cudaStreamDestroy(s); } } guard{st};
-  ARACHNE_CUDA(cudaMemcpyAsync(q, q_h, nb, cudaMemcpyHostToDevice, st));
-  ARACHNE_CUDA(cudaMemcpyAsync(k, k_h, nb, cudaMemcpyHostToDevice, st));
-  ARACHNE_CUDA(cudaMemcpyAsync(v, v_h, nb, cudaMemcpyHostToDevice, st));
+  arachne_host_ctx* c = nullptr;
+  int rc = host_ctx(pl, with_bwd, &c);
+  if (rc) return rc;
+  cudaStream_t st = c->compute, cp = c->copy;
+  float* gq = gq_h ? static_cast<float*>(c->gq) : nullptr;
+  float* gk = gk_h ? static_cast<float*>(c->gk) : nullptr;
+  ARACHNE_CUDA(cudaMemcpyAsync(c->q, q_h, nb, cudaMemcpyHostToDevice, st));
+  ARACHNE_CUDA(cudaMemcpyAsync(c->k, k_h, nb, cudaMemcpyHostToDevice, st));
+  ARACHNE_CUDA(cudaMemcpyAsync(c->v, v_h, nb, cudaMemcpyHostToDevice, st));
   if (gq) ARACHNE_CUDA(cudaMemcpyAsync(gq, gq_h, gb, cudaMemcpyHostToDevice, st));
   if (gk) ARACHNE_CUDA(cudaMemcpyAsync(gk, gk_h, gb, cudaMemcpyHostToDevice, st));
-  if (with_bwd) ARACHNE_CUDA(cudaMemcpyAsync(d_o, do_h, nb, cudaMemcpyHostToDevice, st));
-  rc = arachne_varlen_attn_fwd(pl, q, k, v, static_cast<float*>(gq), static_cast<float*>(gk), o, static_cast<float*>(lse), ws, wsb, st);
-  if (rc) return rc;
-  ARACHNE_CUDA(cudaMemcpyAsync(o_h, o, nb, cudaMemcpyDeviceToHost, st));
-  ARACHNE_CUDA(cudaMemcpyAsync(lse_h, lse, lb, cudaMemcpyDeviceToHost, st));
-  if (with_bwd) {
-    rc = arachne_varlen_attn_bwd(pl, q, k, v, static_cast<float*>(gq), static_cast<float*>(gk), o, static_cast<float*>(lse), d_o,
-                                 dq, dk, dv, ws, wsb, st);
-    if (rc) return rc;
-    ARACHNE_CUDA(cudaMemcpyAsync(dq_h, dq, nb, cudaMemcpyDeviceToHost, st));
-    ARACHNE_CUDA(cudaMemcpyAsync(dk_h, dk, nb, cudaMemcpyDeviceToHost, st));
-    ARACHNE_CUDA(cudaMemcpyAsync(dv_h, dv, nb, cudaMemcpyDeviceToHost, st));
+  if (with_bwd) {      // dO rides up behind Q,K,V on the copy stream while the forward kernels run
+    ARACHNE_CUDA(cudaEventRecord(c->ev_fwd, st));               // (here: Q,K,V copies issued; keeps the link in order)
+    ARACHNE_CUDA(cudaStreamWaitEvent(cp, c->ev_fwd, 0));
+    ARACHNE_CUDA(cudaMemcpyAsync(c->d_o, do_h, nb, cudaMemcpyHostToDevice, cp));
+    ARACHNE_CUDA(cudaEventRecord(c->ev_do_up, cp));
   }
+  rc = arachne_varlen_attn_fwd(pl, c->q, c->k, c->v, gq, gk, c->o, static_cast<float*>(c->lse), c->ws, c->ws_bytes, st);
+  if (rc) return rc;
+  ARACHNE_CUDA(cudaEventRecord(c->ev_fwd, st));
+  // O and LSE come down on the copy stream while the backward runs
+  ARACHNE_CUDA(cudaStreamWaitEvent(cp, c->ev_fwd, 0));
+  ARACHNE_CUDA(cudaMemcpyAsync(o_h, c->o, nb, cudaMemcpyDeviceToHost, cp));
+  ARACHNE_CUDA(cudaMemcpyAsync(lse_h, c->lse, lb, cudaMemcpyDeviceToHost, cp));
+  ARACHNE_CUDA(cudaEventRecord(c->ev_o_down, cp));
+  if (with_bwd) {
+    ARACHNE_CUDA(cudaStreamWaitEvent(st, c->ev_do_up, 0));
+    rc = arachne_varlen_attn_bwd(pl, c->q, c->k, c->v, gq, gk, c->o, static_cast<float*>(c->lse), c->d_o, c->dq, c->dk,
+                                 c->dv, c->ws, c->ws_bytes, st);
+    if (rc) return rc;
+    ARACHNE_CUDA(cudaMemcpyAsync(dv_h, c->dv, nb, cudaMemcpyDeviceToHost, st));
+    ARACHNE_CUDA(cudaMemcpyAsync(dq_h, c->dq, nb, cudaMemcpyDeviceToHost, st));
+    ARACHNE_CUDA(cudaMemcpyAsync(dk_h, c->dk, nb, cudaMemcpyDeviceToHost, st));
+  }
+  ARACHNE_CUDA(cudaStreamSynchronize(cp));
   ARACHNE_CUDA(cudaStreamSynchronize(st));
   return ARACHNE_OK;
 }

@@ -180,3 +180,31 @@ def test_guard_bands_no_out_of_bounds_writes(orc):
         pu.check_full(st, got, ref)
         pu.check_dgamma(got, ref)
         plan.close()
+
+
+def test_host_entry_points_match_device_calls():
+    """arachne_varlen_attn_fwd_host / _fwd_bwd_host (the calls bench.py times as `e2e`: cached device buffers, two
+    streams, dO uploaded under the forward, O/LSE downloaded under the backward) against the device-pointer calls:
+    bit-identical with the deterministic backward, twice in a row on one plan (buffer reuse), pinned and pageable."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(2, 16, 20), (1, 5, 7), (3, 9, 11)], 3, 128, index=2, text_lens=[0, 9, 0])
+    t = inputs.make_inputs(st, device="cuda")
+    gq, gk = _gammas(128, seed=2)
+    ref = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC, gamma_q=gq, gamma_k=gk)
+    plan = binding.plan_for(st, flags=binding.FLAG_DETERMINISTIC)
+    hgq, hgk = torch.as_tensor(gq), torch.as_tensor(gk)
+    for pinned in (True, False, True):
+        h = {k: (v.cpu().pin_memory() if pinned else v.cpu()) for k, v in t.items()}
+        out = {k: torch.full_like(h["q"], 5.0) for k in ("o", "dq", "dk", "dv")}
+        if pinned:
+            out = {k: v.pin_memory() for k, v in out.items()}
+        lse = torch.zeros((plan.H, plan.N), dtype=torch.float32)
+        binding.arachne_varlen_attn_fwd_host(plan, h["q"], h["k"], h["v"], out["o"], lse, hgq, hgk)
+        assert torch.equal(out["o"], ref["O"].cpu()) and torch.equal(lse, ref["LSE"].cpu())
+        out["o"].fill_(5.0); lse.zero_()
+        binding.arachne_varlen_attn_fwd_bwd_host(plan, h["q"], h["k"], h["v"], h["dO"], out["o"], lse, out["dq"], out["dk"],
+                                                 out["dv"], hgq, hgk)
+        assert torch.equal(out["o"], ref["O"].cpu()) and torch.equal(lse, ref["LSE"].cpu())
+        for a, b in (("dq", "dQ"), ("dk", "dK"), ("dv", "dV")):
+            assert torch.equal(out[a], ref[b].cpu()), a
+    plan.close()
