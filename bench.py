@@ -26,8 +26,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1_ncu_full_720p.md); only known for the workload that was captured.
-NCU_TRAFFIC = {("long720p", "bwd_main(fused 5-GEMM | det: dKdV pass)"): 48.74e9, ("long720p", "fwd_kernel"): 11.0e9}
+# `ncu --set full` capture (profiles/r1b_ncu_720p.md); only known for the workload that was captured.
+NCU_TRAFFIC = {("long720p", "bwd_main(fused 5-GEMM | det: dKdV pass)"): 47.08e9, ("long720p", "fwd_kernel"): 11.6e9}
 
 METRIC = "varlen 3D attention fwd+bwd TFLOPS"
 UNIT = "TFLOP/s"
@@ -274,7 +274,7 @@ def main():
     achieved = dom_flops / (dom["ms"] * 1e-3) / 1e12 if dom["ms"] > 0 else 0.0
     roofline = {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peaks["sustained"], "unit": "TFLOP/s",
                 "frac": achieved / peaks["sustained"], "traffic": NCU_TRAFFIC.get((args.workload, dom["name"])),
-                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r1_ncu_full_720p.md)",
+                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r1b_ncu_720p.md)",
                 "peak_source": peaks["source"] + ", bf16_tflops_sustained (kernel timed inside a long step)",
                 "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": calls_b}
 
