@@ -60,6 +60,9 @@ struct arachne_plan {
   TokInfo* d_tok_info = nullptr;
   WorkItem* d_items = nullptr;
   WorkItem* d_fwd_items = nullptr;
+  int* d_item_ptr = nullptr;
+  int* d_fwd_item_ptr = nullptr;
+  int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
   unsigned* d_stats = nullptr;
   float2* d_rope = nullptr;
@@ -117,7 +120,7 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
   FwdParams fp{f.qt, f.kt, f.vt, o, lse};
-  const int grid = std::min(pl->num_sms, pl->n_fwd_items);
+  const int grid = pl->n_fwd_ctas;
   fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
@@ -152,7 +155,7 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
-  const int grid = std::min(pl->num_sms, pl->n_items);
+  const int grid = pl->n_ctas;
   if (deterministic) {
     // two-pass (7 GEMM) path: every output tile owned by one CTA, fixed summation order
     BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv};
@@ -301,6 +304,30 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
       for (int t = 0; t < pl->seqs[b].n_tiles; t += 2)
         fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].n_tiles - t)});
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
+  // Static LPT assignment to the persistent CTAs: the lists are in decreasing-cost order, each item goes to the
+  // least-loaded CTA (ties: lowest index — while costs are equal this is round-robin, so CTAs running side by side
+  // stay on adjacent tiles of the same (sequence, head) group), and every CTA's items are stored contiguously.
+  auto deal = [&](std::vector<WorkItem>& list, int n_cta, auto cost, std::vector<int>& ptr) {
+    std::vector<long long> load(n_cta, 0);
+    std::vector<std::vector<WorkItem>> own(n_cta);
+    for (const WorkItem& w : list) {
+      int best = 0;
+      for (int c = 1; c < n_cta; ++c) if (load[c] < load[best]) best = c;
+      own[best].push_back(w);
+      load[best] += cost(w);
+    }
+    list.clear();
+    ptr.assign(1, 0);
+    for (int c = 0; c < n_cta; ++c) {
+      list.insert(list.end(), own[c].begin(), own[c].end());
+      ptr.push_back(static_cast<int>(list.size()));
+    }
+  };
+  std::vector<int> item_ptr, fwd_item_ptr;
+  pl->n_ctas = std::min(pl->num_sms, pl->n_items);
+  pl->n_fwd_ctas = std::min(pl->num_sms, pl->n_fwd_items);
+  deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].n_tiles); }, item_ptr);
+  deal(fwd_items, pl->n_fwd_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].n_tiles) * w.pad; }, fwd_item_ptr);
   // RoPE tables in fp64 -> fp32 (readings R4, R5)
   std::vector<float2> tab;
   RopeDesc rd{};
@@ -340,6 +367,8 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   }
   PLAN_UP(pl->d_items, items, WorkItem)
   PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
+  PLAN_UP(pl->d_item_ptr, item_ptr, int)
+  PLAN_UP(pl->d_fwd_item_ptr, fwd_item_ptr, int)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_stats), 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
@@ -349,7 +378,7 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.item_ptr = pl->d_item_ptr; pd.fwd_item_ptr = pl->d_fwd_item_ptr; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -385,7 +414,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_fwd_item_ptr); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
   delete pl;
 }
 

@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
     // ------------------------------------------------------------------ producer
     if (lane == 0) {
       uint32_t it = 0, yt = 0;
-      for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+      for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
         const WorkItem wi = pd.items[item];
         const SeqInfo sq = pd.seqs[wi.seq];
         const size_t hoff = wi.head * head_stride;
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
         }
         __syncwarp();
       };
-      for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+      for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
         const WorkItem wi = pd.items[item];
         const uint32_t G = 2u * pd.seqs[wi.seq].n_tiles;
         mbar_wait(x_full, it & 1);
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
     const uint32_t lane_base = static_cast<uint32_t>(warp * 32) << 16;
     const int row = threadIdx.x;
     uint32_t it = 0, yt = 0, g = 0;
-    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const uint32_t G = 2u * sq.n_tiles;

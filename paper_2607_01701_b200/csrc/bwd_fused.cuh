@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     // ------------------------------------------------------------------ producer
     setmaxnreg_dec<56>();
     uint32_t it = 0, g = 0;
-    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const size_t hoff = wi.head * head_stride;
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       }
       __syncwarp();
     };
-    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
       const uint32_t n = pd.seqs[wi.seq].n_tiles;
       mbar_wait(kv_full, it & 1);
@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     const uint32_t tdP = tbase + Cfg::kColDP + lane_base + wg * 64;
     uint8_t* dS_row = sdS + wg * BLK + r * 128;                // this row's 128 bytes in block wg of the dS^T image
     uint32_t it = 0, g = 0;
-    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x, ++it) {
+    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       for (int i = 0; i < sq.n_tiles; ++i, ++g) {
@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
         bulk_commit_group();
       }
     };
-    for (int item = blockIdx.x; item < pd.n_items; item += gridDim.x) {
+    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       for (int i = 0; i < sq.n_tiles; ++i, ++g) {

@@ -30,7 +30,8 @@ struct TokInfo {
 
 // One unit of work for every persistent kernel: (sequence, head, 128-token tile of that sequence).
 // Forward / dQ kernels read it as a QUERY tile, the dK/dV kernel as a KEY tile.  The host orders
-// the list longest-processing-time-first by (sequence, head) group, tiles of a group adjacent.
+// the list longest-processing-time-first by (sequence, head) group, tiles of a group adjacent, then deals the items
+// to the persistent CTAs greedily (each item to the least-loaded CTA) and stores every CTA's items contiguously.
 struct WorkItem {
   int seq;
   int head;
@@ -98,6 +99,8 @@ struct ProblemDesc {
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
   const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int n_fwd_items;
+  const int* item_ptr;       // [n_ctas + 1] CTA c owns items [item_ptr[c], item_ptr[c+1]) (host LPT assignment)
+  const int* fwd_item_ptr;   // [n_fwd_ctas + 1] likewise for fwd_items
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel
   int n_items;
   int n_tiles_total;

@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   if (warp == 8) {
     // ------------------------------------------------------------------ producer
     uint32_t it = 0, ring = 0;
-    for (int item = blockIdx.x; item < pd.n_fwd_items; item += gridDim.x, ++it) {
+    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.fwd_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const int n_q = wi.pad;
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     const uint32_t aQ = smem_u32(sQ), aKV = smem_u32(sKV);
     uint32_t it = 0, ring = 0;      // ring: slot counter at K_0 of the current item (K_j = ring+2j, V_j = ring+2j+1)
     uint32_t cnt[2] = {0, 0};       // per query tile: number of PV tiles issued so far
-    for (int item = blockIdx.x; item < pd.n_fwd_items; item += gridDim.x, ++it) {
+    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.fwd_items[item];
       const int n_kv = pd.seqs[wi.seq].n_tiles;
       const int n_q = wi.pad;
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     // range.  Anything larger (no_norm debug flag, huge gamma) takes the online-softmax path below.
     const float bound = sqrtf(__uint_as_float(pd.stats[0])) * sqrtf(__uint_as_float(pd.stats[1]));
     const bool static_max = bound <= kStaticMaxBound;     // false for NaN / inf
-    for (int item = blockIdx.x; item < pd.n_fwd_items; item += gridDim.x, ++it) {
+    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.fwd_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       if (t >= wi.pad) {
