@@ -38,6 +38,10 @@ struct FwdCfg {
   static constexpr int kNumBars = 2 + 2 * kRing + 8;
   static constexpr int kSmemBytes = kTileBytes * (2 + kRing) + 8 * kNumBars + 16;
   static constexpr int kThreads = 320;
+  // every 4th exp2 on the FMA pipe (ex2_poly3) instead of MUFU: pays at D = 64, where MUFU (16 ex2/clk/SM) is the
+  // busiest unit (cogvideox fwd 13.0 vs 14.7 ms); at D = 128 the loop is tensor/power-bound and the extra FMA-pipe
+  // instructions cost more than they save (720p fwd 148.0 ms without vs 152.7 ms with; profiles/r1_notes.md §10)
+  static constexpr bool kPolyExp = (D == 64);
   // TMEM columns: S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [256+D,256+2D)
   static constexpr uint32_t kColS = 0, kColO = 256;
 };
@@ -200,8 +204,8 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
       float m = 0.f, l = 0.f;
       if (static_max) {
         // ---- static-max softmax: p = 2^s', no row max, no rescale; 32-column chunks, the TMEM load of
-        // chunk c+1 in flight while chunk c is exponentiated; every 4th exp2 on the FMA pipe (MUFU is
-        // the co-critical unit: 16 ex2/clk/SM = 1024 clk per 128x128 tile).
+        // chunk c+1 in flight while chunk c is exponentiated; at D = 64 every 4th exp2 on the FMA pipe
+        // (Cfg::kPolyExp; MUFU: 16 ex2/clk/SM = 1024 clk per 128x128 tile).
         float rs0 = 0.f, rs1 = 0.f;
         for (int j = 0; j < sq.n_tiles; ++j, ++g) {
           mbar_wait(&s_full[t], g & 1);
@@ -220,7 +224,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
 #pragma unroll
               for (int i = 0; i < 32; i += 2) {
                 const float p0 = ex2_approx(__uint_as_float(cur[i]));
-                const float p1 = (i & 2) ? ex2_poly3(__uint_as_float(cur[i + 1])) : ex2_approx(__uint_as_float(cur[i + 1]));
+                const float p1 = (Cfg::kPolyExp && (i & 2)) ? ex2_poly3(__uint_as_float(cur[i + 1])) : ex2_approx(__uint_as_float(cur[i + 1]));
                 rs0 += p0; rs1 += p1;
                 pk[i >> 1] = pack_bf16x2(p0, p1);
               }
