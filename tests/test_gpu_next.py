@@ -208,3 +208,42 @@ def test_host_entry_points_match_device_calls():
         for a, b in (("dq", "dQ"), ("dk", "dK"), ("dv", "dV")):
             assert torch.equal(out[a], ref[b].cpu()), a
     plan.close()
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_packings(orc, seed):
+    """Seeded random packings (sequence count, grids, text lengths, heads, head_dim, RoPE split, gamma, backward mode,
+    sequence order): every output element by element against the oracle.  Lengths are drawn around tile edges
+    (1 .. ~700 tokens) so that single-row tails, exact multiples of 128 and sub-tile sequences all occur."""
+    from paper_2607_01701_b200 import binding
+    rng = np.random.default_rng(1000 + seed)
+    D = int(rng.choice([64, 128]))
+    H = int(rng.integers(1, 6))
+    B = int(rng.integers(1, 7))
+    grids, text = [], []
+    for _ in range(B):
+        kind = rng.integers(0, 4)
+        if kind == 0:
+            g = (1, 1, int(rng.integers(1, 130)))
+        elif kind == 1:
+            g = (int(rng.integers(1, 4)), 8, 16)                       # multiples of 128
+        else:
+            g = (int(rng.integers(1, 5)), int(rng.integers(1, 14)), int(rng.integers(1, 14)))
+        grids.append(g)
+        text.append(int(rng.choice([0, 0, 1, 7, 77, 128])))
+    half = D // 2
+    a = 2 * int(rng.integers(0, half // 2 + 1)); b = 2 * int(rng.integers(0, (D - a) // 4 + 1))
+    rope = (a, b, D - a - b)
+    st = inputs.pack(grids, H, D, index=7, rope_dims=rope, text_lens=text, order=str(rng.choice(["listed", "reversed", "shuffled"])),
+                     seed=seed)
+    t = inputs.make_inputs(st, device="cuda")
+    gq = (0.5 + rng.random(D)).astype(np.float32)
+    gk = (0.5 + rng.random(D)).astype(np.float32)
+    flags = binding.FLAG_DETERMINISTIC if rng.integers(0, 2) else 0
+    got = pu.run_gpu(st, t, flags=flags, gamma_q=gq, gamma_k=gk, with_dgamma=True)
+    x = _np(t)
+    ref = orc.attention(x["q"], x["k"], x["v"], st["cu_seqlens"], st["grids"], dO=x["dO"], gamma_q=gq, gamma_k=gk,
+                        rope_dims=rope, text_lens=st["text_lens"])
+    w = pu.check_full(st, got, ref)
+    w.update(pu.check_dgamma(got, ref))
+    print(seed, D, H, st["grids"], st["text_lens"], rope, flags, {k: f"{v:.1e}" for k, v in w.items()})
