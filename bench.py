@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
+    ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -185,7 +186,7 @@ def main():
 
     # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
     # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
-    st = inputs.structure(args.workload, order=args.order)
+    st = inputs.structure(args.workload, order=args.order, seed_offset=args.seed_offset)
     st["name"] = args.workload
     st_r = dict(st, index=st["index"])          # same structure on every rank; different bytes per rank
     t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * rank, dev)
@@ -292,7 +293,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": args.workload, "order": args.order, "num_seqs": len(st["grids"]), "total_tokens": st["N"],
+        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "num_seqs": len(st["grids"]), "total_tokens": st["N"],
                    "heads": st["H"], "head_dim": st["D"], "flop_per_step": flops,
                    "l2": "inputs larger than L2 (4 x %.0f MB bf16 tensors + tiled workspace)" % (t["q"].numel() * 2 / 1e6),
                    "pct_of_measured_bf16_burst": 100.0 * value / world / peaks["burst"],
