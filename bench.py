@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
+    ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC: two-pass backward, no atomics")
     ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -191,7 +192,7 @@ def main():
     st_r = dict(st, index=st["index"])          # same structure on every rank; different bytes per rank
     t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * rank, dev)
          for tid, k in ((1, "q"), (2, "k"), (3, "v"), (4, "dO"))}
-    plan = binding.plan_for(st_r)
+    plan = binding.plan_for(st_r, flags=binding.FLAG_DETERMINISTIC if args.deterministic else 0)
     ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
     o = torch.empty_like(t["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=dev)
     dq, dk, dv = (torch.empty_like(t["q"]) for _ in range(3))
@@ -293,7 +294,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "num_seqs": len(st["grids"]), "total_tokens": st["N"],
+        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "deterministic_bwd": bool(args.deterministic), "num_seqs": len(st["grids"]), "total_tokens": st["N"],
                    "heads": st["H"], "head_dim": st["D"], "flop_per_step": flops,
                    "l2": "inputs larger than L2 (4 x %.0f MB bf16 tensors + tiled workspace)" % (t["q"].numel() * 2 / 1e6),
                    "pct_of_measured_bf16_burst": 100.0 * value / world / peaks["burst"],
