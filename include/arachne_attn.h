@@ -194,6 +194,37 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const*
                                     float* dgamma_q, float* dgamma_k,
                                     void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* CONTEXT PARALLELISM ("CP ... partitions the sequence ... K/V ring") without a
+ * ring: the packed batch is split by token range into num_shards buffers exactly as for arachne_plan_create_sharded
+ * (shard r = [n_r, num_heads, D], ALL heads), and rank `rank` computes, for ALL heads, the attention of ITS query
+ * tokens [shard_starts[rank], shard_starts[rank+1]) against all keys of their sequences — K and V rows of the other
+ * ranks are read straight from their shards (peer memory; the all-gather of K/V is these loads).
+ *   forward : arachne_varlen_attn_fwd_sharded with this plan; only O rows of the rank's own tokens are written (so only
+ *             o[rank] is touched) and only those columns of the LOCAL lse [num_heads, N] are defined.
+ *   backward: (1) arachne_varlen_attn_bwd_cp_partial on every rank: finishes dQ for the rank's own rows (writes
+ *             dq[rank]) and leaves dk~, dV as fp32 PARTIAL sums over the rank's query rows in dk_partial, dv_partial
+ *             (fp32 [N, num_heads, D] DEVICE buffers that the other ranks can read; rows of sequences the rank does
+ *             not touch are left unwritten);  (2) after a barrier, arachne_cp_reduce on every rank: for the rank's own
+ *             key tokens adds the partials of the contributing ranks in RANK ORDER (fixed order; the reduce-scatter
+ *             is these peer loads), applies un-RoPE + RMSNorm backward, and writes dk[rank], dv[rank] (bf16) and
+ *             dgamma_k (this rank's part; all-reduce it).  dgamma_q comes from step (1) (this rank's part).
+ * Sequences may straddle the cuts; rows of a boundary tile that belong to another rank are masked (P = 0), so nothing
+ * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): CP runs the fused backward.
+ * Workspace for both backward calls: arachne_workspace_bytes(plan, 1).  A rank may own no tokens (empty shard). */
+int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params,
+                           const int32_t* cu_seqlens_host, const int32_t* grids_host,
+                           const int32_t* text_lens_host, int32_t num_shards,
+                           const int32_t* shard_starts_host, int32_t rank);
+int arachne_varlen_attn_bwd_cp_partial(const arachne_plan* plan, const void* const* q, const void* const* k,
+                                       const void* const* v, const float* gamma_q, const float* gamma_k,
+                                       const void* const* o, const float* lse, const void* const* d_o,
+                                       void* const* dq, float* dk_partial, float* dv_partial, float* dgamma_q,
+                                       void* workspace, size_t workspace_bytes, void* cuda_stream);
+/* dk_partials / dv_partials: HOST arrays of num_shards DEVICE pointers (rank r's dk_partial / dv_partial). */
+int arachne_cp_reduce(const arachne_plan* plan, const float* const* dk_partials, const float* const* dv_partials,
+                      const void* const* k, const float* gamma_k, void* const* dk, void* const* dv,
+                      float* dgamma_k, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
  * memory; pinned for the copies to overlap the kernels, pageable works but serialises): copy in,
  * run, copy the results back, and return after everything has completed.  Device buffers and two

@@ -27,6 +27,7 @@ EXPORTS = [
     "arachne_kernel_name", "arachne_plan_enable_profiling", "arachne_plan_kernel_times",
     "arachne_plan_create_joint", "arachne_varlen_attn_bwd_dgamma",
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
+    "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
 ]
 
 
@@ -64,6 +65,14 @@ _lib.arachne_varlen_attn_fwd_sharded.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vp
 _lib.arachne_varlen_attn_bwd_sharded.restype = ctypes.c_int
 _lib.arachne_varlen_attn_bwd_sharded.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vp, _vpp, _vp, _vpp, _vpp, _vpp, _vpp,
                                                  _vp, _vp, _vp, ctypes.c_size_t, _vp]
+_lib.arachne_plan_create_cp.restype = ctypes.c_int
+_lib.arachne_plan_create_cp.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(AttnParams), _i32p, _i32p, _i32p,
+                                        ctypes.c_int32, _i32p, ctypes.c_int32]
+_lib.arachne_varlen_attn_bwd_cp_partial.restype = ctypes.c_int
+_lib.arachne_varlen_attn_bwd_cp_partial.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vp, _vpp, _vp, _vpp, _vpp, _vp, _vp, _vp,
+                                                    _vp, ctypes.c_size_t, _vp]
+_lib.arachne_cp_reduce.restype = ctypes.c_int
+_lib.arachne_cp_reduce.argtypes = [_vp, _vpp, _vpp, _vpp, _vp, _vpp, _vpp, _vp, _vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_fwd_host.restype = ctypes.c_int
 _lib.arachne_varlen_attn_fwd_host.argtypes = [_vp] * 8
 _lib.arachne_varlen_attn_fwd_bwd_host.restype = ctypes.c_int
@@ -104,7 +113,7 @@ class Plan:
     is then the LOCAL head count."""
 
     def __init__(self, cu_seqlens, grids, num_heads, head_dim, rope_dims, rope_theta=10000.0, rms_eps=1e-6,
-                 softmax_scale=0.0, flags=0, text_lens=None, shard_starts=None, total_heads=None, head_offset=0):
+                 softmax_scale=0.0, flags=0, text_lens=None, shard_starts=None, total_heads=None, head_offset=0, cp_rank=None):
         cu = [int(x) for x in cu_seqlens]
         gr = [int(x) for g in grids for x in g]
         self.params = AttnParams()
@@ -129,8 +138,12 @@ class Plan:
             if text_lens is not None:
                 tl = [int(x) for x in text_lens]
                 tl_arr = (ctypes.c_int32 * max(len(tl), 1))(*tl)
-            _check(_lib.arachne_plan_create_sharded(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr,
-                                                    self.num_shards, ss_arr, int(total_heads or num_heads), int(head_offset)))
+            if cp_rank is not None:      # context parallelism: arachne_plan_create_cp
+                _check(_lib.arachne_plan_create_cp(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr,
+                                                   self.num_shards, ss_arr, int(cp_rank)))
+            else:
+                _check(_lib.arachne_plan_create_sharded(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr,
+                                                        self.num_shards, ss_arr, int(total_heads or num_heads), int(head_offset)))
         elif text_lens is None:
             _check(_lib.arachne_plan_create(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr))
         else:
@@ -221,6 +234,25 @@ def arachne_varlen_attn_bwd_sharded(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv
                                                 _ptr_array(d_o, n), _ptr_array(dq, n), _ptr_array(dk, n), _ptr_array(dv, n),
                                                 _ptr(dgamma_q), _ptr(dgamma_k), _ptr(workspace),
                                                 workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
+def arachne_varlen_attn_bwd_cp_partial(plan: Plan, q, k, v, o, lse, d_o, dq, dk_partial, dv_partial, workspace, dgamma_q=None,
+                                       gamma_q=None, gamma_k=None, stream=None):
+    """Context parallelism, step 1: dq[rank] finished; dk_partial, dv_partial: fp32 CUDA [N,H,D] (this rank's partials)."""
+    n = plan.num_shards
+    _check(_lib.arachne_varlen_attn_bwd_cp_partial(plan._h, _ptr_array(q, n), _ptr_array(k, n), _ptr_array(v, n),
+                                                   _ptr(gamma_q), _ptr(gamma_k), _ptr_array(o, n), _ptr(lse),
+                                                   _ptr_array(d_o, n), _ptr_array(dq, n), _ptr(dk_partial), _ptr(dv_partial),
+                                                   _ptr(dgamma_q), _ptr(workspace),
+                                                   workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+
+
+def arachne_cp_reduce(plan: Plan, dk_partials, dv_partials, k, dk, dv, workspace, dgamma_k=None, gamma_k=None, stream=None):
+    """Context parallelism, step 2: dk_partials / dv_partials are lists of every rank's partial buffers."""
+    n = plan.num_shards
+    _check(_lib.arachne_cp_reduce(plan._h, _ptr_array(dk_partials, n), _ptr_array(dv_partials, n), _ptr_array(k, n),
+                                  _ptr(gamma_k), _ptr_array(dk, n), _ptr_array(dv, n), _ptr(dgamma_k), _ptr(workspace),
+                                  workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
 
 
 def arachne_varlen_attn_fwd_host(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None):

@@ -1,0 +1,117 @@
+"""Context parallelism without a ring ("CP ... K/V ring").
+
+Each rank owns a contiguous token range of the packed batch (all heads) and computes the attention of ITS query tokens
+against all keys of their sequences.  Inside one NVSwitch domain the K/V "ring" is unnecessary: the kernels read the
+other ranks' K and V rows straight from their shards (peer memory), and the reduce-scatter of dK / dV is the owner
+reading the other ranks' fp32 partials in rank order (include/arachne_attn.h: arachne_plan_create_cp,
+arachne_varlen_attn_bwd_cp_partial, arachne_cp_reduce).  Unlike Ulysses the degree is not tied to the head count.
+
+This module holds the integer bookkeeping (mirrors of what the plan computes, used by the tests and for sizing) and
+the multi-GPU driver; no attention arithmetic.  Verified: kernels on one GPU with k shard buffers
+(tests/test_gpu_ulysses.py), bookkeeping on CPU (tests/test_ulysses_gloo.py); not run on k GPUs (one-GPU pool).
+"""
+from __future__ import annotations
+
+from typing import List, Sequence, Tuple
+
+TILE = 128
+
+
+def query_tile_range(seq_start: int, seq_len: int, lo: int, hi: int) -> Tuple[int, int]:
+    """(first tile, tile count) of a sequence's 128-row query tiles that hold tokens of [lo, hi) (global indices)."""
+    a, b = max(lo, seq_start), min(hi, seq_start + seq_len)
+    if a >= b:
+        return 0, 0
+    first = (a - seq_start) // TILE
+    return first, (b - 1 - seq_start) // TILE + 1 - first
+
+
+def contributors(starts: Sequence[int], seq_start: int, seq_len: int) -> List[int]:
+    """Ranks whose query range intersects the sequence: the ranks whose dK / dV partials its keys must sum."""
+    return [r for r in range(len(starts) - 1)
+            if starts[r + 1] > starts[r] and starts[r] < seq_start + seq_len and starts[r + 1] > seq_start]
+
+
+def rank_cost(cu_seqlens: Sequence[int], lo: int, hi: int) -> int:
+    """Quadratic cost (query rows x keys) of the rank that owns queries [lo, hi): sum over sequences of rows * L
+    (Eq. 9's alpha2 term).  Equal token counts do NOT mean equal cost when lengths differ."""
+    c = 0
+    for b in range(len(cu_seqlens) - 1):
+        s, e = cu_seqlens[b], cu_seqlens[b + 1]
+        rows = max(0, min(hi, e) - max(lo, s))
+        c += rows * (e - s)
+    return c
+
+
+def balanced_starts(cu_seqlens: Sequence[int], world_size: int) -> List[int]:
+    """Token cuts that equalise rank_cost (not token counts): walk the tokens in order, cut when the running cost
+    passes r/k of the total.  Cuts may fall inside a sequence."""
+    N = cu_seqlens[-1]
+    total = rank_cost(cu_seqlens, 0, N)
+    starts, acc, r = [0], 0, 1
+    for b in range(len(cu_seqlens) - 1):
+        s, e = cu_seqlens[b], cu_seqlens[b + 1]
+        L = e - s
+        while r < world_size and acc + L * L >= total * r / world_size:
+            need = total * r / world_size - acc            # cost still missing for cut r, at L per row
+            starts.append(min(e, s + int(-(-need // L))))
+            r += 1
+        acc += L * L
+    while len(starts) < world_size:
+        starts.append(N)
+    return starts + [N]
+
+
+class ContextParallelAttention:
+    """Forward / backward over a CP group of k GPUs in one NVSwitch domain (torch.distributed + symmetric memory).
+    forward(): barrier -> fwd_sharded -> (no barrier needed: a rank writes only its own O shard).
+    backward(): barrier -> bwd_cp_partial -> barrier -> cp_reduce -> all-reduce of the dgamma parts."""
+
+    def __init__(self, st: dict, group=None, starts=None):
+        import torch
+        import torch.distributed as dist
+        import torch.distributed._symmetric_memory as symm_mem
+
+        from . import binding
+        from .ulysses import SymmetricShards
+
+        self.group, self._dist, self._binding = group, dist, binding
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.starts = list(starts) if starts is not None else balanced_starts(st["cu_seqlens"], self.world)
+        self.n_local = self.starts[self.rank + 1] - self.starts[self.rank]
+        n_max = max(self.starts[r + 1] - self.starts[r] for r in range(self.world))
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.plan = binding.Plan(st["cu_seqlens"], st["grids"], st["H"], st["D"], st["rope_dims"],
+                                 text_lens=st.get("text_lens"), shard_starts=self.starts, cp_rank=self.rank)
+        self.buf = {n: SymmetricShards(n_max, st["H"], st["D"], group, dev) for n in ("q", "k", "v", "o", "dO", "dq", "dk", "dv")}
+        self.part = {}
+        for n in ("dk_partial", "dv_partial"):
+            t = symm_mem.empty((st["N"], st["H"], st["D"]), dtype=torch.float32, device=dev)
+            self.part[n] = (t, [int(p) for p in symm_mem.rendezvous(t, group=group).buffer_ptrs])
+        self.lse = torch.empty((st["H"], st["N"]), dtype=torch.float32, device=dev)
+        self.ws = torch.empty(max(self.plan.workspace_bytes(False), self.plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
+
+    def _barrier(self):
+        import torch
+
+        torch.cuda.current_stream().synchronize()
+        self._dist.barrier(self.group)
+
+    def forward(self, gamma_q=None, gamma_k=None):
+        b = self.buf
+        self._barrier()
+        self._binding.arachne_varlen_attn_fwd_sharded(self.plan, b["q"].ptrs, b["k"].ptrs, b["v"].ptrs, b["o"].ptrs, self.lse,
+                                                      self.ws, gamma_q, gamma_k)
+        return b["o"].local(self.n_local)
+
+    def backward(self, gamma_q=None, gamma_k=None):
+        b = self.buf
+        self._barrier()
+        self._binding.arachne_varlen_attn_bwd_cp_partial(self.plan, b["q"].ptrs, b["k"].ptrs, b["v"].ptrs, b["o"].ptrs, self.lse,
+                                                         b["dO"].ptrs, b["dq"].ptrs, self.part["dk_partial"][0],
+                                                         self.part["dv_partial"][0], self.ws, None, gamma_q, gamma_k)
+        self._barrier()
+        self._binding.arachne_cp_reduce(self.plan, self.part["dk_partial"][1], self.part["dv_partial"][1], b["k"].ptrs,
+                                        b["dk"].ptrs, b["dv"].ptrs, self.ws, None, gamma_k)
+        self._barrier()
+        return b["dq"].local(self.n_local), b["dk"].local(self.n_local), b["dv"].local(self.n_local)

@@ -52,6 +52,7 @@ struct arachne_plan {
   int num_sms = 0;
   int device = 0;
   mutable struct arachne_host_ctx* host = nullptr;   // lazily created by the *_host calls (device buffers, streams)
+  int cp_rank = -1;   // >= 0: context-parallel plan (arachne_plan_create_cp), this process owns the queries of shard cp_rank
   Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
   int q_rot = 0;   // fused backward: query-tile rotation per key tile (ARACHNE_BWD_QROT env, tuning)
   // device arrays (owned)
@@ -78,6 +79,10 @@ struct arachne_plan {
   mutable long long prof_calls[2] = {0, 0};
   cudaEvent_t prof_ev[2][kProfSlots][kMaxKernels + 1] = {};
 };
+
+static int plan_create_impl(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
+                            const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts,
+                            int32_t total_heads, int32_t head_offset, int cp_rank);
 
 namespace {
 
@@ -121,7 +126,7 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   prof_mark(pl, 0, 1, st);
   FwdParams fp{f.qt, f.kt, f.vt, o, lse};
   const int grid = pl->n_fwd_ctas;
-  fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);
+  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);   // (a CP rank may own no queries)
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
   if (pl->profiling) pl->prof_calls[0]++;
@@ -131,7 +136,11 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
 template <int D>
 int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k, const ShardedPtr& v, const float* gq,
                const float* gk, const ShardedPtr& o, const float* lse, const ShardedPtr& d_o, const ShardedPtr& dq,
-               const ShardedPtr& dk, const ShardedPtr& dv, float* dgq, float* dgk, void* ws, cudaStream_t st) {
+               const ShardedPtr& dk, const ShardedPtr& dv, float* dgq, float* dgk, void* ws, cudaStream_t st,
+               float* cp_gk = nullptr, float* cp_gv = nullptr) {
+  // cp_gk / cp_gv (context parallelism, phase 1): dk~ and dV leave as fp32 PARTIALS in these [N,H,D] buffers, only dQ is
+  // finished here (for this rank's query rows); arachne_cp_reduce finishes dK, dV.
+  const bool cp = cp_gk != nullptr;
   uint8_t* w = static_cast<uint8_t*>(ws);
   BwdWs b{};
   b.qt = w; w += pl->img_bytes;
@@ -143,6 +152,7 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   b.gk_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
   b.gq_t = reinterpret_cast<float*>(w); w += pl->gradblk_bytes;     // gradblk_bytes >= grad_bytes: either layout fits
   float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
+  if (cp) b.gk_t = cp_gk;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
   PrepParams pp{};
   pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse; pp.backward = 1;
@@ -167,14 +177,14 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
     prof_mark(pl, 1, 3, st);
   } else {
     // fused single-pass (5 GEMM) path: dQ~ partial tiles reduce-added at L2 (order not fixed)
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, pl->q_rot};
-    bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pl->pd, bp);
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, pl->q_rot};
+    if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pl->pd, bp);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
     prof_mark(pl, 1, 3, st);
   }
-  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, q, k, gq, gk, dq, dk, dgpart};
-  post_kernel<D><<<dim3(pl->post_blocks, 2), 256, 0, st>>>(pl->pd, po);
+  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
+  post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
     dgamma_reduce_kernel<D><<<2, 256, 0, st>>>(dgpart, pl->post_blocks, dgq, dgk);
@@ -223,6 +233,21 @@ int arachne_plan_create_joint(arachne_plan** out, const arachne_attn_params* par
 int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
                                 const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts,
                                 int32_t total_heads, int32_t head_offset) {
+  return plan_create_impl(out, params, cu, grids, text_lens, num_shards, shard_starts, total_heads, head_offset, -1);
+}
+
+int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
+                           const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts, int32_t rank) {
+  if (!params) return ARACHNE_ERR_NULL_POINTER;
+  if (rank < 0 || rank >= num_shards) return ARACHNE_ERR_BAD_SHARDING;
+  if (params->flags & ARACHNE_FLAG_DETERMINISTIC) return ARACHNE_ERR_BAD_PARAM;   // CP runs the fused backward only
+  return plan_create_impl(out, params, cu, grids, text_lens, num_shards, shard_starts, params->num_heads, 0, rank);
+}
+
+}  // extern "C"
+static int plan_create_impl(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids,
+                            const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts,
+                            int32_t total_heads, int32_t head_offset, int cp_rank) {
   if (!out || !params || !cu || !grids) return ARACHNE_ERR_NULL_POINTER;
   if (num_shards < 1 || num_shards > kMaxShards || (num_shards > 1 && !shard_starts)) return ARACHNE_ERR_BAD_SHARDING;
   if (head_offset < 0 || params->num_heads <= 0 || static_cast<long long>(head_offset) + params->num_heads > total_heads)
@@ -277,12 +302,19 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
     s.tile_base = tile_base; s.n_tiles = (s.len + kTileRows - 1) / kTileRows;
     s.T = grids[3 * b]; s.Hg = grids[3 * b + 1]; s.Wg = grids[3 * b + 2];
     s.n_video = s.T * s.Hg * s.Wg;
+    s.qt_lo = 0; s.qt_n = s.n_tiles;
+    if (cp_rank >= 0) {      // context parallelism: only the query tiles that hold tokens of [starts[rank], starts[rank+1])
+      const int lo = std::max(shard_starts ? shard_starts[cp_rank] : 0, s.tok_start);
+      const int hi = std::min(shard_starts ? shard_starts[cp_rank + 1] : p.total_tokens, s.tok_start + s.len);
+      s.qt_lo = lo < hi ? (lo - s.tok_start) / kTileRows : 0;
+      s.qt_n = lo < hi ? (hi - 1 - s.tok_start) / kTileRows + 1 - s.qt_lo : 0;
+    }
     tile_base += s.n_tiles;
     for (int a = 0; a < 3; ++a) ext[a] = std::max(ext[a], grids[3 * b + a]);
     pl->seqs.push_back(s);
   }
   pl->n_tiles_total = tile_base;
-  pl->n_items = tile_base * p.num_heads;
+  pl->cp_rank = cp_rank;
   std::vector<int> tile_seq(pl->n_tiles_total);
   for (int b = 0; b < p.num_seqs; ++b)
     for (int t = 0; t < pl->seqs[b].n_tiles; ++t) tile_seq[pl->seqs[b].tile_base + t] = b;
@@ -293,21 +325,22 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   for (int b = 0; b < p.num_seqs; ++b) order[b] = b;
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return pl->seqs[a].n_tiles > pl->seqs[b].n_tiles; });
   std::vector<WorkItem> items;
-  items.reserve(pl->n_items);
   for (int b : order)
     for (int h = 0; h < p.num_heads; ++h)
-      for (int t = 0; t < pl->seqs[b].n_tiles; ++t) items.push_back(WorkItem{b, h, t, 0});
+      for (int t = 0; t < pl->seqs[b].n_tiles && pl->seqs[b].qt_n > 0; ++t) items.push_back(WorkItem{b, h, t, 0});
   // forward items: pairs of adjacent query tiles (two tiles ping-pong on the tensor pipe), same group order
   std::vector<WorkItem> fwd_items;
   for (int b : order)
     for (int h = 0; h < p.num_heads; ++h)
-      for (int t = 0; t < pl->seqs[b].n_tiles; t += 2)
-        fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].n_tiles - t)});
+      for (int t = pl->seqs[b].qt_lo; t < pl->seqs[b].qt_lo + pl->seqs[b].qt_n; t += 2)
+        fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].qt_lo + pl->seqs[b].qt_n - t)});
+  pl->n_items = static_cast<int>(items.size());
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
   // Static LPT assignment to the persistent CTAs: the lists are in decreasing-cost order, each item goes to the
   // least-loaded CTA (ties: lowest index — while costs are equal this is round-robin, so CTAs running side by side
   // stay on adjacent tiles of the same (sequence, head) group), and every CTA's items are stored contiguously.
   auto deal = [&](std::vector<WorkItem>& list, int n_cta, auto cost, std::vector<int>& ptr) {
+    if (n_cta == 0) { ptr.assign(1, 0); return; }
     std::vector<long long> load(n_cta, 0);
     std::vector<std::vector<WorkItem>> own(n_cta);
     for (const WorkItem& w : list) {
@@ -326,8 +359,10 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   std::vector<int> item_ptr, fwd_item_ptr;
   pl->n_ctas = std::min(pl->num_sms, pl->n_items);
   pl->n_fwd_ctas = std::min(pl->num_sms, pl->n_fwd_items);
-  deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].n_tiles); }, item_ptr);
+  deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].qt_n); }, item_ptr);
   deal(fwd_items, pl->n_fwd_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].n_tiles) * w.pad; }, fwd_item_ptr);
+  if (items.empty()) items.push_back(WorkItem{0, 0, 0, 0});          // (a CP rank that owns no queries: nothing is launched)
+  if (fwd_items.empty()) fwd_items.push_back(WorkItem{0, 0, 0, 0});
   // RoPE tables in fp64 -> fp32 (readings R4, R5)
   std::vector<float2> tab;
   RopeDesc rd{};
@@ -391,6 +426,8 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   pl->sh.H_total = total_heads;
   pl->sh.head_offset = head_offset;
   pd.sh = pl->sh;
+  pd.cp_lo = cp_rank >= 0 ? pl->sh.start[cp_rank] : 0;
+  pd.cp_hi = cp_rank >= 0 ? pl->sh.start[cp_rank + 1] : p.total_tokens;
   pl->tile_bytes = static_cast<size_t>(kTileRows) * p.head_dim * 2;
   pl->img_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * pl->tile_bytes, 1024);
   pl->rowvec_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * sizeof(float), 1024);
@@ -406,6 +443,7 @@ int arachne_plan_create_sharded(arachne_plan** out, const arachne_attn_params* p
   *out = pl;
   return ARACHNE_OK;
 }
+extern "C" {
 
 void arachne_plan_destroy(arachne_plan* pl) {
   if (!pl) return;
@@ -540,6 +578,7 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* pl, const void* const* q
                                     const void* const* d_o, void* const* dq, void* const* dk, void* const* dv,
                                     float* dgamma_q, float* dgamma_k, void* ws, size_t ws_bytes, void* stream) {
   if (!pl || !q || !k || !v || !o || !lse || !d_o || !dq || !dk || !dv || !ws) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->cp_rank >= 0) return ARACHNE_ERR_BAD_SHARDING;      // a context-parallel plan needs bwd_cp_partial + cp_reduce
   ShardedPtr sq, sk, sv, so, sg, sdq, sdk, sdv;
   int rc;
   if ((rc = gather_shards(pl, q, sq)) || (rc = gather_shards(pl, k, sk)) || (rc = gather_shards(pl, v, sv)) ||
@@ -554,6 +593,82 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* pl, const void* const* q
   return pl->p.head_dim == 128
              ? launch_bwd<128>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, sdk, sdv, dgamma_q, dgamma_k, ws, st)
              : launch_bwd<64>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, sdk, sdv, dgamma_q, dgamma_k, ws, st);
+}
+
+int arachne_varlen_attn_bwd_cp_partial(const arachne_plan* pl, const void* const* q, const void* const* k,
+                                       const void* const* v, const float* gamma_q, const float* gamma_k,
+                                       const void* const* o, const float* lse, const void* const* d_o, void* const* dq,
+                                       float* dk_partial, float* dv_partial, float* dgamma_q, void* ws, size_t ws_bytes,
+                                       void* stream) {
+  if (!pl || !q || !k || !v || !o || !lse || !d_o || !dq || !dk_partial || !dv_partial || !ws) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->cp_rank < 0) return ARACHNE_ERR_BAD_SHARDING;
+  ShardedPtr sq, sk, sv, so, sg, sdq, none{};
+  int rc;
+  if ((rc = gather_shards(pl, q, sq)) || (rc = gather_shards(pl, k, sk)) || (rc = gather_shards(pl, v, sv)) ||
+      (rc = gather_shards(pl, o, so)) || (rc = gather_shards(pl, d_o, sg)) || (rc = gather_shards(pl, dq, sdq)))
+    return rc;
+  if (misaligned(lse) || misaligned(ws) || misaligned(dk_partial) || misaligned(dv_partial) ||
+      (gamma_q && misaligned(gamma_q)) || (gamma_k && misaligned(gamma_k)) || (dgamma_q && misaligned(dgamma_q)) ||
+      row_pitch_misaligned(pl))
+    return ARACHNE_ERR_MISALIGNED;
+  if (ws_bytes < bwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  return pl->p.head_dim == 128
+             ? launch_bwd<128>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, none, none, dgamma_q, nullptr, ws, st, dk_partial, dv_partial)
+             : launch_bwd<64>(pl, sq, sk, sv, gamma_q, gamma_k, so, lse, sg, sdq, none, none, dgamma_q, nullptr, ws, st, dk_partial, dv_partial);
+}
+
+}  // extern "C"
+namespace {
+template <int D>
+int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const ShardedPtr& gvp, const ShardedPtr& k, const float* gk,
+                     const ShardedPtr& dk, const ShardedPtr& dv, float* dgk, void* ws, cudaStream_t st) {
+  uint8_t* w = static_cast<uint8_t*>(ws);
+  w += 4 * pl->img_bytes + 2 * pl->rowvec_bytes;                 // same carving as launch_bwd: gk_t, gq_t, dgamma partials
+  float* gk_sum = reinterpret_cast<float*>(w); w += pl->grad_bytes + pl->gradblk_bytes;
+  float* dgpart = dgk ? reinterpret_cast<float*>(w) : nullptr;
+  const int lo = pl->pd.cp_lo, hi = pl->pd.cp_hi;
+  if (hi > lo) {
+    CpReduceParams cp{gkp, gvp, gk_sum, dv, lo, hi};
+    const long long n_vec = static_cast<long long>(hi - lo) * pl->p.num_heads * (D / 4);
+    const int grid = static_cast<int>(std::min<long long>((n_vec + 255) / 256, static_cast<long long>(pl->num_sms) * 8));
+    cp_reduce_kernel<D><<<grid, 256, 0, st>>>(pl->pd, cp);
+    ARACHNE_CUDA(cudaGetLastError());
+  }
+  ShardedPtr none{};
+  PostParams po{nullptr, 0, gk_sum, none, k, nullptr, gk, none, dk, 2, lo, hi, dgpart};
+  post_kernel<D><<<dim3(pl->post_blocks, 1), 256, 0, st>>>(pl->pd, po);
+  ARACHNE_CUDA(cudaGetLastError());
+  if (dgpart) {
+    dgamma_reduce_kernel<D><<<2, 256, 0, st>>>(dgpart, pl->post_blocks, nullptr, dgk);
+    ARACHNE_CUDA(cudaGetLastError());
+  }
+  return ARACHNE_OK;
+}
+}  // namespace
+extern "C" {
+
+int arachne_cp_reduce(const arachne_plan* pl, const float* const* dk_partials, const float* const* dv_partials,
+                      const void* const* k, const float* gamma_k, void* const* dk, void* const* dv, float* dgamma_k,
+                      void* ws, size_t ws_bytes, void* stream) {
+  if (!pl || !dk_partials || !dv_partials || !k || !dk || !dv || !ws) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->cp_rank < 0) return ARACHNE_ERR_BAD_SHARDING;
+  ShardedPtr gkp{}, gvp{}, sk, sdk, sdv;
+  for (int r = 0; r < pl->sh.n_shards; ++r) {       // a partial buffer may be NULL only for a rank that owns no queries
+    const bool empty = pl->sh.start[r + 1] == pl->sh.start[r];
+    if ((!dk_partials[r] || !dv_partials[r]) && !empty) return ARACHNE_ERR_NULL_POINTER;
+    if (misaligned(dk_partials[r]) || misaligned(dv_partials[r])) return ARACHNE_ERR_MISALIGNED;
+    gkp.p[r] = const_cast<float*>(dk_partials[r]);
+    gvp.p[r] = const_cast<float*>(dv_partials[r]);
+  }
+  int rc;
+  if ((rc = gather_shards(pl, k, sk)) || (rc = gather_shards(pl, dk, sdk)) || (rc = gather_shards(pl, dv, sdv))) return rc;
+  if (misaligned(ws) || (gamma_k && misaligned(gamma_k)) || (dgamma_k && misaligned(dgamma_k)) || row_pitch_misaligned(pl))
+    return ARACHNE_ERR_MISALIGNED;
+  if (ws_bytes < bwd_ws_bytes(pl)) return ARACHNE_ERR_WORKSPACE_TOO_SMALL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  return pl->p.head_dim == 128 ? launch_cp_reduce<128>(pl, gkp, gvp, sk, gamma_k, sdk, sdv, dgamma_k, ws, st)
+                               : launch_cp_reduce<64>(pl, gkp, gvp, sk, gamma_k, sdk, sdv, dgamma_k, ws, st);
 }
 
 // ---------------------------------------------------------------- host-buffer convenience calls

@@ -40,6 +40,7 @@ struct BwdFusedParams {
                            //         XOR-swizzled with (row & 7); zeroed by prep_kernel
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
   ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
+  float* gv_t;             // nullable (context parallelism): dV PARTIAL fp32 [N,H,D] written instead of dv
   int q_rot;               // rotate the query-tile order per key tile (spreads the L2 reductions)
 };
 
@@ -154,8 +155,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
         bulk_g2s(sK, bp.kt + xoff, TILE, kv_full);
         bulk_g2s(sV, bp.vt + xoff, TILE, kv_full);
       }
-      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
-        const int qt = q_tile_of(wi, i, sq.n_tiles);
+      for (int i = 0; i < sq.qt_n; ++i, ++g) {
+        const int qt = sq.qt_lo + q_tile_of(wi, i, sq.qt_n);
         const size_t yoff = hoff + static_cast<size_t>(sq.tile_base + qt) * TILE;
         const size_t roff = (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * kTileRows;
         const uint32_t qs = g % QS, qph = (g / QS) & 1, ds = g % DS, dph = (g / DS) & 1;
@@ -253,7 +254,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     };
     for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
-      const uint32_t n = pd.seqs[wi.seq].n_tiles;
+      const uint32_t n = pd.seqs[wi.seq].qt_n;        // query tiles this process visits (all, unless context-parallel)
       mbar_wait(kv_full, it & 1);
       issue_S(g0);
       issue_P(g0);
@@ -284,7 +285,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
+      for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const uint32_t qs = g % QS, qph = (g / QS) & 1;
         const float* lse_s = sLse + qs * 128 + wg * 64;
         const float* dl_s = sDelta + qs * 128 + wg * 64;
@@ -348,15 +349,17 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       const bool valid_row = n < sq.len;
       const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
       const uint32_t tA = tbase + (wg == 0 ? Cfg::kColDV : Cfg::kColDK) + lane_base;
-      const float sc = pd.softmax_scale;
-      __nv_bfloat16* dv_row = (valid_row && wg == 0) ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
+      const bool dv_bf16 = wg == 0 && bp.gv_t == nullptr;      // CP: dV leaves as an fp32 partial like dK~
+      const float sc = wg == 0 ? 1.0f : pd.softmax_scale;
+      float* f32_out = wg == 0 ? bp.gv_t : bp.gk_t;
+      __nv_bfloat16* dv_row = (valid_row && dv_bf16) ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
         uint32_t a[32];
         tmem_ld32(tA + c * 32, a);
         tmem_wait_ld();
         if (valid_row) {
-          if (wg == 0) {
+          if (dv_bf16) {
 #pragma unroll
             for (int i2 = 0; i2 < 32; i2 += 8) {
               uint4 w;
@@ -372,7 +375,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
               float4 f;
               f.x = __uint_as_float(a[i2]) * sc; f.y = __uint_as_float(a[i2 + 1]) * sc;
               f.z = __uint_as_float(a[i2 + 2]) * sc; f.w = __uint_as_float(a[i2 + 3]) * sc;
-              *reinterpret_cast<float4*>(bp.gk_t + out_off + c * 32 + i2) = f;
+              *reinterpret_cast<float4*>(f32_out + out_off + c * 32 + i2) = f;
             }
           }
         }
@@ -415,8 +418,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item) {
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      for (int i = 0; i < sq.n_tiles; ++i, ++g) {
-        const int qt = q_tile_of(wi, i, sq.n_tiles);
+      for (int i = 0; i < sq.qt_n; ++i, ++g) {
+        const int qt = sq.qt_lo + q_tile_of(wi, i, sq.qt_n);
         float* gtile = bp.gq_blk + (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * (kTileRows * D);
         mbar_wait(dq_full, g & 1);
         tc_fence_after();

@@ -15,6 +15,8 @@ struct SeqInfo {
   int tile_base;   // index of the sequence's first 128-token tile in the tiled workspace
   int n_tiles;     // ceil(L_b / 128)
   int T, Hg, Wg;   // latent grid; token n -> (n / (Hg*Wg), (n / Wg) % Hg, n % Wg)   (reading R7)
+  int qt_lo, qt_n; // query tiles [qt_lo, qt_lo + qt_n) of this sequence are computed by this process: all of them
+                   // (0, n_tiles) unless the plan is a context-parallel one (arachne_plan_create_cp)
   int n_video;     // T*Hg*Wg: tokens [0, n_video) are video tokens (rotated); [n_video, len) are text tokens,
                    // normed but NOT rotated (reading R21)
 };
@@ -111,6 +113,7 @@ struct ProblemDesc {
   int no_norm, no_rope;
   RopeDesc rope;
   Sharding sh;
+  int cp_lo, cp_hi;          // context parallelism: this process owns the QUERY tokens [cp_lo, cp_hi) (0, N otherwise)
 };
 
 }  // namespace arachne

@@ -307,7 +307,8 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
       mbar_wait(&pv_done[t], (g - 1) & 1);
       tc_fence_after();
       const int n = (wi.tile + t) * kTileRows + row;     // token inside the sequence
-      const bool valid_row = n < sq.len;
+      const int tok_g = sq.tok_start + n;
+      const bool valid_row = n < sq.len && tok_g >= pd.cp_lo && tok_g < pd.cp_hi;   // CP: only this rank's query rows
       const float inv_l = 1.0f / l;
       __nv_bfloat16* orow = valid_row ? raw_row<__nv_bfloat16>(pd.sh, fp.o, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll

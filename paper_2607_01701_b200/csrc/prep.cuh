@@ -168,9 +168,11 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
       for (int i = 0; i < 8; ++i) dsum += g[i] * oo[i];
       dsum = seg_sum<LPR>(dsum);                                // D_i = sum_d dO*O   (§8 a5)
       if (d0 == 0) {
-        pp.delta_t[row_off + r] = valid ? dsum : 0.f;
+        // context parallelism: query rows of other ranks behave like pad rows here (P = 0: no dK/dV contribution)
+        const bool live = valid && tok >= pd.cp_lo && tok < pd.cp_hi;
+        pp.delta_t[row_off + r] = live ? dsum : 0.f;
         // pad rows get +inf so that P = exp2(s - inf) = 0 for them in the backward kernels
-        pp.lse2_t[row_off + r] = valid ? pp.lse[static_cast<size_t>(h) * pd.N + tok] * 1.4426950408889634f
+        pp.lse2_t[row_off + r] = live ? pp.lse[static_cast<size_t>(h) * pd.N + tok] * 1.4426950408889634f
                                        : __int_as_float(0x7f800000);
       }
     }
@@ -220,6 +222,8 @@ struct PostParams {
   const float* gamma_q;
   const float* gamma_k;
   ShardedPtr dq, dk;            // out bf16, same sharding
+  int which;                    // 0: y = 0 -> dQ, y = 1 -> dK;  1: dQ only (grid.y = 1);  2: dK only (grid.y = 1)
+  int tok_lo, tok_hi;           // only (token, head) rows with tok in [tok_lo, tok_hi) are processed (CP; else 0, N)
   float* dgamma_part;           // nullable: [2][gridDim.x][D] per-block partial sums of dl/dgamma_q, dl/dgamma_k (R22)
 };
 
@@ -235,7 +239,7 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
   __shared__ float s_part[8 * RPW][D];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int sub = lane / LPR, d0 = (lane % LPR) * 8;
-  const bool is_k = blockIdx.y == 1;
+  const bool is_k = pp.which == 2 || blockIdx.y == 1;
   const float* gt = is_k ? pp.gk_t : pp.gq_t;
   const ShardedPtr& xraw_s = is_k ? pp.k : pp.q;
   const float* gamma = is_k ? pp.gamma_k : pp.gamma_q;
@@ -244,10 +248,10 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
   float gam[8], dgam[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) { gam[i] = gamma ? __ldg(&gamma[d0 + i]) : 1.0f; dgam[i] = 0.f; }
-  const int n_rows = pd.N * pd.H;                              // < 2^31 (checked by the plan)
+  const int n_rows = pp.tok_hi * pd.H;                         // < 2^31 (checked by the plan)
   const int stride = gridDim.x * 8 * RPW;
 #pragma unroll 2
-  for (int row0 = (blockIdx.x * 8 + warp) * RPW; row0 < n_rows; row0 += stride) {   // warp-uniform trip count
+  for (int row0 = pp.tok_lo * pd.H + (blockIdx.x * 8 + warp) * RPW; row0 < n_rows; row0 += stride) {   // warp-uniform trip count
     const bool live = row0 + sub < n_rows;                     // ragged end: the lane keeps shuffling, stores nothing
     const int row = live ? row0 + sub : n_rows - 1;            // (token, head)
     const int tok = row / pd.H, h = row - tok * pd.H;
@@ -313,7 +317,7 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
       float a = 0.f;
 #pragma unroll
       for (int w = 0; w < 8 * RPW; ++w) a += s_part[w][threadIdx.x];
-      pp.dgamma_part[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * D + threadIdx.x] = a;
+      pp.dgamma_part[(static_cast<size_t>(is_k ? 1 : 0) * gridDim.x + blockIdx.x) * D + threadIdx.x] = a;
     }
   }
 }
@@ -336,6 +340,47 @@ __global__ void __launch_bounds__(256) dgamma_reduce_kernel(const float* part, i
 #pragma unroll
     for (int i = 0; i < S; ++i) t += s[i][d];
     out[d] = t;
+  }
+}
+
+
+// Context parallelism, phase 2 ("CP ... sequence partition"): every rank has written
+// PARTIAL dk~ and dV (fp32 [N,H,D], from its own query rows) for all keys of the sequences it touches.  The owner of a
+// key token adds the partials of the contributing ranks IN RANK ORDER (fixed order: bit-reproducible) — reading them
+// straight out of the peers' buffers (the reduce-scatter is these loads) — and emits dV (bf16) and the summed dk~ for
+// post_kernel.  Rank r contributes to a token iff its query range intersects the token's sequence.
+struct CpReduceParams {
+  ShardedPtr gk_part, gv_part;   // [n_shards] fp32 [N,H,D] partial buffers, one per rank (local or peer memory)
+  float* gk_sum;                 // out: fp32 [N,H,D], rows [tok_lo, tok_hi) only
+  ShardedPtr dv;                 // out: bf16, token-range sharded like every raw tensor
+  int tok_lo, tok_hi;
+};
+
+template <int D>
+__global__ void __launch_bounds__(256) cp_reduce_kernel(ProblemDesc pd, CpReduceParams cp) {
+  constexpr int VPR = D / 4;                                       // float4 pieces per (token, head) row
+  const long long n_vec = static_cast<long long>(cp.tok_hi - cp.tok_lo) * pd.H * VPR;
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n_vec;
+       i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const int piece = static_cast<int>(i % VPR);
+    const long long rh = i / VPR;
+    const int tok = cp.tok_lo + static_cast<int>(rh / pd.H), h = static_cast<int>(rh % pd.H);
+    const SeqInfo sq = pd.seqs[pd.tok_info[tok].seq];
+    const size_t off = (static_cast<size_t>(tok) * pd.H + h) * D + piece * 4;
+    float4 sk = make_float4(0.f, 0.f, 0.f, 0.f), sv = sk;
+#pragma unroll
+    for (int r = 0; r < kMaxShards; ++r) {
+      if (r < pd.sh.n_shards && pd.sh.start[r + 1] > pd.sh.start[r] && pd.sh.start[r] < sq.tok_start + sq.len &&
+          pd.sh.start[r + 1] > sq.tok_start) {
+        const float4 a = *reinterpret_cast<const float4*>(shard_base<const float>(cp.gk_part, r) + off);
+        const float4 b = *reinterpret_cast<const float4*>(shard_base<const float>(cp.gv_part, r) + off);
+        sk.x += a.x; sk.y += a.y; sk.z += a.z; sk.w += a.w;
+        sv.x += b.x; sv.y += b.y; sv.z += b.z; sv.w += b.w;
+      }
+    }
+    *reinterpret_cast<float4*>(cp.gk_sum + off) = sk;
+    uint2 u; u.x = pack_bf16x2(sv.x, sv.y); u.y = pack_bf16x2(sv.z, sv.w);
+    *reinterpret_cast<uint2*>(raw_row<__nv_bfloat16>(pd.sh, cp.dv, tok, h, D) + piece * 4) = u;
   }
 }
 

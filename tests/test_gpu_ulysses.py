@@ -110,3 +110,81 @@ def test_sharded_validation():
     with pytest.raises(binding.ArachneError) as e:       # a sharded plan through the plain entry point
         binding.arachne_varlen_attn_fwd(plan, x, x, x, x, lse, ws)
     assert e.value.status == 13
+
+
+# ------------------------------------------------------------------ context parallelism (arachne_plan_create_cp)
+def _run_cp(st, t, starts, gamma=None):
+    """k virtual ranks on one GPU: rank r owns the QUERY tokens of shard r (all heads) and reads K, V of every shard."""
+    from paper_2607_01701_b200 import binding
+    N, H, D = st["N"], st["H"], st["D"]
+    k = len(starts) - 1
+    sh = {n: _split(t[n], starts) for n in ("q", "k", "v", "dO")}
+    out = {n: [torch.full_like(x, 7.0) for x in sh["q"]] for n in ("o", "dq", "dk", "dv")}
+    gq, gk = (None, None) if gamma is None else (torch.as_tensor(g, dtype=torch.float32, device="cuda") for g in gamma)
+    plans = [binding.Plan(st["cu_seqlens"], st["grids"], H, D, st["rope_dims"], text_lens=st.get("text_lens"),
+                          shard_starts=starts, cp_rank=r) for r in range(k)]
+    lses, parts_k, parts_v = [], [], []
+    dgq_sum = torch.zeros(D, device="cuda", dtype=torch.float64); dgk_sum = torch.zeros_like(dgq_sum)
+    for r in range(k):
+        ws = torch.empty(plans[r].workspace_bytes(False), dtype=torch.uint8, device="cuda")
+        lse = torch.full((H, N), float("nan"), dtype=torch.float32, device="cuda")
+        binding.arachne_varlen_attn_fwd_sharded(plans[r], sh["q"], sh["k"], sh["v"], out["o"], lse, ws, gq, gk)
+        lses.append(lse)
+    for r in range(k):            # step 1 on every rank (partials poisoned first: unwritten rows must never be read)
+        ws = torch.empty(plans[r].workspace_bytes(True), dtype=torch.uint8, device="cuda")
+        pk = torch.full((N, H, D), float("nan"), dtype=torch.float32, device="cuda"); pv = torch.full_like(pk, float("nan"))
+        dgq = torch.empty(D, device="cuda")
+        binding.arachne_varlen_attn_bwd_cp_partial(plans[r], sh["q"], sh["k"], sh["v"], out["o"], lses[r], sh["dO"], out["dq"],
+                                                   pk, pv, ws, dgq, gq, gk)
+        parts_k.append(pk); parts_v.append(pv); dgq_sum += dgq.double()
+    for r in range(k):            # (barrier) step 2 on every rank
+        ws = torch.empty(plans[r].workspace_bytes(True), dtype=torch.uint8, device="cuda")
+        dgk = torch.empty(D, device="cuda")
+        binding.arachne_cp_reduce(plans[r], parts_k, parts_v, sh["k"], out["dk"], out["dv"], ws, dgk, gk)
+        dgk_sum += dgk.double()
+    torch.cuda.synchronize()
+    lse = torch.empty((H, N), dtype=torch.float32, device="cuda")
+    for r in range(k):
+        lse[:, starts[r]:starts[r + 1]] = lses[r][:, starts[r]:starts[r + 1]]
+    return {"O": torch.cat(out["o"]), "LSE": lse, "dQ": torch.cat(out["dq"]), "dK": torch.cat(out["dk"]),
+            "dV": torch.cat(out["dv"]), "dGq": dgq_sum, "dGk": dgk_sum}
+
+
+@pytest.mark.parametrize("grids,text,H,D,starts", [
+    ([(2, 9, 11), (1, 8, 8), (3, 10, 13)], None, 3, 128, [0, 100, 300, 652]),        # cuts inside tiles and sequences
+    ([(1, 16, 16), (1, 5, 7)], [40, 3], 2, 64, [0, 128, 334]),                       # cut on a tile edge; joint; D = 64
+    ([(4, 16, 16), (1, 2, 3)], None, 2, 128, [0, 0, 513, 1030, 1030]),               # empty shards; a rank owning 517 rows
+])
+def test_context_parallel_equals_oracle(orc, grids, text, H, D, starts):
+    st = inputs.pack(grids, H, D, index=6, text_lens=text)
+    assert starts[-1] == st["N"]
+    t = inputs.make_inputs(st, device="cuda")
+    rng = np.random.default_rng(4)
+    gam = ((0.5 + rng.random(D)).astype(np.float32), (0.5 + rng.random(D)).astype(np.float32))
+    got = _run_cp(st, t, starts, gamma=gam)
+    a = {n: v.float().cpu().numpy().astype(np.float64) for n, v in t.items()}
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], gamma_q=gam[0], gamma_k=gam[1],
+                        rope_dims=st["rope_dims"], text_lens=st["text_lens"])
+    w = pu.check_full(st, got, ref)
+    w.update(pu.check_dgamma(got, ref))
+    print(grids, starts, w)
+    # forward rows are computed exactly as in the plain call: bit-identical O and LSE
+    plain = pu.run_gpu(st, t, gamma_q=gam[0], gamma_k=gam[1], with_bwd=False)
+    assert torch.equal(got["O"], plain["O"]) and torch.equal(got["LSE"], plain["LSE"])
+
+
+def test_context_parallel_validation():
+    from paper_2607_01701_b200 import binding
+    kw = dict(cu_seqlens=[0, 64], grids=[(1, 8, 8)], num_heads=2, head_dim=64, rope_dims=(16, 24, 24))
+    with pytest.raises(binding.ArachneError) as e:
+        binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=2)
+    assert e.value.status == 13
+    with pytest.raises(binding.ArachneError) as e:
+        binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=0, flags=binding.FLAG_DETERMINISTIC)
+    assert e.value.status == 12
+    plan = binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=1)
+    x = [torch.zeros(32, 2, 64, dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    lse = torch.empty(2, 64, device="cuda"); ws = torch.empty(plan.workspace_bytes(True), dtype=torch.uint8, device="cuda")
+    with pytest.raises(binding.ArachneError) as e:       # a CP plan through the Ulysses backward
+        binding.arachne_varlen_attn_bwd_sharded(plan, x, x, x, x, lse, x, x, x, x, ws)
+    assert e.value.status == 13

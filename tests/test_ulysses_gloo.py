@@ -107,3 +107,29 @@ def test_two_rank_gloo_ulysses_rules_equal_all_to_all(tmp_path):
     port = _free_port()
     mp.spawn(_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
     assert (tmp_path / "ok0").read_text() == "ok" and (tmp_path / "ok1").read_text() == "ok"
+
+
+def test_context_parallel_bookkeeping():
+    from paper_2607_01701_b200 import context_parallel as cp
+    cu = [0, 198, 262, 652, 653, 1700]
+    N = cu[-1]
+    for starts in ([0, 100, 300, 652, N], [0, 0, 513, 1030, N], [0, N], cp.balanced_starts(cu, 3), cp.balanced_starts(cu, 8)):
+        assert starts[0] == 0 and starts[-1] == N and all(b >= a for a, b in zip(starts, starts[1:]))
+        for b in range(len(cu) - 1):
+            s, L = cu[b], cu[b + 1] - cu[b]
+            covered = np.zeros((L + 127) // 128, dtype=int)
+            for r in range(len(starts) - 1):
+                first, n = cp.query_tile_range(s, L, starts[r], starts[r + 1])
+                rows = [t for t in range(s, s + L) if starts[r] <= t < starts[r + 1]]              # brute force
+                tiles = sorted({(t - s) // 128 for t in rows})
+                assert tiles == list(range(first, first + n))
+                covered[first:first + n] += 1
+                assert (r in cp.contributors(starts, s, L)) == bool(rows)
+            assert np.all(covered >= 1)                      # every query tile has an owner (boundary tiles: two)
+        costs = [cp.rank_cost(cu, starts[r], starts[r + 1]) for r in range(len(starts) - 1)]
+        assert sum(costs) == sum((cu[i + 1] - cu[i]) ** 2 for i in range(len(cu) - 1))
+    # cost-balanced cuts: no rank more than one row-of-the-longest-sequence above the mean
+    for k in (2, 3, 8):
+        st = cp.balanced_starts(cu, k)
+        costs = [cp.rank_cost(cu, st[r], st[r + 1]) for r in range(k)]
+        assert max(costs) <= sum(costs) / k + max(cu[i + 1] - cu[i] for i in range(len(cu) - 1))
