@@ -183,3 +183,27 @@ def sample_rows(st, per_seq: int = 64, seed: int = 0):
             s.add(r % L)
         rows.extend(cu[b] + x for x in sorted(s))
     return rows
+
+
+# ------------------------------------------------------------------ synthetic cascade-scheduling instances (NEXT-4)
+def cascade_instance(seed: int, n_samples: int = 8, degrees=(1, 2, 4, 8), n_gpus: int = 16):
+    """A seeded scheduling instance shaped like one Arachne training batch: per sample a VAE
+    cascade followed by a DiT cascade (edge VAE -> DiT), sample lengths from the heavy-tailed recipe (R18).  The
+    latency / feasibility TABLES are synthetic numbers with the shape of Eq. 8-9 (work/k + a per-degree overhead; small
+    degrees infeasible for long samples) — no cost model of the method is evaluated here.  Returns plain lists."""
+    grids = heavytail_structure(BASE_SEED + 977 * seed, max_tokens=1 << 30)[:n_samples]
+    state = (seed * 0x9E3779B97F4A7C15 + 12345) & _M64
+    K = [int(k) for k in degrees]
+    L, feas, preds = [], [], []
+    for i, (t, hg, wg) in enumerate(grids):
+        S = t * hg * wg
+        state, r1 = _splitmix64(state)
+        state, r2 = _splitmix64(state)
+        jit1, jit2 = 0.9 + 0.2 * ((r1 >> 11) / float(1 << 53)), 0.9 + 0.2 * ((r2 >> 11) / float(1 << 53))
+        vae = [jit1 * (2.0e-4 * S) / k + 0.02 * (k - 1) for k in K]                       # VAE: linear in tokens
+        dit = [jit2 * (3.0e-4 * S + 2.5e-9 * S * S) * 60 / 1000 / k + 0.05 * math.log2(k) for k in K]   # DiT: Eq. 9 shape
+        L.append(vae); feas.append([True] * len(K)); preds.append([])
+        L.append(dit); feas.append([S / k <= 70000 for k in K]); preds.append([2 * i])    # activation memory ~ tokens / k
+        if not any(feas[-1]):
+            feas[-1][-1] = True
+    return dict(K=K, L=L, feasible=feas, preds=preds, N=n_gpus)
