@@ -30,5 +30,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+SCHED_LIB = os.path.join(CSRC, "libarachne_sched.so")
+SCHED_SRC = [os.path.join(CSRC, "cascade_sched.cpp"), os.path.join(HERE, "..", "include", "arachne_sched.h")]
+
+
+def build_sched(force: bool = False) -> str:
+    """libarachne_sched.so: the host-only cascade scheduler (include/arachne_sched.h).  -ffp-contract=off: the makespans
+    are compared value for value with the Python oracle."""
+    if force or not os.path.exists(SCHED_LIB) or any(os.path.getmtime(f) > os.path.getmtime(SCHED_LIB) for f in SCHED_SRC):
+        subprocess.run(["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", SCHED_LIB,
+                        SCHED_SRC[0]], check=True)
+    return SCHED_LIB
+
+
 if __name__ == "__main__":
+    build_sched(force="--force" in sys.argv)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
