@@ -12,6 +12,11 @@ for _p in (ROOT, HERE):
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a real B200 (run with -m gpu on the GPU box)")
+    # native libraries are git-ignored build artefacts: (re)build them if missing or stale before any test imports a binding
+    from paper_2607_01701_b200 import build
+
+    build.build()
+    build.build_sched()
 
 
 @pytest.fixture(scope="session")
