@@ -225,6 +225,17 @@ int arachne_cp_reduce(const arachne_plan* plan, const float* const* dk_partials,
                       const void* const* k, const float* gamma_k, void* const* dk, void* const* dv,
                       float* dgamma_k, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Peer-memory plumbing for the *_sharded / *_cp calls on one node: CUDA IPC.  arachne_ipc_alloc = cudaMalloc on the
+ * current device + cudaIpcGetMemHandle (handle_out: 64 bytes, HOST; send it to the other ranks by any means);
+ * arachne_ipc_open maps another PROCESS's allocation into this one (the returned device pointer reaches the owner's HBM
+ * over NVLink / NVSwitch when the owner is another GPU; the same GPU works too) — not callable on a handle of this
+ * process; arachne_ipc_close unmaps, arachne_ipc_free frees an arachne_ipc_alloc allocation (after every peer closed it).
+ * Status codes as everywhere (ARACHNE_ERR_CUDA + arachne_last_error_message on a CUDA failure). */
+int arachne_ipc_alloc(size_t bytes, void** dev_ptr, void* handle_out);
+int arachne_ipc_open(const void* handle, void** dev_ptr);
+int arachne_ipc_close(void* dev_ptr);
+int arachne_ipc_free(void* dev_ptr);
+
 /* End-to-end convenience calls with HOST tensors (same layouts, all *_host pointers are host
  * memory; pinned for the copies to overlap the kernels, pageable works but serialises): copy in,
  * run, copy the results back, and return after everything has completed.  Device buffers and two

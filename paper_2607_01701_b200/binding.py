@@ -28,6 +28,7 @@ EXPORTS = [
     "arachne_plan_create_joint", "arachne_varlen_attn_bwd_dgamma",
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
     "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
+    "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free",
 ]
 
 
@@ -87,6 +88,16 @@ _lib.arachne_plan_enable_profiling.argtypes = [_vp, ctypes.c_int]
 _lib.arachne_plan_kernel_times.restype = ctypes.c_int
 _lib.arachne_plan_kernel_times.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_float), ctypes.c_int,
                                            ctypes.POINTER(ctypes.c_int)]
+
+
+_lib.arachne_ipc_alloc.restype = ctypes.c_int
+_lib.arachne_ipc_alloc.argtypes = [ctypes.c_size_t, ctypes.POINTER(_vp), ctypes.c_char_p]
+_lib.arachne_ipc_open.restype = ctypes.c_int
+_lib.arachne_ipc_open.argtypes = [ctypes.c_char_p, ctypes.POINTER(_vp)]
+_lib.arachne_ipc_close.restype = ctypes.c_int
+_lib.arachne_ipc_close.argtypes = [_vp]
+_lib.arachne_ipc_free.restype = ctypes.c_int
+_lib.arachne_ipc_free.argtypes = [_vp]
 
 
 class ArachneError(RuntimeError):
@@ -291,3 +302,40 @@ def backward(plan: Plan, q, k, v, o, lse, d_o, gamma_q=None, gamma_k=None, works
     dgk = torch.empty(plan.D, dtype=torch.float32, device=q.device)
     arachne_varlen_attn_bwd_dgamma(plan, q, k, v, o, lse, d_o, dq, dk, dv, dgq, dgk, ws, gamma_q, gamma_k)
     return dq, dk, dv, dgq, dgk
+
+
+# ---- CUDA IPC plumbing (peer shards on one node)
+def ipc_alloc(nbytes: int):
+    """-> (device address, 64-byte handle).  cudaMalloc on the current device; free with ipc_free."""
+    ptr, handle = _vp(), ctypes.create_string_buffer(64)
+    _check(_lib.arachne_ipc_alloc(nbytes, ctypes.byref(ptr), handle))
+    return int(ptr.value), handle.raw
+
+
+def ipc_open(handle: bytes) -> int:
+    ptr = _vp()
+    _check(_lib.arachne_ipc_open(handle, ctypes.byref(ptr)))
+    return int(ptr.value)
+
+
+def ipc_close(addr: int):
+    _check(_lib.arachne_ipc_close(_vp(addr)))
+
+
+def ipc_free(addr: int):
+    _check(_lib.arachne_ipc_free(_vp(addr)))
+
+
+class _RawCuda:
+    """__cuda_array_interface__ view of raw device memory, so that torch can wrap it without a copy."""
+
+    def __init__(self, addr, shape, typestr):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (addr, False), "version": 3}
+
+
+def tensor_from_address(addr: int, shape, dtype):
+    """torch tensor over raw device memory (bf16 goes through an int16 view: the array interface has no bf16)."""
+    if dtype == torch.bfloat16:
+        return torch.as_tensor(_RawCuda(addr, shape, "<i2"), device="cuda").view(torch.bfloat16)
+    typestr = {torch.float32: "<f4", torch.uint8: "|u1"}[dtype]
+    return torch.as_tensor(_RawCuda(addr, shape, typestr), device="cuda")

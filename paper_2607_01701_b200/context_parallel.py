@@ -67,13 +67,12 @@ class ContextParallelAttention:
     forward(): barrier -> fwd_sharded -> (no barrier needed: a rank writes only its own O shard).
     backward(): barrier -> bwd_cp_partial -> barrier -> cp_reduce -> all-reduce of the dgamma parts."""
 
-    def __init__(self, st: dict, group=None, starts=None):
+    def __init__(self, st: dict, group=None, starts=None, transport: str = "symm"):
         import torch
         import torch.distributed as dist
-        import torch.distributed._symmetric_memory as symm_mem
 
         from . import binding
-        from .ulysses import SymmetricShards
+        from .ulysses import IpcShards, SymmetricShards
 
         self.group, self._dist, self._binding = group, dist, binding
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
@@ -83,11 +82,17 @@ class ContextParallelAttention:
         dev = torch.device("cuda", torch.cuda.current_device())
         self.plan = binding.Plan(st["cu_seqlens"], st["grids"], st["H"], st["D"], st["rope_dims"],
                                  text_lens=st.get("text_lens"), shard_starts=self.starts, cp_rank=self.rank)
-        self.buf = {n: SymmetricShards(n_max, st["H"], st["D"], group, dev) for n in ("q", "k", "v", "o", "dO", "dq", "dk", "dv")}
+        Shards = SymmetricShards if transport == "symm" else IpcShards
+        self.buf = {n: Shards(n_max, st["H"], st["D"], group, dev) for n in ("q", "k", "v", "o", "dO", "dq", "dk", "dv")}
         self.part = {}
-        for n in ("dk_partial", "dv_partial"):
-            t = symm_mem.empty((st["N"], st["H"], st["D"]), dtype=torch.float32, device=dev)
-            self.part[n] = (t, [int(p) for p in symm_mem.rendezvous(t, group=group).buffer_ptrs])
+        for n in ("dk_partial", "dv_partial"):            # fp32 [N,H,D] partial buffers every rank can read
+            if transport == "symm":
+                import torch.distributed._symmetric_memory as symm_mem
+                t = symm_mem.empty((st["N"], st["H"], st["D"]), dtype=torch.float32, device=dev)
+                self.part[n] = (t, [int(p) for p in symm_mem.rendezvous(t, group=group).buffer_ptrs], None)
+            else:
+                sh = IpcShards(0, 0, 0, group, dev, dtype=torch.float32, shape=(st["N"], st["H"], st["D"]))
+                self.part[n] = (sh.local_full, sh.ptrs, sh)
         self.lse = torch.empty((st["H"], st["N"]), dtype=torch.float32, device=dev)
         self.ws = torch.empty(max(self.plan.workspace_bytes(False), self.plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
 
@@ -115,3 +120,9 @@ class ContextParallelAttention:
                                         b["dk"].ptrs, b["dv"].ptrs, self.ws, None, gamma_k)
         self._barrier()
         return b["dq"].local(self.n_local), b["dk"].local(self.n_local), b["dv"].local(self.n_local)
+
+    def close(self):
+        for b in list(self.buf.values()) + [p[2] for p in self.part.values() if p[2] is not None]:
+            if hasattr(b, "close"):
+                b.close()
+        self.plan.close()

@@ -671,6 +671,36 @@ int arachne_cp_reduce(const arachne_plan* pl, const float* const* dk_partials, c
                                : launch_cp_reduce<64>(pl, gkp, gvp, sk, gamma_k, sdk, sdv, dgamma_k, ws, st);
 }
 
+// ---------------------------------------------------------------- CUDA IPC plumbing for peer shards
+int arachne_ipc_alloc(size_t bytes, void** dev_ptr, void* handle_out) {
+  if (!dev_ptr || !handle_out) return ARACHNE_ERR_NULL_POINTER;
+  if (bytes == 0) return ARACHNE_ERR_BAD_SHAPE;
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+  ARACHNE_CUDA(cudaMalloc(dev_ptr, bytes));
+  cudaIpcMemHandle_t h;
+  cudaError_t e = cudaIpcGetMemHandle(&h, *dev_ptr);
+  if (e != cudaSuccess) { cudaFree(*dev_ptr); *dev_ptr = nullptr; return cuda_fail(e, "cudaIpcGetMemHandle"); }
+  std::memcpy(handle_out, &h, sizeof(h));
+  return ARACHNE_OK;
+}
+int arachne_ipc_open(const void* handle, void** dev_ptr) {
+  if (!handle || !dev_ptr) return ARACHNE_ERR_NULL_POINTER;
+  cudaIpcMemHandle_t h;
+  std::memcpy(&h, handle, sizeof(h));
+  ARACHNE_CUDA(cudaIpcOpenMemHandle(dev_ptr, h, cudaIpcMemLazyEnablePeerAccess));
+  return ARACHNE_OK;
+}
+int arachne_ipc_close(void* dev_ptr) {
+  if (!dev_ptr) return ARACHNE_ERR_NULL_POINTER;
+  ARACHNE_CUDA(cudaIpcCloseMemHandle(dev_ptr));
+  return ARACHNE_OK;
+}
+int arachne_ipc_free(void* dev_ptr) {
+  if (!dev_ptr) return ARACHNE_ERR_NULL_POINTER;
+  ARACHNE_CUDA(cudaFree(dev_ptr));
+  return ARACHNE_OK;
+}
+
 // ---------------------------------------------------------------- host-buffer convenience calls
 // Device buffers and the two streams are created on the first host call and cached in the plan (freed by
 // arachne_plan_destroy).  Copies overlap the kernels: dO goes up while the forward runs, O and LSE come down while

@@ -14,8 +14,9 @@ This module holds NO attention arithmetic: integer bookkeeping (who owns which t
 peer-mapped buffer addresses, and the barriers that order the ranks.  The bookkeeping is covered by world-size-2
 gloo tests on CPU (tests/test_ulysses_gloo.py) and the kernels' gather / scatter by single-GPU tests in which
 the k shards are k separate allocations on one device (tests/test_gpu_ulysses.py) — no kernel ever waits on
-another rank's kernel.  The multi-GPU transport (`SymmetricShards`) needs k GPUs and is not exercised on this
-one-GPU pool.
+another rank's kernel.  The drivers below also run as two real processes with real peer mappings (CUDA IPC, both
+ranks on the pool's one GPU: tests/test_gpu_multiproc.py); the symmetric-memory transport (`SymmetricShards`) needs k GPUs
+(it refuses two ranks on one device) and is the one piece not exercised here.
 """
 from __future__ import annotations
 
@@ -84,6 +85,60 @@ class SymmetricShards:
         return self.local_full[:n_local]
 
 
+class IpcShards:
+    """Same interface as SymmetricShards over CUDA IPC (arachne_ipc_alloc / _open): every rank cudaMallocs its shard,
+    the 64-byte handles travel through the process group (all_gather_object), every rank maps the others' shards.  Works
+    with any backend that can gather python objects (gloo, nccl) and also when several ranks share one GPU — which is how
+    the multi-process test runs on a one-GPU box."""
+
+    def __init__(self, n_local_max: int, total_heads: int, head_dim: int, group, device, dtype=None, shape=None):
+        import torch
+        import torch.distributed as dist
+
+        from . import binding
+
+        self._binding = binding
+        self.dtype = dtype or torch.bfloat16
+        self.shape = tuple(shape) if shape is not None else (n_local_max, total_heads, head_dim)
+        numel = 1
+        for x in self.shape:
+            numel *= int(x)
+        nbytes = max(numel, 1) * torch.empty((), dtype=self.dtype).element_size()
+        self._addr, handle = binding.ipc_alloc(nbytes)
+        rank, world = dist.get_rank(group), dist.get_world_size(group)
+        handles = [None] * world
+        dist.all_gather_object(handles, handle, group=group)
+        self._opened = []
+        self.ptrs = []
+        for r in range(world):
+            if r == rank:
+                self.ptrs.append(self._addr)
+            else:
+                a = binding.ipc_open(handles[r])
+                self._opened.append(a)
+                self.ptrs.append(a)
+        self.local_full = binding.tensor_from_address(self._addr, self.shape, self.dtype)
+        self._group = group
+
+    def local(self, n_local: int):
+        return self.local_full[:n_local]
+
+    def close(self):
+        import torch
+        import torch.distributed as dist
+
+        torch.cuda.synchronize()
+        dist.barrier(self._group)                       # nobody is still reading a peer shard
+        for a in self._opened:
+            self._binding.ipc_close(a)
+        self._opened = []
+        dist.barrier(self._group)                       # every peer has unmapped before the owner frees
+        if self._addr:
+            self.local_full = None
+            self._binding.ipc_free(self._addr)
+            self._addr = 0
+
+
 class UlyssesAttention:
     """Forward / backward of the packed attention over an SP group of k GPUs in one NVSwitch domain.
 
@@ -92,7 +147,7 @@ class UlyssesAttention:
     arachne_varlen_attn_fwd_sharded (gather + attention + scatter) -> barrier (every rank's O shard is complete).
     The barriers are the only collectives on the data path; dgamma partials are all-reduced (2 x D floats)."""
 
-    def __init__(self, st: dict, group=None, flags: int = 0):
+    def __init__(self, st: dict, group=None, flags: int = 0, transport: str = "symm"):
         import torch
         import torch.distributed as dist
 
@@ -107,7 +162,8 @@ class UlyssesAttention:
         dev = torch.device("cuda", torch.cuda.current_device())
         self.plan = plan_for_rank(st, self.rank, self.world, flags=flags)
         names = ("q", "k", "v", "o", "dO", "dq", "dk", "dv")
-        self.buf = {n: SymmetricShards(n_max, st["H"], st["D"], group, dev) for n in names}
+        Shards = SymmetricShards if transport == "symm" else IpcShards      # "ipc": CUDA IPC (arachne_ipc_*)
+        self.buf = {n: Shards(n_max, st["H"], st["D"], group, dev) for n in names}
         self.lse = torch.empty((self.plan.H, st["N"]), dtype=torch.float32, device=dev)
         self.ws = torch.empty(max(self.plan.workspace_bytes(False), self.plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
         self._binding = binding
@@ -142,8 +198,20 @@ class UlyssesAttention:
         self._binding.arachne_varlen_attn_bwd_sharded(self.plan, b["q"].ptrs, b["k"].ptrs, b["v"].ptrs, b["o"].ptrs,
                                                       self.lse, b["dO"].ptrs, b["dq"].ptrs, b["dk"].ptrs, b["dv"].ptrs,
                                                       self.ws, dgq, dgk, gamma_q, gamma_k)
-        if with_dgamma:        # gamma is shared by all heads (R1): sum the per-rank partials
-            self._dist.all_reduce(dgq, group=self.group)
-            self._dist.all_reduce(dgk, group=self.group)
+        if with_dgamma:        # gamma is shared by all heads (R1): sum the per-rank partials (2 x D floats)
+            both = torch.stack([dgq, dgk])
+            if self._dist.get_backend(self.group) == "gloo":
+                host = both.cpu()
+                self._dist.all_reduce(host, group=self.group)
+                both = host.to(dgq.device)
+            else:
+                self._dist.all_reduce(both, group=self.group)
+            dgq, dgk = both[0], both[1]
         self._barrier()
         return self.local("dq"), self.local("dk"), self.local("dv"), dgq, dgk
+
+    def close(self):
+        for b in self.buf.values():
+            if hasattr(b, "close"):
+                b.close()
+        self.plan.close()
