@@ -261,6 +261,8 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   const arachne_attn_params& p = *params;
   if (p.head_dim != 64 && p.head_dim != 128) return ARACHNE_ERR_BAD_HEAD_DIM;
   if (p.num_seqs <= 0 || p.num_heads <= 0 || p.total_tokens <= 0 || p.num_heads > 65535) return ARACHNE_ERR_BAD_SHAPE;
+  // 32-bit row / item indices on the device: (tokens + one tile of padding per sequence) x heads must stay below 2^31
+  if ((static_cast<long long>(p.total_tokens) + 128LL * p.num_seqs) * p.num_heads >= (1LL << 31)) return ARACHNE_ERR_BAD_SHAPE;
   int rsum = 0;
   for (int a = 0; a < 3; ++a) {
     if (p.rope_dims[a] < 0 || (p.rope_dims[a] & 1)) return ARACHNE_ERR_BAD_ROPE_DIMS;

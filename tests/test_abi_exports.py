@@ -55,3 +55,11 @@ def test_status_strings_and_validation_without_device():
     gr2 = (ctypes.c_int32 * 3)(1, 8, 9)
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5    # grid mismatch
     assert lib.arachne_varlen_attn_fwd(None, None, None, None, None, None, None, None, None, 0, None) == 1
+    # 32-bit row indices on the device: tokens x heads must stay below 2^31 (rejected before any CUDA call)
+    big = binding.AttnParams()
+    big.num_seqs, big.total_tokens, big.num_heads, big.head_dim = 1, 2 ** 27, 16, 64
+    big.rope_dims[:] = [16, 24, 24]
+    big.rope_theta, big.rms_eps = 10000.0, 1e-6
+    cu_big = (ctypes.c_int32 * 2)(0, 2 ** 27)
+    gr_big = (ctypes.c_int32 * 3)(2 ** 27, 1, 1)
+    assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(big), cu_big, gr_big) == 11
