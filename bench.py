@@ -166,6 +166,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
     ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC: two-pass backward, no atomics")
+    ap.add_argument("--heads", type=int, default=0, help="override the head count: the per-rank share of a Ulysses group of degree H/heads")
     ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -188,6 +189,8 @@ def main():
     # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
     # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
     st = inputs.structure(args.workload, order=args.order, seed_offset=args.seed_offset)
+    if args.heads:
+        st["H"] = args.heads
     st["name"] = args.workload
     st_r = dict(st, index=st["index"])          # same structure on every rank; different bytes per rank
     t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * rank, dev)
