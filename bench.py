@@ -293,6 +293,20 @@ def main():
         v_, dt_, desc, cores = oracle_sample(st, tc, budget_rows=max(8, min(L_max, int(8.0e7 / L_max))), heads=2)
         cpu = {"value": v_, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
+    # per-CTA finish times of the last launch of the two persistent kernels (arachne_plan_cta_times): what the plan's LPT
+    # assignment leaves of the sequence-length skew.  max / mean of the CTA end times; 1.0 = perfectly balanced.
+    cta_balance = None
+    if rank == 0:
+        try:
+            cta_balance = {}
+            for name, is_bwd in (("fwd_kernel", False), ("bwd_fused_kernel", True)):
+                if is_bwd and args.deterministic:
+                    continue
+                _, end_us = plan.cta_times(is_bwd)
+                cta_balance[name] = {"ctas": len(end_us), "end_max_us": max(end_us), "end_mean_us": sum(end_us) / len(end_us),
+                                     "end_min_us": min(end_us), "max_over_mean": max(end_us) / (sum(end_us) / len(end_us))}
+        except Exception as ex:          # never fail the bench line over a diagnostic
+            cta_balance = {"error": str(ex)}
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
@@ -304,7 +318,7 @@ def main():
                    "pct_of_measured_bf16_sustained": 100.0 * value / world / peaks["sustained"],
                    "pct_of_nominal_2250": 100.0 * value / world / 2250.0,
                    "fwd_ms": sum(ms for _, ms in kt_f), "bwd_ms": sum(ms for _, ms in kt_b)},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "cta_balance": cta_balance, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
     }
     print(json.dumps(out))
     if world > 1:

@@ -148,6 +148,14 @@ const char* arachne_kernel_name(int pass, int idx);
 int arachne_plan_enable_profiling(arachne_plan* plan, int enable);
 int arachne_plan_kernel_times(const arachne_plan* plan, int pass, float* ms_sum, int n_kernels, int* n_calls);
 
+/* Per-CTA trace of the LAST launch of a persistent kernel (kernel: 0 = fwd_kernel, 1 = bwd_fused_kernel): every CTA
+ * stamps %globaltimer when it starts and when it has finished its last work item (two 8-byte stores per CTA; always on).
+ * Writes start_us[c], end_us[c] (microseconds since the earliest CTA start) for c < *n_ctas; n = capacity of the arrays
+ * (>= the SM count).  Synchronous (cudaMemcpy): call it after the stream has been synchronised.  The spread of end_us is
+ * the load imbalance the plan's LPT assignment leaves (BASELINE.json north_star: "persistent tile scheduler that
+ * balances work across SMs regardless of sequence-length skew"; the paper's Fig. 9 / Fig. 10 analogue inside one GPU). */
+int arachne_plan_cta_times(const arachne_plan* plan, int kernel, double* start_us, double* end_us, int n, int* n_ctas);
+
 /* Forward.  q, k, v: raw bf16 [N,H,D] (Q, K pre-norm, pre-RoPE).  Writes o (bf16 [N,H,D])
  * and lse (fp32 [H,N]).  workspace: >= arachne_workspace_bytes(plan, 0), 256-byte aligned
  * recommended (16 required); its contents are scratch. */

@@ -28,7 +28,7 @@ EXPORTS = [
     "arachne_plan_create_joint", "arachne_varlen_attn_bwd_dgamma",
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
     "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
-    "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free",
+    "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free", "arachne_plan_cta_times",
 ]
 
 
@@ -98,6 +98,11 @@ _lib.arachne_ipc_close.restype = ctypes.c_int
 _lib.arachne_ipc_close.argtypes = [_vp]
 _lib.arachne_ipc_free.restype = ctypes.c_int
 _lib.arachne_ipc_free.argtypes = [_vp]
+
+
+_lib.arachne_plan_cta_times.restype = ctypes.c_int
+_lib.arachne_plan_cta_times.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                        ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
 
 
 class ArachneError(RuntimeError):
@@ -180,6 +185,13 @@ class Plan:
         _check(_lib.arachne_plan_kernel_times(self._h, 1 if bwd else 0, ms, n, ctypes.byref(calls)))
         c = max(calls.value, 1)
         return [(_lib.arachne_kernel_name(1 if bwd else 0, i).decode(), ms[i] / c) for i in range(n)], calls.value
+
+    def cta_times(self, bwd: bool):
+        """(start_us[], end_us[]) of every CTA of the last fwd_kernel / bwd_fused_kernel launch (arachne_plan_cta_times)."""
+        cap = 256
+        s, e, n = (ctypes.c_double * cap)(), (ctypes.c_double * cap)(), ctypes.c_int(0)
+        _check(_lib.arachne_plan_cta_times(self._h, 1 if bwd else 0, s, e, cap, ctypes.byref(n)))
+        return list(s[:n.value]), list(e[:n.value])
 
     def close(self):
         if self._h:

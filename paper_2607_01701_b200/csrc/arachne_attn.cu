@@ -61,11 +61,14 @@ struct arachne_plan {
   TokInfo* d_tok_info = nullptr;
   WorkItem* d_items = nullptr;
   WorkItem* d_fwd_items = nullptr;
+  WorkItem* d_dyn_items = nullptr;      // the global LPT-ordered lists (dynamic distribution in fwd_kernel / bwd_fused_kernel)
+  WorkItem* d_dyn_fwd_items = nullptr;
   int* d_item_ptr = nullptr;
   int* d_fwd_item_ptr = nullptr;
   int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
   unsigned* d_stats = nullptr;
+  unsigned long long* d_cta_trace = nullptr;   // [2][kTraceMaxCtas][2] globaltimer ns (arachne_plan_cta_times)
   float2* d_rope = nullptr;
   ProblemDesc pd{};
   // workspace layout
@@ -162,6 +165,7 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.q_prescale = 1.0f;
   pp.gq_zero = deterministic ? nullptr : b.gq_t;
   prof_mark(pl, 1, 0, st);
+  ARACHNE_CUDA(cudaMemsetAsync(pl->d_stats + 3, 0, sizeof(unsigned), st));       // bwd_fused_kernel's work counter
   prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
@@ -359,6 +363,9 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     }
   };
   std::vector<int> item_ptr, fwd_item_ptr;
+  std::vector<WorkItem> dyn_items = items, dyn_fwd_items = fwd_items;     // before the static deal: global LPT order
+  if (dyn_items.empty()) dyn_items.push_back(WorkItem{0, 0, 0, 0});
+  if (dyn_fwd_items.empty()) dyn_fwd_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_ctas = std::min(pl->num_sms, pl->n_items);
   pl->n_fwd_ctas = std::min(pl->num_sms, pl->n_fwd_items);
   deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].qt_n); }, item_ptr);
@@ -404,18 +411,24 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   PLAN_UP(pl->d_items, items, WorkItem)
   PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
+  PLAN_UP(pl->d_dyn_items, dyn_items, WorkItem)
+  PLAN_UP(pl->d_dyn_fwd_items, dyn_fwd_items, WorkItem)
   PLAN_UP(pl->d_item_ptr, item_ptr, int)
   PLAN_UP(pl->d_fwd_item_ptr, fwd_item_ptr, int)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_stats), 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
   if ((e = cudaMemset(pl->d_stats, 0, 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
+  if (pl->num_sms <= kTraceMaxCtas) {
+    if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
+    if ((e = cudaMemset(pl->d_cta_trace, 0, 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
+  }
   int rc = p.head_dim == 128 ? configure_kernels<128>() : configure_kernels<64>();
   if (rc != ARACHNE_OK) { arachne_plan_destroy(pl); return rc; }
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.item_ptr = pl->d_item_ptr; pd.fwd_item_ptr = pl->d_fwd_item_ptr; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats;
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.fwd_item_ptr = pl->d_fwd_item_ptr; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats; pd.cta_trace = pl->d_cta_trace; pd.work_counter = reinterpret_cast<int*>(pl->d_stats + 2);
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -454,7 +467,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_fwd_item_ptr); cudaFree(pl->d_stats); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_fwd_item_ptr); cudaFree(pl->d_stats); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
   delete pl;
 }
 
@@ -477,6 +490,21 @@ const char* arachne_kernel_name(int pass, int idx) {
   if (pass == 0 && idx >= 0 && idx < 2) return fwd[idx];
   if (pass == 1 && idx >= 0 && idx < 4) return bwd[idx];
   return "";
+}
+
+int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us, double* end_us, int n, int* n_ctas) {
+  if (!pl || !start_us || !end_us || !n_ctas) return ARACHNE_ERR_NULL_POINTER;
+  if (kernel < 0 || kernel > 1 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
+  const int ctas = kernel == 0 ? pl->n_fwd_ctas : pl->n_ctas;
+  if (n < ctas) return ARACHNE_ERR_BAD_PARAM;
+  std::vector<unsigned long long> t(static_cast<size_t>(kTraceMaxCtas) * 2);
+  ARACHNE_CUDA(cudaMemcpy(t.data(), pl->d_cta_trace + static_cast<size_t>(kernel) * kTraceMaxCtas * 2, t.size() * sizeof(unsigned long long),
+                          cudaMemcpyDeviceToHost));
+  unsigned long long t0 = ~0ull;
+  for (int c = 0; c < ctas; ++c) t0 = std::min(t0, t[2 * c]);
+  for (int c = 0; c < ctas; ++c) { start_us[c] = (t[2 * c] - t0) * 1e-3; end_us[c] = (t[2 * c + 1] - t0) * 1e-3; }
+  *n_ctas = ctas;
+  return ARACHNE_OK;
 }
 
 int arachne_plan_enable_profiling(arachne_plan* pl, int enable) {

@@ -51,9 +51,9 @@ struct BwdFusedCfg {
   static constexpr int kDOStages = (D == 128) ? 1 : 2;
   static constexpr int kDSBytes = kTileRows * kTileRows * 2;      // dS^T image, 128 x 128 bf16
   static constexpr int kStageBytes = kTileRows * 64 * 4;           // dQ~ staging: 128 rows x 64 fp32
-  static constexpr int kNumBars = 2 + 2 * kQStages + 2 * kDOStages + 9;
+  static constexpr int kNumBars = 2 + 2 * kQStages + 2 * kDOStages + 9 + 2 * kItemRing;
   static constexpr int kSmemBytes = kTileBytes * (2 + kQStages + kDOStages) + kDSBytes + kStageBytes +
-                                    kQStages * 1024 + 8 * kNumBars + 16;
+                                    kQStages * 1024 + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 512;   // 4 warpgroups: compute, compute, dQ~ drain, {producer, MMA, 2 idle warps}
   static constexpr uint32_t kColS = 0, kColDP = 128, kColDV = 256, kColDK = 256 + D;
 };
@@ -114,7 +114,11 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
   uint64_t* dq_empty = dq_full + 1;        // drain (128) -> MMA
   uint64_t* acc_done = dq_empty + 1;       // MMA -> compute (epilogue)
   uint64_t* acc_free = acc_done + 1;       // compute (256) -> MMA
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_free + 1);
+  uint64_t* it_full = acc_free + 1;        // [kItemRing] work-item ring (sm100.cuh)
+  uint64_t* it_empty = it_full + kItemRing;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(it_empty + kItemRing);
+  int* sItem = reinterpret_cast<int*>(tmem_slot + 1);      // [kItemRing] (the 16 spare bytes of the layout hold 1 + up to 3; see kSmemBytes)
+  const ItemRing ring{sItem, it_full, it_empty};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -127,11 +131,13 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     mbar_init(ds_free, 1);
     mbar_init(dq_full, 1); mbar_init(dq_empty, 128);
     mbar_init(acc_done, 1); mbar_init(acc_free, 256);
+    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], 13); }   // consumers: MMA + 8 compute + 4 drain warps
     fence_mbar_init();
   }
   if (warp == 13) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
+  if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(1 * kTraceMaxCtas + blockIdx.x) * 2] = globaltimer_ns();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
   const float scale_log2 = pd.softmax_scale * 1.4426950408889634f;
@@ -144,8 +150,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     // ------------------------------------------------------------------ producer
     setmaxnreg_dec<56>();
     uint32_t it = 0, g = 0;
-    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.items[item];
+    for (;; ++it) {
+      const int item = item_fetch_producer(ring, it, pd.work_counter + 1, pd.n_items, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const size_t hoff = wi.head * head_stride;
       mbar_wait(kv_free, (it & 1) ^ 1);
@@ -252,8 +260,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       }
       __syncwarp();
     };
-    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.items[item];
+    for (;; ++it) {
+      const int item = item_fetch_consumer(ring, it, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_items[item];
       const uint32_t n = pd.seqs[wi.seq].qt_n;        // query tiles this process visits (all, unless context-parallel)
       mbar_wait(kv_full, it & 1);
       issue_S(g0);
@@ -282,8 +292,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     const uint32_t tdP = tbase + Cfg::kColDP + lane_base + wg * 64;
     uint8_t* dS_row = sdS + wg * BLK + r * 128;                // this row's 128 bytes in block wg of the dS^T image
     uint32_t it = 0, g = 0;
-    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.items[item];
+    for (;; ++it) {
+      const int item = item_fetch_consumer(ring, it, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const uint32_t qs = g % QS, qph = (g / QS) & 1;
@@ -415,8 +427,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
         bulk_commit_group();
       }
     };
-    for (int item = pd.item_ptr[blockIdx.x]; item < pd.item_ptr[blockIdx.x + 1]; ++item) {
-      const WorkItem wi = pd.items[item];
+    for (uint32_t it = 0;; ++it) {
+      const int item = item_fetch_consumer(ring, it, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const int qt = sq.qt_lo + q_tile_of(wi, i, sq.qt_n);
@@ -447,6 +461,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
   }
   tc_fence_before();
   __syncthreads();
+  if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(1 * kTraceMaxCtas + blockIdx.x) * 2 + 1] = globaltimer_ns();
   if (warp == 13) tmem_dealloc(tbase, 512);
 }
 

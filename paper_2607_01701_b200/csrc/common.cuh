@@ -94,6 +94,13 @@ __device__ __forceinline__ T* raw_row(const Sharding& sh, const ShardedPtr& t, i
   return shard_base<T>(t, r) + off;
 }
 
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+constexpr int kTraceMaxCtas = 256;
+
 struct ProblemDesc {
   const SeqInfo* seqs;
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
@@ -101,6 +108,9 @@ struct ProblemDesc {
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
   const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int n_fwd_items;
+  const WorkItem* dyn_items;     // [n_items] the same items in the global LPT order, taken dynamically (work_counter)
+  const WorkItem* dyn_fwd_items; // [n_fwd_items]
+  int* work_counter;             // [2] next index into dyn_fwd_items / dyn_items; zeroed by the host before each launch
   const int* item_ptr;       // [n_ctas + 1] CTA c owns items [item_ptr[c], item_ptr[c+1]) (host LPT assignment)
   const int* fwd_item_ptr;   // [n_fwd_ctas + 1] likewise for fwd_items
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel
@@ -113,6 +123,7 @@ struct ProblemDesc {
   int no_norm, no_rope;
   RopeDesc rope;
   Sharding sh;
+  unsigned long long* cta_trace;   // nullable: [kernel 0 fwd | 1 bwd_fused][gridDim.x][2] globaltimer ns at CTA start / end
   int cp_lo, cp_hi;          // context parallelism: this process owns the QUERY tokens [cp_lo, cp_hi) (0, N otherwise)
 };
 

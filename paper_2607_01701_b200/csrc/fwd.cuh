@@ -82,6 +82,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   if (warp == 9) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
+  if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2] = globaltimer_ns();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
   const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
@@ -336,6 +337,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   }
   tc_fence_before();
   __syncthreads();
+  if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2 + 1] = globaltimer_ns();
   if (warp == 9) tmem_dealloc(tbase, 512);
 }
 

@@ -73,6 +73,37 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   }
 }
 
+// ---------------------------------------------------------------- dynamic work distribution inside a persistent CTA
+// One lane of the producer warp takes the next index of the (LPT-ordered) work list with an atomic and publishes it
+// through a small ring in shared memory; every other warp role reads it from there.  `it` is the CTA-local item
+// counter (the same in every role).  A negative item ends the loop.  n_consumer_warps arrive on `empty` per slot.
+constexpr int kItemRing = 4;
+struct ItemRing {
+  int* slot;          // [kItemRing]
+  uint64_t* full;     // [kItemRing] producer (1 arrival) -> consumers
+  uint64_t* empty;    // [kItemRing] consumer warps -> producer
+};
+__device__ __forceinline__ int item_fetch_producer(const ItemRing& r, uint32_t it, int* counter, int n_items, int lane) {
+  const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
+  int item = 0;
+  if (lane == 0) {
+    mbar_wait(&r.empty[s], ph ^ 1);
+    item = atomicAdd(counter, 1);
+    if (item >= n_items) item = -1;
+    r.slot[s] = item;
+    mbar_arrive(&r.full[s]);          // release: the slot write is visible to whoever observes the phase
+  }
+  return __shfl_sync(0xffffffffu, item, 0);
+}
+__device__ __forceinline__ int item_fetch_consumer(const ItemRing& r, uint32_t it, int lane) {
+  const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
+  mbar_wait(&r.full[s], ph);
+  const int item = r.slot[s];
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&r.empty[s]);
+  return item;
+}
+
 // ---------------------------------------------------------------- bulk copies (TMA engine)
 // global -> shared, completion signalled on an mbarrier (complete_tx)
 __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes,
