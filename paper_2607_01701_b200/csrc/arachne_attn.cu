@@ -60,11 +60,9 @@ struct arachne_plan {
   int* d_tile_seq = nullptr;
   TokInfo* d_tok_info = nullptr;
   WorkItem* d_items = nullptr;
-  WorkItem* d_fwd_items = nullptr;
   WorkItem* d_dyn_items = nullptr;      // the global LPT-ordered lists (dynamic distribution in fwd_kernel / bwd_fused_kernel)
   WorkItem* d_dyn_fwd_items = nullptr;
   int* d_item_ptr = nullptr;
-  int* d_fwd_item_ptr = nullptr;
   int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
   unsigned* d_stats = nullptr;
@@ -342,9 +340,11 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
         fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].qt_lo + pl->seqs[b].qt_n - t)});
   pl->n_items = static_cast<int>(items.size());
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
-  // Static LPT assignment to the persistent CTAs: the lists are in decreasing-cost order, each item goes to the
-  // least-loaded CTA (ties: lowest index — while costs are equal this is round-robin, so CTAs running side by side
-  // stay on adjacent tiles of the same (sequence, head) group), and every CTA's items are stored contiguously.
+  // fwd_kernel and bwd_fused_kernel take the items of these LPT-ordered lists DYNAMICALLY (an atomic counter, sm100.cuh
+  // ItemRing): list scheduling in decreasing-cost order, and CTAs that are a little faster simply take more items.
+  // The deterministic two-pass kernels keep a STATIC LPT assignment: each item goes to the least-loaded CTA (ties: lowest
+  // index — while costs are equal this is round-robin, so CTAs running side by side stay on adjacent tiles of the same
+  // (sequence, head) group), and every CTA's items are stored contiguously.
   auto deal = [&](std::vector<WorkItem>& list, int n_cta, auto cost, std::vector<int>& ptr) {
     if (n_cta == 0) { ptr.assign(1, 0); return; }
     std::vector<long long> load(n_cta, 0);
@@ -362,16 +362,14 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
       ptr.push_back(static_cast<int>(list.size()));
     }
   };
-  std::vector<int> item_ptr, fwd_item_ptr;
+  std::vector<int> item_ptr;
   std::vector<WorkItem> dyn_items = items, dyn_fwd_items = fwd_items;     // before the static deal: global LPT order
   if (dyn_items.empty()) dyn_items.push_back(WorkItem{0, 0, 0, 0});
   if (dyn_fwd_items.empty()) dyn_fwd_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_ctas = std::min(pl->num_sms, pl->n_items);
   pl->n_fwd_ctas = std::min(pl->num_sms, pl->n_fwd_items);
   deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].qt_n); }, item_ptr);
-  deal(fwd_items, pl->n_fwd_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].n_tiles) * w.pad; }, fwd_item_ptr);
   if (items.empty()) items.push_back(WorkItem{0, 0, 0, 0});          // (a CP rank that owns no queries: nothing is launched)
-  if (fwd_items.empty()) fwd_items.push_back(WorkItem{0, 0, 0, 0});
   // RoPE tables in fp64 -> fp32 (readings R4, R5)
   std::vector<float2> tab;
   RopeDesc rd{};
@@ -410,11 +408,9 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     PLAN_UP(pl->d_tok_info, ti, TokInfo)
   }
   PLAN_UP(pl->d_items, items, WorkItem)
-  PLAN_UP(pl->d_fwd_items, fwd_items, WorkItem)
   PLAN_UP(pl->d_dyn_items, dyn_items, WorkItem)
   PLAN_UP(pl->d_dyn_fwd_items, dyn_fwd_items, WorkItem)
   PLAN_UP(pl->d_item_ptr, item_ptr, int)
-  PLAN_UP(pl->d_fwd_item_ptr, fwd_item_ptr, int)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_stats), 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
@@ -428,7 +424,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.fwd_items = pl->d_fwd_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.fwd_item_ptr = pl->d_fwd_item_ptr; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats; pd.cta_trace = pl->d_cta_trace; pd.work_counter = reinterpret_cast<int*>(pl->d_stats + 2);
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats; pd.cta_trace = pl->d_cta_trace; pd.work_counter = reinterpret_cast<int*>(pl->d_stats + 2);
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -467,7 +463,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_fwd_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_fwd_item_ptr); cudaFree(pl->d_stats); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
   delete pl;
 }
 

@@ -106,13 +106,11 @@ struct ProblemDesc {
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
   const TokInfo* tok_info;   // [N]
   const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
-  const WorkItem* fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int n_fwd_items;
   const WorkItem* dyn_items;     // [n_items] the same items in the global LPT order, taken dynamically (work_counter)
-  const WorkItem* dyn_fwd_items; // [n_fwd_items]
+  const WorkItem* dyn_fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int* work_counter;             // [2] next index into dyn_fwd_items / dyn_items; zeroed by the host before each launch
   const int* item_ptr;       // [n_ctas + 1] CTA c owns items [item_ptr[c], item_ptr[c+1]) (host LPT assignment)
-  const int* fwd_item_ptr;   // [n_fwd_ctas + 1] likewise for fwd_items
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel
   int n_items;
   int n_tiles_total;

@@ -35,8 +35,8 @@ template <int D>
 struct FwdCfg {
   static constexpr int kTileBytes = kTileRows * D * 2;
   static constexpr int kRing = (D == 128) ? 5 : 8;       // K/V ring slots (K_j, V_j alternate)
-  static constexpr int kNumBars = 2 + 2 * kRing + 8;
-  static constexpr int kSmemBytes = kTileBytes * (2 + kRing) + 8 * kNumBars + 16;
+  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * kItemRing;
+  static constexpr int kSmemBytes = kTileBytes * (2 + kRing) + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 320;
   // every 4th exp2 on the FMA pipe (ex2_poly3) instead of MUFU: pays at D = 64, where MUFU (16 ex2/clk/SM) is the
   // busiest unit (cogvideox fwd 13.0 vs 14.7 ms); at D = 128 the loop is tensor/power-bound and the extra FMA-pipe
@@ -66,7 +66,11 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   uint64_t* p_full = s_full + 2;         // [2] softmax (128 arrivals) -> MMA
   uint64_t* pv_done = p_full + 2;        // [2] MMA (commit) -> softmax: one phase per PV
   uint64_t* o_free = pv_done + 2;        // [2] softmax epilogue (128 arrivals) -> MMA
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_free + 2);
+  uint64_t* it_full = o_free + 2;        // [kItemRing] work-item ring (sm100.cuh): items are taken dynamically
+  uint64_t* it_empty = it_full + kItemRing;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(it_empty + kItemRing);
+  int* sItem = reinterpret_cast<int*>(tmem_slot + 1);
+  const ItemRing item_ring{sItem, it_full, it_empty};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -77,6 +81,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
       mbar_init(&s_full[t], 1); mbar_init(&p_full[t], 128);
       mbar_init(&pv_done[t], 1); mbar_init(&o_free[t], 128);
     }
+    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], 9); }   // consumers: MMA + 8 softmax warps
     fence_mbar_init();
   }
   if (warp == 9) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
@@ -90,8 +95,10 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   if (warp == 8) {
     // ------------------------------------------------------------------ producer
     uint32_t it = 0, ring = 0;
-    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.fwd_items[item];
+    for (;; ++it) {
+      const int item = item_fetch_producer(item_ring, it, pd.work_counter, pd.n_fwd_items, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_fwd_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const int n_q = wi.pad;
       const uint8_t* hbase_q = fp.qt + wi.head * head_stride;
@@ -125,8 +132,10 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     const uint32_t aQ = smem_u32(sQ), aKV = smem_u32(sKV);
     uint32_t it = 0, ring = 0;      // ring: slot counter at K_0 of the current item (K_j = ring+2j, V_j = ring+2j+1)
     uint32_t cnt[2] = {0, 0};       // per query tile: number of PV tiles issued so far
-    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.fwd_items[item];
+    for (;; ++it) {
+      const int item = item_fetch_consumer(item_ring, it, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_fwd_items[item];
       const int n_kv = pd.seqs[wi.seq].n_tiles;
       const int n_q = wi.pad;
       // S_t,j : waits K_j on first use, releases the slot (and Q^ after the last tile) on last use
@@ -194,8 +203,10 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     // range.  Anything larger (no_norm debug flag, huge gamma) takes the online-softmax path below.
     const float bound = sqrtf(__uint_as_float(pd.stats[0])) * sqrtf(__uint_as_float(pd.stats[1]));
     const bool static_max = bound <= kStaticMaxBound;     // false for NaN / inf
-    for (int item = pd.fwd_item_ptr[blockIdx.x]; item < pd.fwd_item_ptr[blockIdx.x + 1]; ++item, ++it) {
-      const WorkItem wi = pd.fwd_items[item];
+    for (;; ++it) {
+      const int item = item_fetch_consumer(item_ring, it, lane);
+      if (item < 0) break;
+      const WorkItem wi = pd.dyn_fwd_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       if (t >= wi.pad) {
         // odd trailing tile: warps 4-7 sit this item out, but keep the o_free phase in step with `it`
