@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/r1b_ncu_720p.md); only known for the workload that was captured.
-NCU_TRAFFIC = {("long720p", "bwd_main(fused 5-GEMM | det: dKdV pass)"): 47.08e9, ("long720p", "fwd_kernel"): 11.6e9}
+NCU_TRAFFIC = {("long720p", "bwd_main(fused 5-GEMM | det: dKdV pass)"): 52.91e9, ("long720p", "fwd_kernel"): 6.10e9}
 
 METRIC = "varlen 3D attention fwd+bwd TFLOPS"
 UNIT = "TFLOP/s"
