@@ -4,7 +4,9 @@
 // of the additions is not fixed -> run-to-run bit differences; ARACHNE_FLAG_DETERMINISTIC selects
 // the two-pass kernels of bwd.cuh instead).
 //
-// Work item = (sequence b, head h, 128-row KEY tile).  The CTA keeps K^ and V of the tile in shared
+// Work item = (sequence b, head h, 128-row KEY tile).
+// Items are taken DYNAMICALLY from the plan's LPT-ordered list: lane 0 of the producer warp does an atomicAdd on a per-launch
+// counter and hands the index to the other warp roles through a 4-slot shared-memory ring (sm100.cuh, ItemRing).  The CTA keeps K^ and V of the tile in shared
 // memory and streams the ceil(L_b/128) QUERY tiles of sequence b only (block-diagonal):
 //
 //   S^T  = K^  Q^_i^T        SS   [128 keys x 128 queries] fp32 -> TMEM cols [0,128)

@@ -1,6 +1,8 @@
 // Forward kernel (§8 a2-a4): persistent, warp-specialised, tcgen05 + TMEM, two query tiles in flight.
 //
 // Work item = (sequence b, head h, PAIR of 128-row query tiles) (a trailing odd tile runs alone).
+// Items are taken DYNAMICALLY from the plan's LPT-ordered list: lane 0 of the producer warp does an atomicAdd on a per-launch
+// counter and hands the index to the other warp roles through a 4-slot shared-memory ring (sm100.cuh, ItemRing).
 // Per item the CTA streams the ceil(L_b/128) key/value tiles of sequence b ONLY (block-diagonal:
 // no other tile is ever touched, no masked-out tile is computed).  The two query tiles ping-pong on
 // the tensor pipe so that the softmax of one overlaps the GEMMs of the other:
