@@ -195,7 +195,9 @@ def main():
     st_r = dict(st, index=st["index"])          # same structure on every rank; different bytes per rank
     t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * rank, dev)
          for tid, k in ((1, "q"), (2, "k"), (3, "v"), (4, "dO"))}
+    t_plan = time.perf_counter()
     plan = binding.plan_for(st_r, flags=binding.FLAG_DETERMINISTIC if args.deterministic else 0)
+    plan_ms = 1e3 * (time.perf_counter() - t_plan)      # host: validation, work lists, LPT order, RoPE / token tables, upload (not in the step)
     ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
     o = torch.empty_like(t["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=dev)
     dq, dk, dv = (torch.empty_like(t["q"]) for _ in range(3))
@@ -311,7 +313,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "deterministic_bwd": bool(args.deterministic), "num_seqs": len(st["grids"]), "total_tokens": st["N"],
+        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "plan_create_ms": round(plan_ms, 3), "deterministic_bwd": bool(args.deterministic), "num_seqs": len(st["grids"]), "total_tokens": st["N"],
                    "heads": st["H"], "head_dim": st["D"], "flop_per_step": flops,
                    "l2": "inputs larger than L2 (4 x %.0f MB bf16 tensors + tiled workspace)" % (t["q"].numel() * 2 / 1e6),
                    "pct_of_measured_bf16_burst": 100.0 * value / world / peaks["burst"],
