@@ -115,7 +115,11 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
   const int t = gtile - sq.tile_base;
   const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
   const size_t row_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows;
-  if (pp.gq_zero) {
+  // Context parallelism: K^ / V images are needed for every tile of a sequence this rank touches, the QUERY-side data
+  // (Q^ image, dO image, lse2, delta, the dq~ accumulator) only for the tiles that hold some of the rank's own rows.
+  const bool touched = sq.qt_n > 0;                              // a sequence without rows of this rank: nothing to prepare
+  const bool q_side = t >= sq.qt_lo && t < sq.qt_lo + sq.qt_n;   // always true without CP
+  if (pp.gq_zero && q_side) {
     float4* z = reinterpret_cast<float4*>(pp.gq_zero + (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * (kTileRows * D));
     for (int i = threadIdx.x; i < kTileRows * D / 4; i += 256) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
@@ -127,7 +131,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
   }
   const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll 1
-  for (int r = warp * RPW + sub; r < kTileRows; r += 8 * RPW) {
+  for (int r = warp * RPW + sub; touched && r < kTileRows; r += 8 * RPW) {
     const int n = t * kTileRows + r;            // token index inside the sequence
     const bool valid = n < sq.len;
     const int tok = sq.tok_start + (valid ? n : 0);
@@ -137,10 +141,10 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     const size_t src = raw_off(pd.sh, tok, h, D, shard) + d0;
     uint4 uq = zero4, uk = zero4, uv = zero4, ug = zero4, uo = zero4;
     if (valid) {
-      uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
+      if (q_side) uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
       uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src);
       uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);
-      if (pp.backward) {
+      if (pp.backward && q_side) {
         ug = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src);
         uo = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.o, shard) + src);
       }
@@ -153,12 +157,12 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     const float qs = norm_rope8<D>(xq, gq, cs, pd.no_norm != 0, pd.eps, pp.q_prescale);
     const float ks = norm_rope8<D>(xk, gk, cs, pd.no_norm != 0, pd.eps, 1.0f);
     const uint32_t ioff = image_off(r, d0);
-    *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, pp.out_fmt) : zero4;   // (eps = 0: 0 * inf)
+    if (q_side) *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, pp.out_fmt) : zero4;   // (eps = 0: 0 * inf)
     *reinterpret_cast<uint4*>(pp.kt + img_off + ioff) = valid ? pack8(xk, pp.out_fmt) : zero4;
     *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
     // row norms are only needed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, seg_sum<LPR>(qs)); kn = fmaxf(kn, seg_sum<LPR>(ks)); }
-    if (pp.backward) {
+    if (pp.backward && q_side) {
       *reinterpret_cast<uint4*>(pp.dot + img_off + ioff) = ug;
       float g[8], oo[8];
       unpack_bf16x8(ug, g);
