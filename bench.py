@@ -1,20 +1,23 @@
 #!/usr/bin/env python
 """bench.py — varlen 3D attention fwd+bwd TFLOPS on B200 (BASELINE.json `metric`).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload long720p] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload long720p] [--impl reference] [--sp ulysses|cp]
 
-One "step" = one forward + one backward of the whole hot path (prep, fwd, prep, dK/dV, dQ, post
-kernels) over one packed batch of synthetic N(0,1) bf16 inputs of the named BASELINE.json config.
-`value` = 14*D*H*sum(L_b^2) / t (real lengths; norm/RoPE/softmax and the extra recompute GEMMs of
-the deterministic two-pass backward count as time, not FLOPs), inputs resident in HBM.  `e2e` is
-the same metric through the C-ABI host call (pinned host buffers, H2D + D2H inside the timed
-region).  `roofline` is for the dominant kernel, timed live with CUDA events recorded by the
-library on the launching stream.  `cpu_baseline` is the fp64 oracle timed on the host cores on a
-bounded sample of the same workload (reported, not a target).  Prints ONE JSON line.
+One "step" = one forward + one backward of the whole hot path (prep, fwd, prep, scale, backward main, post kernels)
+over one packed batch of synthetic N(0,1) bf16 inputs of the named BASELINE.json config.
+`value` = 14*D*H*sum(L_b^2) / t (real lengths; norm/RoPE/softmax and every prologue / epilogue kernel count as time, not
+FLOPs), inputs resident in HBM.  `e2e` is the same metric through the C-ABI host call (pinned host buffers, H2D + D2H
+inside the timed region; median of >= 5 repetitions).  `roofline` is for the dominant kernel, timed live with CUDA events
+recorded by the library on the launching stream.  `cpu_baseline` is the fp64 oracle timed on the host cores on a bounded
+sample of the same workload (reported, not a target).  `config.targets` carries BOTH north_star targets in one record:
+the 720p long clip (>= 60 % of the measured bf16 burst peak) and the heavy-tailed batch (>= 50 %), plus the deterministic
+backward on the main workload.  Prints ONE JSON line.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import hashlib
 import json
 import os
 import subprocess
@@ -25,12 +28,10 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1b_ncu_720p.md); only known for the workload that was captured.
-NCU_TRAFFIC = {("long720p", "bwd_main(fused 5-GEMM | det: dKdV pass)"): 52.91e9, ("long720p", "fwd_kernel"): 6.10e9}
-
 METRIC = "varlen 3D attention fwd+bwd TFLOPS"
 UNIT = "TFLOP/s"
+WORKLOADS = ["tiny", "bucket256", "mixed480p", "long720p", "heavytail", "joint720p", "cogvideox"]
+TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")      # written by hand from an `ncu --set full` capture (profiles/r2_ncu.md)
 
 
 def load_peaks():
@@ -42,6 +43,32 @@ def load_peaks():
                     hbm=float(p["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
     # fallback stated in B200_PROFILING.md
     return dict(burst=1590.0, sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the CUDA sources: ties an ncu capture to the kernels it was taken from."""
+    d = os.path.join(ROOT, "paper_2607_01701_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, f), "rb") as fh:
+                h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed capture — only if the capture
+    was taken from the kernels as they are now (source hash); otherwise None and the reason."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
+        return None, f"{TRAFFIC_CSV} absent"
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload and row["kernel"] in kernel:
+                if row["src_sha"] != kernel_source_hash():
+                    return None, f"{TRAFFIC_CSV}: capture predates the current kernels (src {row['src_sha']} != {kernel_source_hash()})"
+                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), f"{TRAFFIC_CSV} ({row['report']}, src {row['src_sha']})"
+    return None, f"{TRAFFIC_CSV}: no row for {workload} / {kernel}"
 
 
 class ClockSampler:
@@ -118,7 +145,6 @@ def oracle_sample(st, tensors_cpu, budget_rows=6, heads=2):
 
 def run_reference(args):
     """--impl reference: the oracle on the host cores (this tier's reference arm)."""
-    import torch
     from paper_2607_01701_b200 import inputs
 
     rank = int(os.environ.get("RANK", "0"))
@@ -129,7 +155,6 @@ def run_reference(args):
     from oracle import arachne_oracle as orc
     orc.build()
     # a bounded sample per step so that K+W steps finish within minutes
-    sub = {n: None for n in ("q", "k", "v", "dO")}
     cu = st["cu_seqlens"]
     b = max(range(len(cu) - 1), key=lambda i: cu[i + 1] - cu[i])
     L = cu[b + 1] - cu[b]
@@ -155,90 +180,156 @@ def run_reference(args):
     }))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="long720p", choices=["tiny", "bucket256", "mixed480p", "long720p", "heavytail", "joint720p", "cogvideox"])
-    ap.add_argument("--impl", default="arachne", choices=["arachne", "reference"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
-    ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC: two-pass backward, no atomics")
-    ap.add_argument("--heads", type=int, default=0, help="override the head count: the per-rank share of a Ulysses group of degree H/heads")
-    ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
+class Env:
+    """Process-wide context: ranks, device, barrier."""
 
-    import torch
-    import torch.distributed as dist
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist = torch, dist
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU fallback")
+        torch.cuda.set_device(self.local_rank)
+        self.dev = torch.device("cuda", self.local_rank)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=self.dev)
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, x: float) -> float:
+        if self.world == 1:
+            return x
+        tt = self.torch.tensor([x], device=self.dev, dtype=self.torch.float64)
+        self.dist.all_reduce(tt, op=self.dist.ReduceOp.MAX)
+        return float(tt.item())
+
+
+def time_workload(env: Env, workload, steps, warmup, deterministic=False, order="listed", seed_offset=0, heads=0, keep=False):
+    """W untimed + K timed steps of `workload` (device-resident inputs; every rank its own batch of the same structure).
+    Returns the measurement dict (and, with keep, the live objects for the e2e / cpu_baseline legs)."""
+    torch = env.torch
     from paper_2607_01701_b200 import binding, inputs     # raises if libarachne_attn.so is missing
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
-    # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
-    st = inputs.structure(args.workload, order=args.order, seed_offset=args.seed_offset)
-    if args.heads:
-        st["H"] = args.heads
-    st["name"] = args.workload
-    st_r = dict(st, index=st["index"])          # same structure on every rank; different bytes per rank
-    t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * rank, dev)
+    st = inputs.structure(workload, order=order, seed_offset=seed_offset)
+    if heads:
+        st["H"] = heads
+    st["name"] = workload
+    t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * env.rank, env.dev)
          for tid, k in ((1, "q"), (2, "k"), (3, "v"), (4, "dO"))}
     t_plan = time.perf_counter()
-    plan = binding.plan_for(st_r, flags=binding.FLAG_DETERMINISTIC if args.deterministic else 0)
+    plan = binding.plan_for(st, flags=binding.FLAG_DETERMINISTIC if deterministic else 0)
     plan_ms = 1e3 * (time.perf_counter() - t_plan)      # host: validation, work lists, LPT order, RoPE / token tables, upload (not in the step)
-    ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
-    o = torch.empty_like(t["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=dev)
+    ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device=env.dev)
+    o = torch.empty_like(t["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=env.dev)
     dq, dk, dv = (torch.empty_like(t["q"]) for _ in range(3))
     flops = inputs.attention_flops(st)
-    s2 = flops / (14.0 * st["D"] * st["H"])
 
     def step():
         binding.arachne_varlen_attn_fwd(plan, t["q"], t["k"], t["v"], o, lse, ws)
         binding.arachne_varlen_attn_bwd(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
+    warmup = max(warmup, 3)
+    for _ in range(warmup):
         step()
-    barrier()
+    env.barrier()
     plan.enable_profiling(True)
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
+    sampler = ClockSampler(env.local_rank)
+    if env.rank == 0:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    env.barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record()
-    barrier()
-    clocks = sampler.stop() if rank == 0 else None
-    ms_total = e0.elapsed_time(e1)
-    if world > 1:
-        tt = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
-    ms_step = ms_total / args.steps
-    value = world * flops / (ms_step * 1e-3) / 1e12
-    kt_f, calls_f = plan.kernel_times(False)
+    env.barrier()
+    clocks = sampler.stop() if env.rank == 0 else None
+    ms_total = env.max_over_ranks(e0.elapsed_time(e1))
+    ms_step = ms_total / steps
+    kt_f, _ = plan.kernel_times(False)
     kt_b, calls_b = plan.kernel_times(True)
     plan.enable_profiling(False)
-    launches = args.steps * (plan.num_launches(False) + plan.num_launches(True))
+    r = dict(workload=workload, st=st, flops=flops, ms_step=ms_step, ms_total=ms_total, steps=steps, warmup=warmup,
+             value=env.world * flops / (ms_step * 1e-3) / 1e12, kt_f=kt_f, kt_b=kt_b, calls_b=calls_b, clocks=clocks,
+             plan_ms=plan_ms, launches=steps * (plan.num_launches(False) + plan.num_launches(True)),
+             tensor_mb=t["q"].numel() * 2 / 1e6, deterministic=deterministic)
+    cta_balance = None
+    if env.rank == 0:
+        # per-CTA finish times of the last launch of the two persistent kernels (arachne_plan_cta_times): what the plan's LPT
+        # order + dynamic hand-out leaves of the sequence-length skew.  max / mean of the CTA end times; 1.0 = balanced.
+        try:
+            cta_balance = {}
+            for name, is_bwd in (("fwd_kernel", False), ("bwd_fused_kernel", True)):
+                if is_bwd and deterministic and not plan.deterministic_is_fused():
+                    continue
+                _, end_us = plan.cta_times(is_bwd)
+                cta_balance[name] = {"ctas": len(end_us), "end_max_us": max(end_us), "end_mean_us": sum(end_us) / len(end_us),
+                                     "end_min_us": min(end_us), "max_over_mean": max(end_us) / (sum(end_us) / len(end_us))}
+        except Exception as ex:          # never fail the bench line over a diagnostic
+            cta_balance = {"error": str(ex)}
+    r["cta_balance"] = cta_balance
+    if keep:
+        r.update(plan=plan, t=t, ws=ws)
+    else:
+        plan.close()
+    return r
+
+
+def target_entry(r, peaks, target_pct=None):
+    e = {"tflops": round(r["value"], 1), "ms_per_step": round(r["ms_step"], 3), "steps": r["steps"],
+         "pct_of_measured_bf16_burst": round(100.0 * r["value"] / r["world"] / peaks["burst"], 2),
+         "sm_mhz": r["clocks"]["sm_mhz"] if r["clocks"] else None, "reasons": r["clocks"]["reasons"] if r["clocks"] else None,
+         "fwd_ms": round(sum(ms for _, ms in r["kt_f"]), 3), "bwd_ms": round(sum(ms for _, ms in r["kt_b"]), 3)}
+    if target_pct is not None:
+        e["north_star_target_pct_of_burst"] = target_pct
+        e["met"] = e["pct_of_measured_bf16_burst"] >= target_pct
+    return e
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="long720p", choices=WORKLOADS)
+    ap.add_argument("--impl", default="arachne", choices=["arachne", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-targets", action="store_true", help="skip the extra legs (heavytail, deterministic) of config.targets")
+    ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
+    ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC backward as the main measurement")
+    ap.add_argument("--heads", type=int, default=0, help="override the head count: the per-rank share of a Ulysses group of degree H/heads")
+    ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
+    ap.add_argument("--sp", default="none", choices=["none", "ulysses", "cp"],
+                    help="N > 1: strong scaling of ONE batch over the N GPUs with sequence parallelism (peer memory, fused All-to-All)")
+    ap.add_argument("--src-hash", action="store_true", help="print the kernel source hash (for profiles/r2_traffic.csv) and exit")
+    args = ap.parse_args()
+    if args.src_hash:
+        print(kernel_source_hash())
+        return
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sp != "none":
+        from paper_2607_01701_b200 import sp_bench
+        return sp_bench.run(args)
+
+    env = Env()
+    torch = env.torch
+    from paper_2607_01701_b200 import binding
+
+    # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
+    # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
+    r = time_workload(env, args.workload, args.steps, args.warmup, deterministic=args.deterministic, order=args.order,
+                      seed_offset=args.seed_offset, heads=args.heads, keep=True)
+    r["world"] = env.world
+    st, plan, t, flops = r["st"], r["plan"], r["t"], r["flops"]
+    s2 = flops / (14.0 * st["D"] * st["H"])
 
     # ---- e2e through the C-ABI host entry point (pinned host buffers; H2D/D2H inside the timed region)
     e2e = None
@@ -247,84 +338,102 @@ def main():
         hq, hk, hv, hdo = (x.cpu().pin_memory() for x in (t["q"], t["k"], t["v"], t["dO"]))
         ho, hdq, hdk, hdv = (torch.empty_like(hq).pin_memory() for _ in range(4))
         hlse = torch.empty((plan.H, plan.N), dtype=torch.float32).pin_memory()
-        del ws
+        r.pop("ws")
         torch.cuda.empty_cache()
-        binding.arachne_varlen_attn_fwd_bwd_host(plan, hq, hk, hv, hdo, ho, hlse, hdq, hdk, hdv)   # warm-up
-        barrier()
-        n_e2e = 2
-        t0 = time.perf_counter()
+        binding.arachne_varlen_attn_fwd_bwd_host(plan, hq, hk, hv, hdo, ho, hlse, hdq, hdk, hdv)   # warm-up (allocates the plan's device buffers)
+        env.barrier()
+        n_e2e = max(5, min(args.steps, 20))
+        dts = []
         for _ in range(n_e2e):
-            binding.arachne_varlen_attn_fwd_bwd_host(plan, hq, hk, hv, hdo, ho, hlse, hdq, hdk, hdv)
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            tt = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
-        e2e = {"value": world * flops / dt / 1e12, "unit": UNIT, "h2d_bytes_per_step": 4 * nb,
-               "d2h_bytes_per_step": 4 * nb + hlse.numel() * 4, "ms_per_step": dt * 1e3,
+            t0 = time.perf_counter()
+            binding.arachne_varlen_attn_fwd_bwd_host(plan, hq, hk, hv, hdo, ho, hlse, hdq, hdk, hdv)   # returns after its own sync
+            dts.append(time.perf_counter() - t0)
+        dts.sort()
+        dt = env.max_over_ranks(dts[len(dts) // 2])
+        e2e = {"value": env.world * flops / dt / 1e12, "unit": UNIT, "h2d_bytes_per_step": 4 * nb,
+               "d2h_bytes_per_step": 4 * nb + hlse.numel() * 4, "ms_per_step": dt * 1e3, "reps": n_e2e, "stat": "median",
+               "ms_min": dts[0] * 1e3, "ms_max": dts[-1] * 1e3,
                "api": "arachne_varlen_attn_fwd_bwd_host (pinned host buffers)"}
-
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        del hq, hk, hv, hdo, ho, hdq, hdk, hdv
 
     peaks = load_peaks()
+    # ---- both north_star targets (and the deterministic backward) in the same record
+    targets = None
+    if not args.no_targets and args.workload == "long720p" and not args.deterministic and not args.heads:
+        tc_main = {k: x.cpu() for k, x in t.items()} if (env.rank == 0 and not args.no_cpu_baseline) else None
+        for k in list(t):
+            del t[k]
+        plan_main_closed = True
+        plan.close()
+        torch.cuda.empty_cache()
+        targets = {"long720p": target_entry(r, peaks, 60.0)}
+        ht = time_workload(env, "heavytail", 5, 3); ht["world"] = env.world
+        targets["heavytail"] = target_entry(ht, peaks, 50.0)
+        torch.cuda.empty_cache()
+        det = time_workload(env, "long720p", 3, 3, deterministic=True); det["world"] = env.world
+        targets["long720p_deterministic"] = target_entry(det, peaks, 60.0)
+        torch.cuda.empty_cache()
+    else:
+        tc_main = {k: x.cpu() for k, x in t.items()} if (env.rank == 0 and not args.no_cpu_baseline) else None
+        plan_main_closed = False
+
+    if env.rank != 0:
+        if env.world > 1:
+            env.dist.destroy_process_group()
+        return
+
     # ---- roofline of the dominant kernel: dense contraction -> tensor roofline.
-    # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); fused backward kernel
+    # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); backward main kernel
     # 10*D*H*S2 (S, dP, dV, dK, dQ — the 5-GEMM backward convention).
     alg = {"fwd_kernel": 4.0, "bwd_main(fused 5-GEMM | det: dKdV pass)": 10.0}
-    kernels = [{"name": n, "ms": ms} for n, ms in kt_f + kt_b]
+    kernels = [{"name": n, "ms": ms} for n, ms in r["kt_f"] + r["kt_b"]]
     dom = max(kernels, key=lambda k_: k_["ms"])
     dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2
     achieved = dom_flops / (dom["ms"] * 1e-3) / 1e12 if dom["ms"] > 0 else 0.0
-    roofline = {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peaks["sustained"], "unit": "TFLOP/s",
-                "frac": achieved / peaks["sustained"], "traffic": NCU_TRAFFIC.get((args.workload, dom["name"])),
-                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r1b_ncu_720p.md)",
-                "peak_source": peaks["source"] + ", bf16_tflops_sustained (kernel timed inside a long step)",
-                "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": calls_b}
+    # Denominator by run length (B200_PROFILING.md): a timed region under a second runs at boost clocks -> the burst figure;
+    # a longer one settles under the 1 kW power cap -> the sustained figure.
+    long_run = r["ms_total"] >= 1000.0
+    peak_kind = "bf16_tflops_sustained (timed region %.1f s >= 1 s: power-capped clocks)" % (r["ms_total"] / 1e3) if long_run \
+        else "bf16_tflops burst (timed region %.2f s < 1 s: boost clocks)" % (r["ms_total"] / 1e3)
+    peak = peaks["sustained"] if long_run else peaks["burst"]
+    traffic, traffic_src = ncu_traffic(args.workload, dom["name"])
+    roofline = {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "frac_of_burst": achieved / peaks["burst"], "frac_of_sustained": achieved / peaks["sustained"],
+                "traffic": traffic, "traffic_unit": "bytes/launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                "traffic_source": traffic_src, "peak_source": peaks["source"] + ", " + peak_kind,
+                "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": r["calls_b"]}
 
     cpu = None
     if not args.no_cpu_baseline:
         from oracle import arachne_oracle as orc
         orc.build()
-        tc = {k: x.cpu() for k, x in t.items()}
         L_max = max(st["cu_seqlens"][i + 1] - st["cu_seqlens"][i] for i in range(len(st["grids"])))
         # ~10-20 s of oracle time: rows x 2 heads x L_max ~ 2e7 query-row x key products
-        v_, dt_, desc, cores = oracle_sample(st, tc, budget_rows=max(8, min(L_max, int(8.0e7 / L_max))), heads=2)
+        v_, dt_, desc, cores = oracle_sample(st, tc_main, budget_rows=max(8, min(L_max, int(8.0e7 / L_max))), heads=2)
         cpu = {"value": v_, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
 
-    # per-CTA finish times of the last launch of the two persistent kernels (arachne_plan_cta_times): what the plan's LPT
-    # assignment leaves of the sequence-length skew.  max / mean of the CTA end times; 1.0 = perfectly balanced.
-    cta_balance = None
-    if rank == 0:
-        try:
-            cta_balance = {}
-            for name, is_bwd in (("fwd_kernel", False), ("bwd_fused_kernel", True)):
-                if is_bwd and args.deterministic:
-                    continue
-                _, end_us = plan.cta_times(is_bwd)
-                cta_balance[name] = {"ctas": len(end_us), "end_max_us": max(end_us), "end_mean_us": sum(end_us) / len(end_us),
-                                     "end_min_us": min(end_us), "max_over_mean": max(end_us) / (sum(end_us) / len(end_us))}
-        except Exception as ex:          # never fail the bench line over a diagnostic
-            cta_balance = {"error": str(ex)}
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": env.world, "steps": args.steps, "warmup": r["warmup"],
+        "ms_per_step": r["ms_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "plan_create_ms": round(plan_ms, 3), "deterministic_bwd": bool(args.deterministic), "num_seqs": len(st["grids"]), "total_tokens": st["N"],
+        "config": {"workload": args.workload, "order": args.order, "seed_offset": args.seed_offset, "plan_create_ms": round(r["plan_ms"], 3),
+                   "deterministic_bwd": bool(args.deterministic), "num_seqs": len(st["grids"]), "total_tokens": st["N"],
                    "heads": st["H"], "head_dim": st["D"], "flop_per_step": flops,
-                   "l2": "inputs larger than L2 (4 x %.0f MB bf16 tensors + tiled workspace)" % (t["q"].numel() * 2 / 1e6),
-                   "pct_of_measured_bf16_burst": 100.0 * value / world / peaks["burst"],
-                   "pct_of_measured_bf16_sustained": 100.0 * value / world / peaks["sustained"],
-                   "pct_of_nominal_2250": 100.0 * value / world / 2250.0,
-                   "fwd_ms": sum(ms for _, ms in kt_f), "bwd_ms": sum(ms for _, ms in kt_b)},
-        "cta_balance": cta_balance, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+                   "operands": "Q^,K^ fp16 (fwd and bwd recompute), dS fp16 x 2^k, P,V,dO bf16, fp32 accumulate",
+                   "l2": "inputs larger than L2 (4 x %.0f MB bf16 tensors + tiled workspace)" % r["tensor_mb"],
+                   "pct_of_measured_bf16_burst": 100.0 * r["value"] / env.world / peaks["burst"],
+                   "pct_of_measured_bf16_sustained": 100.0 * r["value"] / env.world / peaks["sustained"],
+                   "pct_of_nominal_2250": 100.0 * r["value"] / env.world / 2250.0,
+                   "fwd_ms": sum(ms for _, ms in r["kt_f"]), "bwd_ms": sum(ms for _, ms in r["kt_b"]),
+                   "targets": targets},
+        "cta_balance": r["cta_balance"], "clocks": r["clocks"], "e2e": e2e, "gpu_launches": r["launches"], "roofline": roofline,
+        "cpu_baseline": cpu,
     }
     print(json.dumps(out))
-    if world > 1:
-        dist.destroy_process_group()
+    if not plan_main_closed:
+        plan.close()
+    if env.world > 1:
+        env.dist.destroy_process_group()
 
 
 if __name__ == "__main__":

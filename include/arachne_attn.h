@@ -57,14 +57,33 @@ typedef enum {
   ARACHNE_ERR_CUDA = 10,             /* CUDA runtime error; text in arachne_last_error_message */
   ARACHNE_ERR_BAD_SHAPE = 11,        /* num_seqs/num_heads/total_tokens <= 0, or too large  */
   ARACHNE_ERR_BAD_PARAM = 12,        /* non-finite / non-positive theta, eps < 0, bad flags */
-  ARACHNE_ERR_BAD_SHARDING = 13      /* see arachne_plan_create_sharded; or a sharded plan passed to a plain call */
+  ARACHNE_ERR_BAD_SHARDING = 13,     /* see arachne_plan_create_sharded; or a sharded plan passed to a plain call */
+  ARACHNE_ERR_LOGIT_RANGE = 14       /* tau > 1 without ARACHNE_FLAG_WIDE_LOGITS: see "Verified envelope" below      */
 } arachne_status;
 
 enum {
   ARACHNE_FLAG_DETERMINISTIC = 1,    /* bwd: bit-reproducible run to run (same device, plan) */
   ARACHNE_FLAG_NO_NORM = 2,          /* debug: skip RMSNorm (x^ = x)                         */
-  ARACHNE_FLAG_NO_ROPE = 4           /* debug: skip RoPE (x~ = x^)                           */
+  ARACHNE_FLAG_NO_ROPE = 4,          /* debug: skip RoPE (x~ = x^)                           */
+  ARACHNE_FLAG_WIDE_LOGITS = 8       /* the caller accepts logits outside the verified envelope (below) */
 };
+
+/* Verified envelope (reading R19).  Q^ and K^ enter the tensor cores as fp16 — the most precise 16-bit
+ * operand format, legal because RMSNorm bounds |x^_d| <= |gamma|inf * sqrt(D) — in the forward and, bit for bit the
+ * same images, in the backward's recompute of S.  The rounding error of a logit is proportional to its size:
+ * |delta s_ij| <= 2^-10 * beta with beta = softmax_scale * D * |gamma_q|inf * |gamma_k|inf the logit bound, and LSE
+ * inherits it without averaging once the softmax is peaked.  Let
+ *     tau = softmax_scale * sqrt(D) * |gamma_q|inf * |gamma_k|inf        (= 1 for every BASELINE.json config).
+ * BASELINE.json's tolerances (O rel-L2 <= 1e-2, max-abs <= 2e-2, LSE max-abs <= 1e-3, dQ/dK/dV rel-L2 <= 2e-2) are
+ * claimed for tau <= 1.  For tau > 1 the O and gradient tolerances still hold as far as they have been measured
+ * (tau = 9: gamma_q = gamma_k = 3, tests/test_gpu_parity.py), but LSE is only bounded by 2^-10 * beta (measured
+ * max-abs: 5e-4..1.2e-3 at tau = 1.6, 3e-3 at tau = 4, 9e-3 at tau = 9).  Because this is a precision limit and not a
+ * failure, it is reported instead of hidden:
+ *   - arachne_plan_create* returns ARACHNE_ERR_LOGIT_RANGE when softmax_scale * sqrt(D) > 1 (known on the host) unless
+ *     ARACHNE_FLAG_WIDE_LOGITS (or the debug flag NO_NORM, whose logits are unbounded anyway) is set;
+ *   - gamma lives in device memory, so |gamma|inf is only known to the kernels: a forward launched WITHOUT the flag whose
+ *     tau exceeds 1 still runs, and leaves a sticky mark in the plan that arachne_plan_logit_status returns.
+ * Callers with learned QK-norm weights either set the flag (accepting the LSE bound above) or poll the status. */
 
 /* Problem description.  Plain data, copied by arachne_plan_create. */
 typedef struct {
@@ -81,7 +100,19 @@ typedef struct {
   int32_t flags;          /* ARACHNE_FLAG_*                                                */
 } arachne_attn_params;
 
+/* The tensors are CONTIGUOUS [N, H, D]: SURVEY §8(b) sketched optional q/k/v token and head strides; they are not part of
+ * this ABI because every raw row is read exactly once by the in-call prologue (prep_kernel), so a strided caller loses
+ * nothing by making the tensors contiguous first, and the sharded entry points below already cover the one strided
+ * layout the method needs (a head range of a wider [n, total_heads, D] tensor). */
+
 typedef struct arachne_plan arachne_plan;
+
+/* A plan is IMMUTABLE schedule data (work lists, token tables, RoPE tables) plus three pieces of mutable state that the
+ * hot path touches: (1) the sticky envelope word written by out-of-envelope forwards (arachne_plan_logit_status), (2) the
+ * per-CTA trace of the last launch (arachne_plan_cta_times) and (3), only while arachne_plan_enable_profiling is on, the
+ * timing events.  Everything a launch needs to mutate (dynamic work counters, logit bound, dS scaling tables) lives in the
+ * header of the CALLER'S workspace, so one plan may serve concurrent calls on different streams provided each call has
+ * its own workspace (and profiling is off); the *_host calls keep per-plan device buffers and are not re-entrant. */
 
 /* Build the reusable schedule for one packing (a DiT cascade runs ~60 layers x
  * (2 fwd + 1 bwd) on the same packing).  Validates everything,
@@ -132,18 +163,27 @@ void arachne_plan_destroy(arachne_plan* plan);
  * Returns 0 if plan is NULL or pass is invalid. */
 size_t arachne_workspace_bytes(const arachne_plan* plan, int pass);
 
-/* Number of kernels one call enqueues (for launch accounting). pass: 0 = fwd, 1 = bwd. */
+/* Number of kernels one arachne_varlen_attn_fwd (pass 0) / arachne_varlen_attn_bwd (pass 1) call enqueues, for launch
+ * accounting: fwd 2; bwd 4 (prep, bwd_scale, fused main, post) or 5 with ARACHNE_FLAG_DETERMINISTIC (two main passes);
+ * the _dgamma form adds one. */
 int arachne_num_launches(const arachne_plan* plan, int pass);
 
-/* Name of kernel `idx` (0-based, launch order) of a pass; "" if out of range. */
+/* Name of TIMED INTERVAL `idx` (0-based, launch order) of a pass — the unit arachne_plan_kernel_times reports: fwd has 2
+ * (prep_kernel, fwd_kernel), bwd has 4 (prep + bwd_scale, main kernel, second main pass [deterministic only, else 0 ms],
+ * post [+ dgamma reduce]); "" if out of range. */
 const char* arachne_kernel_name(int pass, int idx);
+
+/* Sticky envelope status of a plan ("Verified envelope" above).  ARACHNE_OK if no forward launched on this plan without
+ * ARACHNE_FLAG_WIDE_LOGITS has seen tau > 1; else ARACHNE_ERR_LOGIT_RANGE and *tau_seen (nullable) = the largest tau.
+ * Synchronous (cudaMemcpy of 4 bytes): call it after the stream has been synchronised. */
+int arachne_plan_logit_status(const arachne_plan* plan, float* tau_seen);
 
 /* Per-kernel device timing for benchmarks (bench.py's roofline figure).  When enabled, fwd/bwd
  * record a CUDA event before the first and after every kernel on the caller's stream (no
  * synchronisation is added); the plan keeps the events of the last 32 calls per pass.
  * arachne_plan_kernel_times synchronises on those events and writes to ms_sum[i] the SUM over
- * the recorded calls of kernel i's duration in milliseconds (ms_sum has n_kernels >=
- * arachne_num_launches entries) and the number of calls to *n_calls.  Enabling resets the ring.
+ * the recorded calls of timed interval i's duration in milliseconds (ms_sum has n_kernels >= 2 (fwd) / 4 (bwd)
+ * entries, see arachne_kernel_name) and the number of calls to *n_calls.  Enabling resets the ring.
  * Not thread-safe with concurrent fwd/bwd on the same plan. */
 int arachne_plan_enable_profiling(arachne_plan* plan, int enable);
 int arachne_plan_kernel_times(const arachne_plan* plan, int pass, float* ms_sum, int n_kernels, int* n_calls);

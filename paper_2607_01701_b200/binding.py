@@ -18,7 +18,8 @@ if not os.path.exists(_LIB_PATH):
         "(nvcc, sm_100a). There is no CPU fallback.")
 _lib = ctypes.CDLL(_LIB_PATH)
 
-FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE = 1, 2, 4
+FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE, FLAG_WIDE_LOGITS = 1, 2, 4, 8
+ERR_LOGIT_RANGE = 14
 
 EXPORTS = [
     "arachne_plan_create", "arachne_plan_destroy", "arachne_workspace_bytes", "arachne_num_launches",
@@ -29,6 +30,7 @@ EXPORTS = [
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
     "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
     "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free", "arachne_plan_cta_times",
+    "arachne_plan_logit_status",
 ]
 
 
@@ -105,6 +107,10 @@ _lib.arachne_plan_cta_times.argtypes = [_vp, ctypes.c_int, ctypes.POINTER(ctypes
                                         ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
 
 
+_lib.arachne_plan_logit_status.restype = ctypes.c_int
+_lib.arachne_plan_logit_status.argtypes = [_vp, ctypes.POINTER(ctypes.c_float)]
+
+
 class ArachneError(RuntimeError):
     def __init__(self, status: int):
         self.status = status
@@ -177,9 +183,18 @@ class Plan:
     def enable_profiling(self, enable=True):
         _check(_lib.arachne_plan_enable_profiling(self._h, 1 if enable else 0))
 
+    def deterministic_is_fused(self) -> bool:
+        """True when ARACHNE_FLAG_DETERMINISTIC runs bwd_fused_kernel with the ordered dQ~ reduction (5 launches -> 4)."""
+        return self.num_launches(True) == 4
+
+    def logit_status(self):
+        """(status, tau): arachne_plan_logit_status — ERR_LOGIT_RANGE once a forward without FLAG_WIDE_LOGITS saw tau > 1."""
+        tau = ctypes.c_float(0.0)
+        return int(_lib.arachne_plan_logit_status(self._h, ctypes.byref(tau))), float(tau.value)
+
     def kernel_times(self, bwd: bool):
-        """[(kernel name, mean ms per call)] over the calls recorded since enable_profiling()."""
-        n = self.num_launches(bwd)
+        """[(timed interval name, mean ms per call)] over the calls recorded since enable_profiling()."""
+        n = 4 if bwd else 2
         ms = (ctypes.c_float * n)()
         calls = ctypes.c_int(0)
         _check(_lib.arachne_plan_kernel_times(self._h, 1 if bwd else 0, ms, n, ctypes.byref(calls)))

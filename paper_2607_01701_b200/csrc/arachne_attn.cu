@@ -54,7 +54,10 @@ struct arachne_plan {
   mutable struct arachne_host_ctx* host = nullptr;   // lazily created by the *_host calls (device buffers, streams)
   int cp_rank = -1;   // >= 0: context-parallel plan (arachne_plan_create_cp), this process owns the queries of shard cp_rank
   Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
-  int q_rot = 0;   // fused backward: query-tile rotation per key tile (ARACHNE_BWD_QROT env, tuning)
+  int n_groups = 0;        // num_seqs * num_heads: (sequence, head) groups (dS scaling tables in the workspace header)
+  size_t hdr_bytes = 0;    // WsHeader + group tables at the start of every workspace
+  unsigned* d_envelope = nullptr;   // sticky: float bits of the largest out-of-envelope logit bound seen (arachne_plan_logit_status)
+  float bound_limit = 0.f; // forward: logit bound (log2 units) above which a launch without ARACHNE_FLAG_WIDE_LOGITS is flagged
   // device arrays (owned)
   SeqInfo* d_seqs = nullptr;
   int* d_tile_seq = nullptr;
@@ -65,7 +68,6 @@ struct arachne_plan {
   int* d_item_ptr = nullptr;
   int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
-  unsigned* d_stats = nullptr;
   unsigned long long* d_cta_trace = nullptr;   // [2][kTraceMaxCtas][2] globaltimer ns (arachne_plan_cta_times)
   float2* d_rope = nullptr;
   ProblemDesc pd{};
@@ -99,8 +101,23 @@ int configure_kernels() {
 struct FwdWs { uint8_t *qt, *kt, *vt; };
 struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
 
-size_t fwd_ws_bytes(const arachne_plan* pl) { return 3 * pl->img_bytes; }
-size_t bwd_ws_bytes(const arachne_plan* pl) { return 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
+size_t fwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + 3 * pl->img_bytes; }
+size_t bwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
+
+// The first hdr_bytes of every workspace hold the per-call mutable words of the kernels (WsHeader: logit bound, dynamic
+// work counters) and, for the backward, the per-(sequence, head) dS-scaling tables: the plan itself carries no per-launch
+// state, so concurrent calls on one plan are safe as long as each has its own workspace.
+ProblemDesc per_call_desc(const arachne_plan* pl, void* ws) {
+  ProblemDesc pd = pl->pd;
+  uint8_t* w = static_cast<uint8_t*>(ws);
+  WsHeader* hdr = reinterpret_cast<WsHeader*>(w);
+  pd.stats = hdr->qk_bound;
+  pd.work_counter = hdr->work_counter;
+  pd.dq_error = &hdr->dq_error;
+  pd.grp_stats = reinterpret_cast<unsigned*>(w + sizeof(WsHeader));
+  pd.grp_sk = reinterpret_cast<float*>(w + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16);
+  return pd;
+}
 
 inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st) {
   if (!pl->profiling) return;
@@ -111,23 +128,23 @@ inline void prof_mark(const arachne_plan* pl, int pass, int idx, cudaStream_t st
 template <int D>
 int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k, const ShardedPtr& v, const float* gq,
                const float* gk, const ShardedPtr& o, float* lse, void* ws, cudaStream_t st) {
-  uint8_t* w = static_cast<uint8_t*>(ws);
+  uint8_t* w = static_cast<uint8_t*>(ws) + pl->hdr_bytes;
   FwdWs f{w, w + pl->img_bytes, w + 2 * pl->img_bytes};
+  const ProblemDesc pd = per_call_desc(pl, ws);
   PrepParams pp{};
   pp.q = q; pp.k = k; pp.v = v;
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
-  pp.out_fmt = FMT_F16;
   pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // S leaves the tensor core in the exp2 domain
-  pp.stats = pl->d_stats;
+  pp.stats = pd.stats;
   prof_mark(pl, 0, 0, st);
-  ARACHNE_CUDA(cudaMemsetAsync(pl->d_stats, 0, 4 * sizeof(unsigned), st));
-  prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
+  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader), st));
+  prep_kernel<D, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
-  FwdParams fp{f.qt, f.kt, f.vt, o, lse};
+  FwdParams fp{f.qt, f.kt, f.vt, o, lse, pl->d_envelope, pl->bound_limit};
   const int grid = pl->n_fwd_ctas;
-  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pl->pd, fp);   // (a CP rank may own no queries)
+  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp);   // (a CP rank may own no queries)
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
   if (pl->profiling) pl->prof_calls[0]++;
@@ -142,7 +159,8 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   // cp_gk / cp_gv (context parallelism, phase 1): dk~ and dV leave as fp32 PARTIALS in these [N,H,D] buffers, only dQ is
   // finished here (for this rank's query rows); arachne_cp_reduce finishes dK, dV.
   const bool cp = cp_gk != nullptr;
-  uint8_t* w = static_cast<uint8_t*>(ws);
+  uint8_t* w = static_cast<uint8_t*>(ws) + pl->hdr_bytes;
+  const ProblemDesc pd = per_call_desc(pl, ws);
   BwdWs b{};
   b.qt = w; w += pl->img_bytes;
   b.kt = w; w += pl->img_bytes;
@@ -156,37 +174,38 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   if (cp) b.gk_t = cp_gk;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
   PrepParams pp{};
-  pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse; pp.backward = 1;
+  pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse;
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
-  pp.out_fmt = FMT_BF16;
-  pp.q_prescale = 1.0f;
+  pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // the forward's operand images, bit for bit
   pp.gq_zero = deterministic ? nullptr : b.gq_t;
   prof_mark(pl, 1, 0, st);
-  ARACHNE_CUDA(cudaMemsetAsync(pl->d_stats + 3, 0, sizeof(unsigned), st));       // bwd_fused_kernel's work counter
-  prep_kernel<D><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pl->pd, pp);
+  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16, st));   // header + group maxima
+  prep_kernel<D, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
+  ARACHNE_CUDA(cudaGetLastError());
+  bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
   const int grid = pl->n_ctas;
   if (deterministic) {
     // two-pass (7 GEMM) path: every output tile owned by one CTA, fixed summation order
     BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv};
-    bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 1);
+    bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pd, bp, 1);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
-    bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pl->pd, bp, 2);
+    bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pd, bp, 2);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 3, st);
   } else {
     // fused single-pass (5 GEMM) path: dQ~ partial tiles reduce-added at L2 (order not fixed)
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, pl->q_rot};
-    if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pl->pd, bp);
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv};
+    if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
     prof_mark(pl, 1, 3, st);
   }
   PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
-  post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pl->pd, po);
+  post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
     dgamma_reduce_kernel<D><<<2, 256, 0, st>>>(dgpart, pl->post_blocks, dgq, dgk);
@@ -217,6 +236,7 @@ const char* arachne_status_string(int s) {
     case ARACHNE_ERR_BAD_SHAPE: return "bad shape";
     case ARACHNE_ERR_BAD_PARAM: return "bad parameter";
     case ARACHNE_ERR_BAD_SHARDING: return "bad sharding (1..8 shards, starts 0..N non-decreasing, head_offset + num_heads <= total_heads)";
+    case ARACHNE_ERR_LOGIT_RANGE: return "logit range outside the verified envelope (softmax_scale*sqrt(D)*|gamma_q|inf*|gamma_k|inf > 1): pass ARACHNE_FLAG_WIDE_LOGITS";
     default: return "unknown status";
   }
 }
@@ -272,8 +292,14 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
   if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
-      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~7))
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~15))
     return ARACHNE_ERR_BAD_PARAM;
+  {
+    // envelope (reading R19): an explicit softmax_scale above 1/sqrt(D) widens the logits beyond what the gates are claimed for
+    const float sc = p.softmax_scale == 0.f ? 1.0f / std::sqrt(static_cast<float>(p.head_dim)) : p.softmax_scale;
+    if (sc * std::sqrt(static_cast<float>(p.head_dim)) > 1.0001f && !(p.flags & (ARACHNE_FLAG_WIDE_LOGITS | ARACHNE_FLAG_NO_NORM)))
+      return ARACHNE_ERR_LOGIT_RANGE;
+  }
   if (cu[0] != 0) return ARACHNE_ERR_BAD_CU_SEQLENS;
   for (int b = 0; b < p.num_seqs; ++b)
     if (cu[b + 1] <= cu[b]) return ARACHNE_ERR_BAD_CU_SEQLENS;          // R16: L_b >= 1
@@ -413,8 +439,8 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   PLAN_UP(pl->d_item_ptr, item_ptr, int)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
-  if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_stats), 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
-  if ((e = cudaMemset(pl->d_stats, 0, 4 * sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
+  if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_envelope), sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
+  if ((e = cudaMemset(pl->d_envelope, 0, sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
   if (pl->num_sms <= kTraceMaxCtas) {
     if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
     if ((e = cudaMemset(pl->d_cta_trace, 0, 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
@@ -424,7 +450,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.stats = pl->d_stats; pd.cta_trace = pl->d_cta_trace; pd.work_counter = reinterpret_cast<int*>(pl->d_stats + 2);
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.cta_trace = pl->d_cta_trace;   // stats, counters, group tables: per call (per_call_desc)
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -450,7 +476,14 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     pl->post_blocks = static_cast<int>(std::min<long long>((rows + rpb - 1) / rpb, static_cast<long long>(pl->num_sms) * 8));
     pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
   }
-  if (const char* e = std::getenv("ARACHNE_BWD_QROT")) pl->q_rot = std::atoi(e);
+  pl->n_groups = p.num_seqs * p.num_heads;
+  pl->hdr_bytes = align_up(sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * (16 + 8), 1024);
+  {
+    // Envelope (reading R19): north_star's gates are claimed for tau = softmax_scale*sqrt(D)*|gamma_q|inf*|gamma_k|inf
+    // <= 1 (every BASELINE.json config has tau = 1).  The forward's logit bound in log2 units is tau*sqrt(D)*log2(e).
+    const bool wide = (p.flags & (ARACHNE_FLAG_WIDE_LOGITS | ARACHNE_FLAG_NO_NORM)) != 0;
+    pl->bound_limit = wide ? INFINITY : 1.001f * std::sqrt(static_cast<float>(p.head_dim)) * 1.4426950408889634f;
+  }
   *out = pl;
   return ARACHNE_OK;
 }
@@ -463,7 +496,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_stats); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_envelope); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
   delete pl;
 }
 
@@ -476,12 +509,17 @@ size_t arachne_workspace_bytes(const arachne_plan* pl, int pass) {
 
 int arachne_num_launches(const arachne_plan* pl, int pass) {
   if (!pl) return 0;
-  return pass == 0 ? 2 : (pass == 1 ? 4 : 0);
+  if (pass == 0) return 2;                                              // prep_kernel, fwd_kernel
+  if (pass == 1) return (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) ? 5  // prep, bwd_scale, dK/dV pass, dQ pass, post
+                                                                   : 4; // prep, bwd_scale, bwd_fused, post
+  return 0;
 }
+
+static int num_timed_intervals(int pass) { return pass == 0 ? 2 : (pass == 1 ? 4 : 0); }
 
 const char* arachne_kernel_name(int pass, int idx) {
   static const char* fwd[] = {"prep_kernel(fwd: RMSNorm+RoPE -> fp16 tiles)", "fwd_kernel"};
-  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> bf16 tiles, delta)", "bwd_main(fused 5-GEMM | det: dKdV pass)",
+  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> fp16 tiles, delta) + bwd_scale_kernel", "bwd_main(fused 5-GEMM | det: dKdV pass)",
                               "bwd_second(det only: dQ pass)", "post_kernel(un-RoPE + RMSNorm bwd)"};
   if (pass == 0 && idx >= 0 && idx < 2) return fwd[idx];
   if (pass == 1 && idx >= 0 && idx < 4) return bwd[idx];
@@ -503,6 +541,18 @@ int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us,
   return ARACHNE_OK;
 }
 
+int arachne_plan_logit_status(const arachne_plan* pl, float* tau_seen) {
+  if (!pl) return ARACHNE_ERR_NULL_POINTER;
+  unsigned bits = 0;
+  ARACHNE_CUDA(cudaMemcpy(&bits, pl->d_envelope, sizeof(bits), cudaMemcpyDeviceToHost));
+  float bound;
+  std::memcpy(&bound, &bits, sizeof(bound));
+  // the kernel records the logit bound in log2 units: tau * sqrt(D) * log2(e)
+  const float tau = bound / (std::sqrt(static_cast<float>(pl->p.head_dim)) * 1.4426950408889634f);
+  if (tau_seen) *tau_seen = bits ? tau : 0.f;
+  return bits ? ARACHNE_ERR_LOGIT_RANGE : ARACHNE_OK;
+}
+
 int arachne_plan_enable_profiling(arachne_plan* pl, int enable) {
   if (!pl) return ARACHNE_ERR_NULL_POINTER;
   if (enable && !pl->prof_ev[0][0][0]) {
@@ -518,7 +568,7 @@ int arachne_plan_enable_profiling(arachne_plan* pl, int enable) {
 int arachne_plan_kernel_times(const arachne_plan* pl, int pass, float* ms_sum, int n_kernels, int* n_calls) {
   if (!pl || !ms_sum || !n_calls) return ARACHNE_ERR_NULL_POINTER;
   if (pass < 0 || pass > 1 || !pl->profiling) return ARACHNE_ERR_BAD_PARAM;
-  const int nk = arachne_num_launches(pl, pass);
+  const int nk = num_timed_intervals(pass);
   if (n_kernels < nk) return ARACHNE_ERR_BAD_PARAM;
   const long long calls = std::min<long long>(pl->prof_calls[pass], arachne_plan::kProfSlots);
   for (int i = 0; i < nk; ++i) ms_sum[i] = 0.f;
@@ -650,7 +700,7 @@ template <int D>
 int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const ShardedPtr& gvp, const ShardedPtr& k, const float* gk,
                      const ShardedPtr& dk, const ShardedPtr& dv, float* dgk, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
-  w += 4 * pl->img_bytes + 2 * pl->rowvec_bytes;                 // same carving as launch_bwd: gk_t, gq_t, dgamma partials
+  w += pl->hdr_bytes + 4 * pl->img_bytes + 2 * pl->rowvec_bytes;   // same carving as launch_bwd: gk_t, gq_t, dgamma partials
   float* gk_sum = reinterpret_cast<float*>(w); w += pl->grad_bytes + pl->gradblk_bytes;
   float* dgpart = dgk ? reinterpret_cast<float*>(w) : nullptr;
   const int lo = pl->pd.cp_lo, hi = pl->pd.cp_hi;

@@ -10,7 +10,7 @@
 //       dV  += P^T dO_sub       dK~ += dS^T Q^_sub         (A operand = P^T / dS^T in TMEM)
 //   kIsDQ = true   (dQ pass, QUERY tile stationary):     X1 = Q^, X2 = dO ; stream Y1 = K^, Y2 = V
 //       S    = Q^ K^_sub^T      dP   = dO V_sub^T         [128 queries x 64 keys] each
-//       dS   = exp2(S c - lse2[row]) * (dP - delta[row])
+//       dS   = exp2(S - lse2[row]) * (dP - delta[row]) * sk
 //       dQ~ += dS K^_sub
 //
 // The streamed 128-row tile is consumed in two 64-row halves so that S and dP can be double
@@ -27,8 +27,8 @@
 namespace arachne {
 
 struct BwdParams {
-  const uint8_t* qt;       // Q^ bf16 images   [H][n_tiles][TILE]
-  const uint8_t* kt;       // K^ bf16 images
+  const uint8_t* qt;       // Q^' fp16 images (q~ * softmax_scale * log2e)   [H][n_tiles][TILE]
+  const uint8_t* kt;       // K^ fp16 images
   const uint8_t* vt;       // V  bf16 images
   const uint8_t* dot;      // dO bf16 images
   const float* lse2_t;     // [H][n_tiles][128]  lse*log2e, +inf on pad rows
@@ -87,7 +87,6 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
   __syncthreads();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
-  const float scale_log2 = pd.softmax_scale * 1.4426950408889634f;
   const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
   const uint8_t* gX1 = kIsDQ ? bp.qt : bp.kt;
   const uint8_t* gX2 = kIsDQ ? bp.dot : bp.vt;
@@ -126,8 +125,11 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
     // ------------------------------------------------------------------ MMA issuer (whole warp convergent,
     // one elected lane issues: keeps descriptors in uniform registers, no per-instruction election loop)
     {
-      constexpr uint32_t idesc_sdp = make_idesc(128, 64, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
-      constexpr uint32_t idesc_acc = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+      // S from the forward's fp16 Q^', K^ images; dS fp16 (scaled by the group's sk); P, V, dO bf16
+      constexpr uint32_t idesc_s = make_idesc(128, 64, FMT_F16, FMT_F16, MAJOR_K, MAJOR_K);
+      constexpr uint32_t idesc_dp = make_idesc(128, 64, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
+      constexpr uint32_t idesc_pv = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+      constexpr uint32_t idesc_ds = make_idesc(128, D, FMT_F16, FMT_F16, MAJOR_K, MAJOR_MN);
       const uint32_t aX1 = smem_u32(sX1), aX2 = smem_u32(sX2), aY1 = smem_u32(sY1), aY2 = smem_u32(sY2);
       const uint32_t tAcc0 = tbase + Cfg::kColAcc0, tAcc1 = tbase + Cfg::kColAcc1;
       uint32_t it = 0, yt = 0, g = 0;
@@ -141,12 +143,12 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
-          umma_ss(tS, make_sdesc(aX1 + koff, 16, 1024), make_sdesc(aY1 + yb + koff, 16, 1024), idesc_sdp, kk > 0);
+          umma_ss(tS, make_sdesc(aX1 + koff, 16, 1024), make_sdesc(aY1 + yb + koff, 16, 1024), idesc_s, kk > 0);
         }
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
-          umma_ss(tdP, make_sdesc(aX2 + koff, 16, 1024), make_sdesc(aY2 + yb + koff, 16, 1024), idesc_sdp, kk > 0);
+          umma_ss(tdP, make_sdesc(aX2 + koff, 16, 1024), make_sdesc(aY2 + yb + koff, 16, 1024), idesc_dp, kk > 0);
         }
         umma_commit(&sdp_full[gg & 1]);
         }
@@ -172,10 +174,10 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
             const uint32_t roff = st * TILE + (u * 64 + kk * 16) * 128;     // K rows of the MN-major B operand
             const uint32_t acc = (s > 0 || kk > 0) ? 1u : 0u;
             if (!kIsDQ) {
-              umma_ts(tAcc0, tP + kk * 8, make_sdesc(aY2 + roff, BLK, 1024), idesc_acc, acc);    // dV += P^T dO
-              umma_ts(tAcc1, tdS + kk * 8, make_sdesc(aY1 + roff, BLK, 1024), idesc_acc, acc);   // dK~ += dS^T Q^
+              umma_ts(tAcc0, tP + kk * 8, make_sdesc(aY2 + roff, BLK, 1024), idesc_pv, acc);    // dV += P^T dO
+              umma_ts(tAcc1, tdS + kk * 8, make_sdesc(aY1 + roff, BLK, 1024), idesc_ds, acc);   // dK~ += dS^T Q^'
             } else {
-              umma_ts(tAcc0, tdS + kk * 8, make_sdesc(aY1 + roff, BLK, 1024), idesc_acc, acc);   // dQ~ += dS K^
+              umma_ts(tAcc0, tdS + kk * 8, make_sdesc(aY1 + roff, BLK, 1024), idesc_ds, acc);   // dQ~ += dS K^
             }
           }
           if (u == 1) umma_commit(&y_empty[st]);
@@ -197,6 +199,8 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
       const WorkItem wi = pd.items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       const uint32_t G = 2u * sq.n_tiles;
+      const float2 skv = *reinterpret_cast<const float2*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2);
+      const float sk = skv.x;                    // dS is rounded to fp16 as dS * sk (delta already carries sk: bwd_scale_kernel)
       float lse2_r = 0.f, delta_r = 0.f;
       if (kIsDQ) {
         const size_t roff = (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + wi.tile) * kTileRows + row;
@@ -227,12 +231,12 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
               const float2 dv2 = *reinterpret_cast<const float2*>(&sDelta[st * 128 + col]);
               l0 = lv.x; l1 = lv.y; d0 = dv2.x; d1 = dv2.y;
             }
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c]), scale_log2, -l0));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), scale_log2, -l1));
-            const float ds0 = p0 * (__uint_as_float(dpv[c]) - d0);
-            const float ds1 = p1 * (__uint_as_float(dpv[c + 1]) - d1);
+            const float p0 = ex2_approx(__uint_as_float(sv[c]) - l0);        // S is already in the exp2 domain (Q^')
+            const float p1 = ex2_approx(__uint_as_float(sv[c + 1]) - l1);
+            const float ds0 = p0 * fmaf(__uint_as_float(dpv[c]), sk, -d0);
+            const float ds1 = p1 * fmaf(__uint_as_float(dpv[c + 1]), sk, -d1);
             pp[c >> 1] = pack_bf16x2(p0, p1);
-            dd[c >> 1] = pack_bf16x2(ds0, ds1);
+            dd[c >> 1] = pack_f16x2(ds0, ds1);
           }
           if (!kIsDQ) tmem_st16(tS + half * 16, pp);
           tmem_st16(tdP + half * 16, dd);
@@ -248,7 +252,8 @@ __global__ void __launch_bounds__(192, 1) bwd_kernel(ProblemDesc pd, BwdParams b
       const bool valid_row = n < sq.len;
       const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
       const uint32_t tA0 = tbase + Cfg::kColAcc0 + lane_base, tA1 = tbase + Cfg::kColAcc1 + lane_base;
-      const float sc = pd.softmax_scale;
+      // dq~ = scale * dS k~;  dk~ = scale * dS^T q~ = ln2 * dS^T Q^';  dS carries sk
+      const float sc = (kIsDQ ? pd.softmax_scale : 0.6931471805599453f) * skv.y;
       __nv_bfloat16* dv_row = valid_row ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
       float* gout = (kIsDQ ? bp.gq_t : bp.gk_t) + out_off;
 #pragma unroll

@@ -11,8 +11,8 @@
 //
 //   S^T  = K^  Q^_i^T        SS   [128 keys x 128 queries] fp32 -> TMEM cols [0,128)
 //   dP^T = V   dO_i^T        SS                                  -> TMEM cols [128,256)
-//   P^T  = exp2(S^T c - lse2[query])            bf16, written back over S^T (A operand of dV)
-//   dS^T = P^T * (dP^T - delta[query])          bf16, written to shared memory (one tile image)
+//   P^T  = exp2(S^T - lse2[query])              bf16, written back over S^T (A operand of dV)
+//   dS^T = P^T * (dP^T - delta[query]) * sk     fp16, written to shared memory (one tile image); sk: prep.cuh
 //   dV  += P^T  dO_i         TS   acc TMEM cols [256,256+D)
 //   dK~ += dS^T Q^_i         SS   acc TMEM cols [256+D,256+2D)   (A = dS^T image, K-major)
 //   dQ~_i = dS  K^           SS   -> TMEM cols [128,256) (aliases dP^T) (A = dS^T image, MN-major)
@@ -32,8 +32,8 @@
 namespace arachne {
 
 struct BwdFusedParams {
-  const uint8_t* qt;       // Q^ bf16 images   [H][n_tiles][TILE]
-  const uint8_t* kt;       // K^ bf16 images
+  const uint8_t* qt;       // Q^' fp16 images (q~ * softmax_scale * log2e)   [H][n_tiles][TILE]
+  const uint8_t* kt;       // K^ fp16 images
   const uint8_t* vt;       // V  bf16 images
   const uint8_t* dot;      // dO bf16 images
   const float* lse2_t;     // [H][n_tiles][128]  lse*log2e, +inf on pad rows
@@ -43,7 +43,6 @@ struct BwdFusedParams {
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
   ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
   float* gv_t;             // nullable (context parallelism): dV PARTIAL fp32 [N,H,D] written instead of dv
-  int q_rot;               // rotate the query-tile order per key tile (spreads the L2 reductions)
 };
 
 template <int D>
@@ -142,11 +141,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
   if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(1 * kTraceMaxCtas + blockIdx.x) * 2] = globaltimer_ns();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
-  const float scale_log2 = pd.softmax_scale * 1.4426950408889634f;
   const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
 
-  // query tile visited at inner iteration i of a work item (same function in every role)
-  auto q_tile_of = [&](const WorkItem& wi, int i, int n) { return bp.q_rot ? (i + wi.tile * bp.q_rot) % n : i; };
 
   if (warp == 12) {
     // ------------------------------------------------------------------ producer
@@ -166,7 +162,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
         bulk_g2s(sV, bp.vt + xoff, TILE, kv_full);
       }
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
-        const int qt = sq.qt_lo + q_tile_of(wi, i, sq.qt_n);
+        const int qt = sq.qt_lo + i;
         const size_t yoff = hoff + static_cast<size_t>(sq.tile_base + qt) * TILE;
         const size_t roff = (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * kTileRows;
         const uint32_t qs = g % QS, qph = (g / QS) & 1, ds = g % DS, dph = (g / DS) & 1;
@@ -188,10 +184,14 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
   } else if (warp == 13) {
     // ------------------------------------------------------------------ MMA issuer
     setmaxnreg_dec<56>();
-    constexpr uint32_t idesc_sdp = make_idesc(128, 128, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
+    // Operand formats: S^T is recomputed from the forward's fp16 Q^', K^ images (same bytes -> same logits as
+    // the stored LSE was built from); dS^T is fp16 as well (scaled by the group's power of two sk), so that it can pair with
+    // those images in dK~ and dQ~; P^T, V and dO stay bf16 (range).
+    constexpr uint32_t idesc_s = make_idesc(128, 128, FMT_F16, FMT_F16, MAJOR_K, MAJOR_K);
+    constexpr uint32_t idesc_dp = make_idesc(128, 128, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_K);
     constexpr uint32_t idesc_dv = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
-    constexpr uint32_t idesc_dk = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
-    constexpr uint32_t idesc_dq = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_MN, MAJOR_MN);
+    constexpr uint32_t idesc_dk = make_idesc(128, D, FMT_F16, FMT_F16, MAJOR_K, MAJOR_MN);
+    constexpr uint32_t idesc_dq = make_idesc(128, D, FMT_F16, FMT_F16, MAJOR_MN, MAJOR_MN);
     const uint32_t aK = smem_u32(sK), aV = smem_u32(sV), aQ = smem_u32(sQ), adO = smem_u32(sdO), adS = smem_u32(sdS);
     const uint32_t tS = tbase + Cfg::kColS, tdP = tbase + Cfg::kColDP, tdV = tbase + Cfg::kColDV, tdK = tbase + Cfg::kColDK;
     uint32_t it = 0, g0 = 0;
@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
-          umma_ss(tS, make_sdesc(aK + koff, 16, 1024), make_sdesc(aQ + qs * TILE + koff, 16, 1024), idesc_sdp, kk > 0);
+          umma_ss(tS, make_sdesc(aK + koff, 16, 1024), make_sdesc(aQ + qs * TILE + koff, 16, 1024), idesc_s, kk > 0);
         }
         umma_commit(s_full);
       }
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
           const uint32_t koff = (kk >> 2) * BLK + (kk & 3) * 32;
-          umma_ss(tdP, make_sdesc(aV + koff, 16, 1024), make_sdesc(adO + ds * TILE + koff, 16, 1024), idesc_sdp, kk > 0);
+          umma_ss(tdP, make_sdesc(aV + koff, 16, 1024), make_sdesc(adO + ds * TILE + koff, 16, 1024), idesc_dp, kk > 0);
         }
         umma_commit(dp_full);
       }
@@ -299,6 +299,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       if (item < 0) break;
       const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
+      const float2 skv = *reinterpret_cast<const float2*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2);
+      const float sk = skv.x;                    // dS is rounded to fp16 as dS * sk (delta already carries sk: bwd_scale_kernel)
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const uint32_t qs = g % QS, qph = (g / QS) & 1;
         const float* lse_s = sLse + qs * 128 + wg * 64;
@@ -316,8 +318,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
 #pragma unroll
           for (int c = 0; c < 32; c += 2) {
             const float2 l2 = *reinterpret_cast<const float2*>(&lse_s[half * 32 + c]);
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c]), scale_log2, -l2.x));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), scale_log2, -l2.y));
+            const float p0 = ex2_approx(__uint_as_float(sv[c]) - l2.x);       // S^T is already in the exp2 domain (Q^')
+            const float p1 = ex2_approx(__uint_as_float(sv[c + 1]) - l2.y);
             p[half * 32 + c] = p0; p[half * 32 + c + 1] = p1;
             pk[c >> 1] = pack_bf16x2(p0, p1);
           }
@@ -342,9 +344,9 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
             for (int e = 0; e < 8; e += 2) {
               const int c = c8 * 8 + e;
               const float2 d2 = *reinterpret_cast<const float2*>(&dl_s[half * 32 + c]);
-              const float ds0 = p[half * 32 + c] * (__uint_as_float(dpv[c]) - d2.x);
-              const float ds1 = p[half * 32 + c + 1] * (__uint_as_float(dpv[c + 1]) - d2.y);
-              w[e >> 1] = pack_bf16x2(ds0, ds1);
+              const float ds0 = p[half * 32 + c] * fmaf(__uint_as_float(dpv[c]), sk, -d2.x);
+              const float ds1 = p[half * 32 + c + 1] * fmaf(__uint_as_float(dpv[c + 1]), sk, -d2.y);
+              w[e >> 1] = pack_f16x2(ds0, ds1);
             }
             const uint32_t chunk = half * 4 + c8;
             *reinterpret_cast<uint4*>(dS_row + ((chunk ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
@@ -364,7 +366,8 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       const size_t out_off = (static_cast<size_t>(sq.tok_start + n) * pd.H + wi.head) * D;
       const uint32_t tA = tbase + (wg == 0 ? Cfg::kColDV : Cfg::kColDK) + lane_base;
       const bool dv_bf16 = wg == 0 && bp.gv_t == nullptr;      // CP: dV leaves as an fp32 partial like dK~
-      const float sc = wg == 0 ? 1.0f : pd.softmax_scale;
+      // dk~ = scale * dS^T q~ = ln2 * dS^T Q^' (Q^' = q~ * scale * log2e), and dS carries sk
+      const float sc = wg == 0 ? 1.0f : 0.6931471805599453f * skv.y;
       float* f32_out = wg == 0 ? bp.gv_t : bp.gk_t;
       __nv_bfloat16* dv_row = (valid_row && dv_bf16) ? raw_row<__nv_bfloat16>(pd.sh, bp.dv, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll
@@ -404,7 +407,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tdQ = tbase + Cfg::kColDP + lane_base;
     const bool leader = threadIdx.x == 256;
-    const float sc = pd.softmax_scale;
+    float sc = 0.f;                                                 // softmax_scale / sk of the current item
     float* stage_row = reinterpret_cast<float*>(sStage) + q * 32;   // row q of staging buffer 0; buffer 1 at +128*32
     uint32_t g = 0;
     // chunk = 32 d-columns of the tile (16 KB, contiguous in the blocked global layout).  Two staging
@@ -434,8 +437,9 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       if (item < 0) break;
       const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
+      sc = pd.softmax_scale * pd.grp_sk[(static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2 + 1];
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
-        const int qt = sq.qt_lo + q_tile_of(wi, i, sq.qt_n);
+        const int qt = sq.qt_lo + i;
         float* gtile = bp.gq_blk + (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * (kTileRows * D);
         mbar_wait(dq_full, g & 1);
         tc_fence_after();

@@ -111,7 +111,13 @@ struct ProblemDesc {
   const WorkItem* dyn_fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int* work_counter;             // [2] next index into dyn_fwd_items / dyn_items; zeroed by the host before each launch
   const int* item_ptr;       // [n_ctas + 1] CTA c owns items [item_ptr[c], item_ptr[c+1]) (host LPT assignment)
-  unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel
+  unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel.  stats,
+                             // work_counter, grp_stats and grp_sk live in the header of the CALLER'S workspace (WsHeader below),
+                             // i.e. they are per call: two calls on one plan with different workspaces do not share them
+  unsigned* grp_stats;       // backward: [num_seqs * H][4] float bits, (sequence, head) group g: [0] max_i |dO_i|^2, [1] max_j |V_j|^2
+  unsigned* dq_error;        // WsHeader::dq_error
+  float* grp_sk;             // backward: [num_seqs * H][2] = (sk, 1/sk): the power of two dS is multiplied by before it is
+                             // rounded to fp16 (bwd_scale_kernel, prep.cuh)
   int n_items;
   int n_tiles_total;
   int num_seqs;
@@ -124,5 +130,14 @@ struct ProblemDesc {
   unsigned long long* cta_trace;   // nullable: [kernel 0 fwd | 1 bwd_fused][gridDim.x][2] globaltimer ns at CTA start / end
   int cp_lo, cp_hi;          // context parallelism: this process owns the QUERY tokens [cp_lo, cp_hi) (0, N otherwise)
 };
+
+// Header of every workspace (forward and backward): the per-call mutable words of the kernels.
+struct WsHeader {
+  unsigned qk_bound[2];      // ProblemDesc::stats
+  int work_counter[2];       // ProblemDesc::work_counter ([0] fwd_kernel, [1] bwd_fused_kernel)
+  unsigned dq_error;         // ordered (deterministic) dQ~ reduction: set if a ticket wait timed out
+  unsigned pad[11];
+};
+static_assert(sizeof(WsHeader) == 64, "WsHeader");
 
 }  // namespace arachne

@@ -31,6 +31,8 @@ struct FwdParams {
   const uint8_t* vt;      // V bf16 images
   ShardedPtr o;           // [N,H_total,D] bf16, possibly sharded by token range (common.cuh)
   float* lse;             // [H,N]
+  unsigned* envelope;     // plan-owned sticky word: float bits of the largest logit bound that exceeded bound_limit
+  float bound_limit;      // logit bound (log2 units) the gates are claimed for; +inf with ARACHNE_FLAG_WIDE_LOGITS
 };
 
 template <int D>
@@ -96,6 +98,11 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
 
   if (warp == 8) {
     // ------------------------------------------------------------------ producer
+    if (blockIdx.x == 0 && lane == 0) {
+      // outside the envelope the gates are claimed for (DESIGN.md §6 / R19): leave a sticky mark (arachne_plan_logit_status)
+      const float bound = sqrtf(__uint_as_float(pd.stats[0])) * sqrtf(__uint_as_float(pd.stats[1]));
+      if (bound > fp.bound_limit) atomicMax(fp.envelope, __float_as_uint(bound));
+    }
     uint32_t it = 0, ring = 0;
     for (;; ++it) {
       const int item = item_fetch_producer(item_ring, it, pd.work_counter, pd.n_fwd_items, lane);

@@ -1,5 +1,5 @@
 // Elementwise (HBM-bound) kernels around the tensor-core kernels:
-//   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> 16-bit operand tile images;
+//   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> fp16 operand tile images;
 //                 V, dO -> tile images (zero-padded tails); D_i = rowsum(dO*O); LSE*log2e padded.
 //   post_kernel : §8 a8.  dq~, dk~ (fp32) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK (+ dgamma partials, R22).
 // Thread mapping: a lane owns 8 contiguous elements (one 16-byte bf16 load / store, one swizzle chunk of a tile
@@ -17,7 +17,6 @@ namespace arachne {
 struct PrepParams {
   ShardedPtr q, k, v;          // raw bf16 [N, H_total, D], possibly sharded by token range (common.cuh)
   ShardedPtr d_o, o;           // backward only
-  int backward;                // 0 forward, 1 backward (d_o, o, lse valid)
   const float* lse;            // nullable (forward)
   const float* gamma_q;        // nullable => ones
   const float* gamma_k;
@@ -28,10 +27,10 @@ struct PrepParams {
   float* lse2_t;               // [H][n_tiles][128]  lse * log2(e); +inf on pad rows
   float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
   float* gq_zero;              // nullable: blocked dq~ accumulator [H][n_tiles][128*D] to clear (fused backward)
-  int out_fmt;                 // FMT_F16 (forward: LSE accuracy) or FMT_BF16 (backward)
-  float q_prescale;            // Q^ is multiplied by this before rounding (forward: softmax_scale*log2(e), so that
-                               // S comes out of the tensor core already in the exp2 domain; backward: 1)
-  unsigned* stats;             // nullable: [0] = max_i |q~_i|^2, [1] = max_j |k~_j|^2 as float bits (atomicMax);
+  float q_prescale;            // Q^ is multiplied by softmax_scale*log2(e) before it is rounded to fp16, so that S leaves the
+                               // tensor core already in the exp2 domain — in the forward AND in the backward's recompute, which
+                               // therefore sees bit-identical operands (P = exp2(S - LSE) consistent with the stored LSE)
+  unsigned* stats;             // nullable (forward): [0] = max_i |q~'_i|^2, [1] = max_j |k~_j|^2 as float bits (atomicMax);
                                // the forward kernel derives its logit bound from them (static-max softmax)
 };
 
@@ -103,7 +102,7 @@ __device__ __forceinline__ float norm_rope8(float (&x)[8], const float (&gam)[8]
   return nrm;
 }
 
-template <int D>
+template <int D, bool kBwd>
 __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams pp) {
   constexpr int LPR = D / 8, RPW = 32 / LPR;
   constexpr int TILE_BYTES = kTileRows * D * 2;
@@ -111,6 +110,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int sub = lane / LPR, d0 = (lane % LPR) * 8;
   float qn = 0.f, kn = 0.f;      // largest |q~|^2, |k~|^2 seen by this lane's rows (no_norm only)
+  float gn = 0.f, vn = 0.f;      // backward: largest |dO_i|^2, |V_j|^2 seen by this lane's rows (bound on dS, bwd_scale_kernel)
   const SeqInfo sq = pd.seqs[pd.tile_seq[gtile]];
   const int t = gtile - sq.tile_base;
   const size_t img_off = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * TILE_BYTES;
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
       if (q_side) uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
       uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src);
       uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);
-      if (pp.backward && q_side) {
+      if (kBwd && q_side) {
         ug = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src);
         uo = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.o, shard) + src);
       }
@@ -157,12 +157,19 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     const float qs = norm_rope8<D>(xq, gq, cs, pd.no_norm != 0, pd.eps, pp.q_prescale);
     const float ks = norm_rope8<D>(xk, gk, cs, pd.no_norm != 0, pd.eps, 1.0f);
     const uint32_t ioff = image_off(r, d0);
-    if (q_side) *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, pp.out_fmt) : zero4;   // (eps = 0: 0 * inf)
-    *reinterpret_cast<uint4*>(pp.kt + img_off + ioff) = valid ? pack8(xk, pp.out_fmt) : zero4;
+    if (q_side) *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, FMT_F16) : zero4;   // (eps = 0: 0 * inf)
+    *reinterpret_cast<uint4*>(pp.kt + img_off + ioff) = valid ? pack8(xk, FMT_F16) : zero4;
     *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
     // row norms are only needed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, seg_sum<LPR>(qs)); kn = fmaxf(kn, seg_sum<LPR>(ks)); }
-    if (pp.backward && q_side) {
+    if (kBwd) {
+      float vv[8], v2 = 0.f;
+      unpack_bf16x8(uv, vv);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) v2 += vv[i] * vv[i];
+      vn = fmaxf(vn, seg_sum<LPR>(v2));
+    }
+    if (kBwd && q_side) {
       *reinterpret_cast<uint4*>(pp.dot + img_off + ioff) = ug;
       float g[8], oo[8];
       unpack_bf16x8(ug, g);
@@ -171,6 +178,10 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
 #pragma unroll
       for (int i = 0; i < 8; ++i) dsum += g[i] * oo[i];
       dsum = seg_sum<LPR>(dsum);                                // D_i = sum_d dO*O   (§8 a5)
+      float g2 = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) g2 += g[i] * g[i];
+      gn = fmaxf(gn, seg_sum<LPR>(g2));
       if (d0 == 0) {
         // context parallelism: query rows of other ranks behave like pad rows here (P = 0: no dK/dV contribution)
         const bool live = valid && tok >= pd.cp_lo && tok < pd.cp_hi;
@@ -179,6 +190,20 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
         pp.lse2_t[row_off + r] = live ? pp.lse[static_cast<size_t>(h) * pd.N + tok] * 1.4426950408889634f
                                        : __int_as_float(0x7f800000);
       }
+    }
+  }
+  if (kBwd && touched) {
+    // per (sequence, head) group: max_i |dO_i|^2 and max_j |V_j|^2 (non-negative floats order like their bit patterns;
+    // NaN / inf sort last and make bwd_scale_kernel fall back to sk = 1)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      gn = fmaxf(gn, __shfl_xor_sync(0xffffffffu, gn, o));
+      vn = fmaxf(vn, __shfl_xor_sync(0xffffffffu, vn, o));
+    }
+    if (lane == 0) {
+      unsigned* gs = pd.grp_stats + (static_cast<size_t>(pd.tile_seq[gtile]) * pd.H + h) * 4;
+      atomicMax(&gs[0], __float_as_uint(gn));
+      atomicMax(&gs[1], __float_as_uint(vn));
     }
   }
   if (pp.stats) {
@@ -214,6 +239,34 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
         atomicMax(&pp.stats[1], __float_as_uint(kn));
       }
     }
+  }
+}
+
+// dS scaling for the fp16 backward GEMMs.  The backward recomputes S from the SAME fp16 Q^', K^ images as the
+// forward, so dS must be fp16 too (tcgen05 kind::f16 takes one 16-bit format per instruction pair of operands); fp16 has 5
+// exponent bits, so dS is multiplied by a power of two sk chosen per (sequence, head) group from a rigorous bound:
+//   |dS_ij| = P_ij |dO_i.V_j - dO_i.O_i| <= 2 max_i|dO_i| max_j|V_j|      (P_ij <= 1; O_i is a convex combination of the V_j)
+//   sk = 2^floor(log2(32768 / (2.02 max|dO| max|V|)))   =>   |dS sk| <= 32768 < 65504, never overflows;
+// entries more than 2^-29 below the bound lose relative (not absolute) precision in fp16 subnormals — their absolute error,
+// 2^-25/sk, stays ~2^16 times below bf16's at the bound.  The factor is folded into delta (this kernel) and the dP FFMA.
+// Grid (n_tiles_total, H), 128 threads (one row each).
+__global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* delta_t) {
+  const int gtile = blockIdx.x, h = blockIdx.y;
+  const int b = pd.tile_seq[gtile];
+  const size_t g = static_cast<size_t>(b) * pd.H + h;
+  const float gn = __uint_as_float(pd.grp_stats[g * 4]), vn = __uint_as_float(pd.grp_stats[g * 4 + 1]);
+  const float bound = 2.02f * sqrtf(gn) * sqrtf(vn);
+  float sk = 1.0f;
+  if (bound > 0.f && bound < 3.0e38f) {      // (false for NaN)
+    int e = static_cast<int>(floorf(log2f(32768.0f / bound)));
+    e = max(-60, min(60, e));
+    sk = exp2f(static_cast<float>(e));
+  }
+  const size_t row = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows + threadIdx.x;
+  delta_t[row] *= sk;
+  if (threadIdx.x == 0 && gtile == pd.seqs[b].tile_base) {
+    pd.grp_sk[g * 2] = sk;
+    pd.grp_sk[g * 2 + 1] = 1.0f / sk;
   }
 }
 

@@ -31,7 +31,7 @@ def test_status_strings_and_validation_without_device():
     from paper_2607_01701_b200 import binding
 
     lib = binding._lib
-    for s in range(0, 14):
+    for s in range(0, 15):
         assert lib.arachne_status_string(s).decode() not in ("", "unknown status")
     assert lib.arachne_status_string(99).decode() == "unknown status"
     assert lib.arachne_workspace_bytes(None, 0) == 0
@@ -63,3 +63,11 @@ def test_status_strings_and_validation_without_device():
     cu_big = (ctypes.c_int32 * 2)(0, 2 ** 27)
     gr_big = (ctypes.c_int32 * 3)(2 ** 27, 1, 1)
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(big), cu_big, gr_big) == 11
+    # envelope (arachne_attn.h "Verified envelope"): an explicit softmax_scale with scale*sqrt(D) > 1 is refused on the host
+    # unless the caller passes ARACHNE_FLAG_WIDE_LOGITS (then validation goes on: here to the grid check)
+    p.softmax_scale = 0.2
+    assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == binding.ERR_LOGIT_RANGE
+    p.flags = binding.FLAG_WIDE_LOGITS
+    assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5
+    p.flags = 16                                                                       # unknown flag bit
+    assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 12
