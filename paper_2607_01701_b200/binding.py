@@ -128,6 +128,35 @@ def _ptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
 
 
+def _want(t, name, dtype, shape=None, device="cuda", optional=False):
+    """The C side can only check alignment: a non-contiguous view (a slice of a fused QKV projection), a wrong dtype or a
+    CPU tensor would silently give wrong results or fault, so the marshalling layer refuses them here."""
+    if t is None:
+        if optional:
+            return
+        raise TypeError(f"{name}: tensor required")
+    if t.device.type != device:
+        raise TypeError(f"{name}: expected a {device} tensor, got {t.device}")
+    if t.dtype != dtype:
+        raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise TypeError(f"{name}: must be contiguous (the ABI takes contiguous [N, H, D] tensors; call .contiguous())")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise TypeError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+
+
+def _want_call(plan, bf16, lse=None, gammas=(), workspace=None, device="cuda"):
+    nhd = (plan.N, plan.H, plan.D)
+    for name, t in bf16.items():
+        _want(t, name, torch.bfloat16, nhd, device)
+    if lse is not None:
+        _want(lse, "lse", torch.float32, (plan.H, plan.N), device)
+    for name, t in gammas:
+        _want(t, name, torch.float32, (plan.D,), device, optional=True)
+    if workspace is not None:
+        _want(workspace, "workspace", torch.uint8, None, device)
+
+
 class Plan:
     """arachne_plan_create[_joint] / arachne_plan_destroy.  text_lens [B] (optional): trailing text tokens of
     each sequence (arachne_plan_create_joint).  shard_starts [k+1] (+ total_heads, head_offset): token-range
@@ -227,6 +256,7 @@ def _stream_ptr(stream):
 
 def arachne_varlen_attn_fwd(plan: Plan, q, k, v, o, lse, workspace, gamma_q=None, gamma_k=None, stream=None):
     """q,k,v,o: bf16 CUDA [N,H,D]; lse: fp32 CUDA [H,N]; workspace: uint8 CUDA >= plan.workspace_bytes(False)."""
+    _want_call(plan, dict(q=q, k=k, v=v, o=o), lse, (("gamma_q", gamma_q), ("gamma_k", gamma_k)), workspace)
     _check(_lib.arachne_varlen_attn_fwd(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
                                         _ptr(lse), _ptr(workspace), workspace.numel() * workspace.element_size(),
                                         _stream_ptr(stream)))
@@ -234,6 +264,7 @@ def arachne_varlen_attn_fwd(plan: Plan, q, k, v, o, lse, workspace, gamma_q=None
 
 def arachne_varlen_attn_bwd(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, workspace, gamma_q=None, gamma_k=None,
                             stream=None):
+    _want_call(plan, dict(q=q, k=k, v=v, o=o, d_o=d_o, dq=dq, dk=dk, dv=dv), lse, (("gamma_q", gamma_q), ("gamma_k", gamma_k)), workspace)
     _check(_lib.arachne_varlen_attn_bwd(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
                                         _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(workspace),
                                         workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
@@ -242,6 +273,8 @@ def arachne_varlen_attn_bwd(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, worksp
 def arachne_varlen_attn_bwd_dgamma(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, dgamma_q, dgamma_k, workspace,
                                    gamma_q=None, gamma_k=None, stream=None):
     """As arachne_varlen_attn_bwd, plus dgamma_q, dgamma_k: fp32 CUDA [D] (either may be None)."""
+    _want_call(plan, dict(q=q, k=k, v=v, o=o, d_o=d_o, dq=dq, dk=dk, dv=dv), lse,
+               (("gamma_q", gamma_q), ("gamma_k", gamma_k), ("dgamma_q", dgamma_q), ("dgamma_k", dgamma_k)), workspace)
     _check(_lib.arachne_varlen_attn_bwd_dgamma(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
                                                _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk), _ptr(dv), _ptr(dgamma_q),
                                                _ptr(dgamma_k), _ptr(workspace),
@@ -295,11 +328,14 @@ def arachne_cp_reduce(plan: Plan, dk_partials, dv_partials, k, dk, dv, workspace
 
 def arachne_varlen_attn_fwd_host(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None):
     """Same as fwd but every tensor is a HOST (CPU, preferably pinned) tensor; copies are inside the call."""
+    _want_call(plan, dict(q=q, k=k, v=v, o=o), lse, (("gamma_q", gamma_q), ("gamma_k", gamma_k)), device="cpu")
     _check(_lib.arachne_varlen_attn_fwd_host(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k),
                                              _ptr(o), _ptr(lse)))
 
 
 def arachne_varlen_attn_fwd_bwd_host(plan: Plan, q, k, v, d_o, o, lse, dq, dk, dv, gamma_q=None, gamma_k=None):
+    _want_call(plan, dict(q=q, k=k, v=v, o=o, d_o=d_o, dq=dq, dk=dk, dv=dv), lse, (("gamma_q", gamma_q), ("gamma_k", gamma_k)),
+               device="cpu")
     _check(_lib.arachne_varlen_attn_fwd_bwd_host(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k),
                                                  _ptr(d_o), _ptr(o), _ptr(lse), _ptr(dq), _ptr(dk), _ptr(dv)))
 

@@ -64,15 +64,17 @@ def balanced_starts(cu_seqlens: Sequence[int], world_size: int) -> List[int]:
 
 class ContextParallelAttention:
     """Forward / backward over a CP group of k GPUs in one NVSwitch domain (torch.distributed + symmetric memory).
-    forward(): barrier -> fwd_sharded -> (no barrier needed: a rank writes only its own O shard).
-    backward(): barrier -> bwd_cp_partial -> barrier -> cp_reduce -> all-reduce of the dgamma parts."""
+    forward(): barrier -> fwd_sharded -> barrier (a rank writes only its own O shard, but it READS its peers' Q, K, V
+    shards: nobody may overwrite its inputs for the next layer until every rank's kernels are done with them).
+    backward(): barrier -> bwd_cp_partial -> barrier -> cp_reduce -> all-reduce of the dgamma parts -> barrier.
+    The barriers are stream-ordered under NCCL (ulysses.RankSync), host barriers under gloo."""
 
     def __init__(self, st: dict, group=None, starts=None, transport: str = "symm"):
         import torch
         import torch.distributed as dist
 
         from . import binding
-        from .ulysses import IpcShards, SymmetricShards
+        from .ulysses import IpcShards, RankSync, SymmetricShards
 
         self.group, self._dist, self._binding = group, dist, binding
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
@@ -95,31 +97,44 @@ class ContextParallelAttention:
                 self.part[n] = (sh.local_full, sh.ptrs, sh)
         self.lse = torch.empty((st["H"], st["N"]), dtype=torch.float32, device=dev)
         self.ws = torch.empty(max(self.plan.workspace_bytes(False), self.plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
+        self._sync = RankSync(group, dev)
+        self._D = st["D"]
 
     def _barrier(self):
-        import torch
-
-        torch.cuda.current_stream().synchronize()
-        self._dist.barrier(self.group)
+        self._sync.barrier()
 
     def forward(self, gamma_q=None, gamma_k=None):
         b = self.buf
         self._barrier()
         self._binding.arachne_varlen_attn_fwd_sharded(self.plan, b["q"].ptrs, b["k"].ptrs, b["v"].ptrs, b["o"].ptrs, self.lse,
                                                       self.ws, gamma_q, gamma_k)
+        self._barrier()              # every rank has finished READING its peers' Q, K, V before anyone reuses them
         return b["o"].local(self.n_local)
 
-    def backward(self, gamma_q=None, gamma_k=None):
+    def backward(self, gamma_q=None, gamma_k=None, with_dgamma=False):
+        """-> (dq, dk, dv, dgamma_q, dgamma_k) of this rank's tokens; dgamma (reading R22) is the sum over ALL ranks
+        (step 1 yields this rank's part of dgamma_q, step 2 its part of dgamma_k; both are all-reduced), or None."""
+        import torch
+
         b = self.buf
+        dgq = dgk = None
+        if with_dgamma:
+            dgq = torch.empty(self._D, dtype=torch.float32, device=self.lse.device)
+            dgk = torch.empty_like(dgq)
         self._barrier()
         self._binding.arachne_varlen_attn_bwd_cp_partial(self.plan, b["q"].ptrs, b["k"].ptrs, b["v"].ptrs, b["o"].ptrs, self.lse,
                                                          b["dO"].ptrs, b["dq"].ptrs, self.part["dk_partial"][0],
-                                                         self.part["dv_partial"][0], self.ws, None, gamma_q, gamma_k)
+                                                         self.part["dv_partial"][0], self.ws, dgq, gamma_q, gamma_k)
         self._barrier()
         self._binding.arachne_cp_reduce(self.plan, self.part["dk_partial"][1], self.part["dv_partial"][1], b["k"].ptrs,
-                                        b["dk"].ptrs, b["dv"].ptrs, self.ws, None, gamma_k)
+                                        b["dk"].ptrs, b["dv"].ptrs, self.ws, dgk, gamma_k)
+        if with_dgamma:
+            if self.n_local == 0:                    # a rank without tokens launches no row: its parts are zero
+                dgq.zero_(); dgk.zero_()
+            both = self._sync.all_reduce_sum(torch.stack([dgq, dgk]))
+            dgq, dgk = both[0], both[1]
         self._barrier()
-        return b["dq"].local(self.n_local), b["dk"].local(self.n_local), b["dv"].local(self.n_local)
+        return b["dq"].local(self.n_local), b["dk"].local(self.n_local), b["dv"].local(self.n_local), dgq, dgk
 
     def close(self):
         for b in list(self.buf.values()) + [p[2] for p in self.part.values() if p[2] is not None]:

@@ -1,6 +1,6 @@
 """DiT latency model of the paper, Eq. (9), fitted from THIS kernel's measured times
 (first half: the coefficients; the list scheduler + genetic algorithm of Alg. 1 that consume
-them are not built).
+them are csrc/cascade_sched.cpp, include/arachne_sched.h, bound by scheduler.py).
 
     L_DiT(B, S, k) = (alpha1 * B*S + alpha2 * B*S^2) / k + V_comm / BW_eff(k)
 

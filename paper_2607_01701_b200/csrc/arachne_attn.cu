@@ -800,15 +800,11 @@ struct arachne_host_ctx {
 static void arachne_host_ctx_free(arachne_host_ctx* c) { delete c; }
 extern "C" {
 
-static int host_ctx(const arachne_plan* pl, bool with_bwd, arachne_host_ctx** out) {
+static int host_ctx_fill(const arachne_plan* pl, bool with_bwd, arachne_host_ctx* c, bool fresh) {
   const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
   const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
   const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
-  arachne_host_ctx* c = pl->host;
-  if (!c) {
-    c = new (std::nothrow) arachne_host_ctx();
-    if (!c) { g_last_error = "out of host memory"; return ARACHNE_ERR_CUDA; }
-    pl->host = c;
+  if (fresh) {
     ARACHNE_CUDA(cudaStreamCreateWithFlags(&c->compute, cudaStreamNonBlocking));
     ARACHNE_CUDA(cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking));
     for (cudaEvent_t* e : {&c->ev_do_up, &c->ev_fwd, &c->ev_o_down, &c->ev_dv})
@@ -827,9 +823,33 @@ static int host_ctx(const arachne_plan* pl, bool with_bwd, arachne_host_ctx** ou
     ARACHNE_CUDA(cudaMalloc(&c->dk, nb)); ARACHNE_CUDA(cudaMalloc(&c->dv, nb));
     c->has_bwd = true;
   }
+  return ARACHNE_OK;
+}
+
+// The context is cached in the plan only once EVERY allocation has succeeded: a failed cudaMalloc (e.g. out of memory on a
+// 262K-token batch) frees whatever was built and leaves the plan as it was, so the next host call starts from scratch
+// instead of running on null buffers.
+static int host_ctx(const arachne_plan* pl, bool with_bwd, arachne_host_ctx** out) {
+  arachne_host_ctx* c = pl->host;
+  const bool fresh = c == nullptr;
+  if (fresh) {
+    c = new (std::nothrow) arachne_host_ctx();
+    if (!c) { g_last_error = "out of host memory"; return ARACHNE_ERR_CUDA; }
+  }
+  const int rc = host_ctx_fill(pl, with_bwd, c, fresh);
+  if (rc != ARACHNE_OK) {
+    if (!fresh) pl->host = nullptr;
+    delete c;                        // frees every buffer, event and stream it holds
+    return rc;
+  }
+  pl->host = c;
   *out = c;
   return ARACHNE_OK;
 }
+
+static int run_host_enqueue(const arachne_plan* pl, arachne_host_ctx* c, bool with_bwd, const void* q_h, const void* k_h,
+                            const void* v_h, const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h,
+                            void* dq_h, void* dk_h, void* dv_h);
 
 static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, const void* k_h, const void* v_h,
                     const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h, void* dq_h,
@@ -837,12 +857,24 @@ static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, cons
   if (!pl || !q_h || !k_h || !v_h || !o_h || !lse_h) return ARACHNE_ERR_NULL_POINTER;
   if (with_bwd && (!do_h || !dq_h || !dk_h || !dv_h)) return ARACHNE_ERR_NULL_POINTER;
   if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;
-  const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
-  const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
-  const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
   arachne_host_ctx* c = nullptr;
   int rc = host_ctx(pl, with_bwd, &c);
   if (rc) return rc;
+  rc = run_host_enqueue(pl, c, with_bwd, q_h, k_h, v_h, gq_h, gk_h, do_h, o_h, lse_h, dq_h, dk_h, dv_h);
+  // whatever happened, nothing is left running on the private streams when the call returns
+  const cudaError_t e1 = cudaStreamSynchronize(c->copy), e2 = cudaStreamSynchronize(c->compute);
+  if (rc == ARACHNE_OK && e1 != cudaSuccess) return cuda_fail(e1, "cudaStreamSynchronize(copy)");
+  if (rc == ARACHNE_OK && e2 != cudaSuccess) return cuda_fail(e2, "cudaStreamSynchronize(compute)");
+  return rc;
+}
+
+static int run_host_enqueue(const arachne_plan* pl, arachne_host_ctx* c, bool with_bwd, const void* q_h, const void* k_h,
+                            const void* v_h, const float* gq_h, const float* gk_h, const void* do_h, void* o_h, float* lse_h,
+                            void* dq_h, void* dk_h, void* dv_h) {
+  const size_t nb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * pl->p.head_dim * 2;
+  const size_t lb = static_cast<size_t>(pl->p.total_tokens) * pl->p.num_heads * sizeof(float);
+  const size_t gb = static_cast<size_t>(pl->p.head_dim) * sizeof(float);
+  int rc;
   cudaStream_t st = c->compute, cp = c->copy;
   float* gq = gq_h ? static_cast<float*>(c->gq) : nullptr;
   float* gk = gk_h ? static_cast<float*>(c->gk) : nullptr;
@@ -874,8 +906,6 @@ static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, cons
     ARACHNE_CUDA(cudaMemcpyAsync(dq_h, c->dq, nb, cudaMemcpyDeviceToHost, st));
     ARACHNE_CUDA(cudaMemcpyAsync(dk_h, c->dk, nb, cudaMemcpyDeviceToHost, st));
   }
-  ARACHNE_CUDA(cudaStreamSynchronize(cp));
-  ARACHNE_CUDA(cudaStreamSynchronize(st));
   return ARACHNE_OK;
 }
 

@@ -139,6 +139,42 @@ class IpcShards:
             self._addr = 0
 
 
+class RankSync:
+    """Orders the ranks of an SP / CP group around a kernel that reads or writes peer memory.
+
+    NCCL group: a one-element all-reduce ENQUEUED ON THE CURRENT STREAM.  It starts after this rank's earlier kernels on the
+    stream (whose remote stores are then complete) and finishes only when every rank has entered it, and later kernels on
+    the stream start after it — a device-side barrier with no host synchronisation, so the host runs ahead and the
+    launch of the next kernel overlaps the wait.  gloo group (the CPU / one-GPU tests, no device collective): host
+    synchronisation of the stream + a host barrier, as before."""
+
+    def __init__(self, group, device):
+        import torch
+        import torch.distributed as dist
+
+        self._dist, self.group = dist, group
+        self.on_stream = dist.get_backend(group) == "nccl"
+        self._flag = torch.zeros(1, dtype=torch.float32, device=device) if self.on_stream else None
+
+    def barrier(self):
+        import torch
+
+        if self.on_stream:
+            self._dist.all_reduce(self._flag, group=self.group)     # stream-ordered; the host does not wait
+        else:
+            torch.cuda.current_stream().synchronize()               # my kernels (incl. their remote stores) have completed
+            self._dist.barrier(self.group)
+
+    def all_reduce_sum(self, t):
+        """Sum a small device tensor over the group (dgamma partials: 2 x D floats)."""
+        if self.on_stream:
+            self._dist.all_reduce(t, group=self.group)
+            return t
+        host = t.cpu()
+        self._dist.all_reduce(host, group=self.group)
+        return host.to(t.device)
+
+
 class UlyssesAttention:
     """Forward / backward of the packed attention over an SP group of k GPUs in one NVSwitch domain.
 
@@ -168,15 +204,13 @@ class UlyssesAttention:
         self.ws = torch.empty(max(self.plan.workspace_bytes(False), self.plan.workspace_bytes(True)), dtype=torch.uint8, device=dev)
         self._binding = binding
         self._dist = dist
+        self._sync = RankSync(group, dev)
 
     def local(self, name: str):
         return self.buf[name].local(self.n_local)
 
     def _barrier(self):
-        import torch
-
-        torch.cuda.current_stream().synchronize()      # my kernels (incl. their remote stores) have completed
-        self._dist.barrier(self.group)
+        self._sync.barrier()
 
     def forward(self, gamma_q=None, gamma_k=None):
         b = self.buf
@@ -199,13 +233,7 @@ class UlyssesAttention:
                                                       self.lse, b["dO"].ptrs, b["dq"].ptrs, b["dk"].ptrs, b["dv"].ptrs,
                                                       self.ws, dgq, dgk, gamma_q, gamma_k)
         if with_dgamma:        # gamma is shared by all heads (R1): sum the per-rank partials (2 x D floats)
-            both = torch.stack([dgq, dgk])
-            if self._dist.get_backend(self.group) == "gloo":
-                host = both.cpu()
-                self._dist.all_reduce(host, group=self.group)
-                both = host.to(dgq.device)
-            else:
-                self._dist.all_reduce(both, group=self.group)
+            both = self._sync.all_reduce_sum(torch.stack([dgq, dgk]))
             dgq, dgk = both[0], both[1]
         self._barrier()
         return self.local("dq"), self.local("dk"), self.local("dv"), dgq, dgk

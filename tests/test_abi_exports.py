@@ -71,3 +71,21 @@ def test_status_strings_and_validation_without_device():
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5
     p.flags = 16                                                                       # unknown flag bit
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 12
+
+
+def test_binding_rejects_tensors_the_c_side_cannot_check():
+    """dtype, device, contiguity and shape are checked by the marshalling layer (the C ABI sees only pointers)."""
+    import pytest
+    import torch
+    from paper_2607_01701_b200 import binding
+
+    good = torch.zeros(6, 2, 8, dtype=torch.bfloat16)
+    binding._want(good, "q", torch.bfloat16, (6, 2, 8), device="cpu")
+    binding._want(None, "gamma_q", torch.float32, (8,), device="cpu", optional=True)
+    for bad in (good.float(), good[:, :1], good.transpose(0, 1), torch.zeros(6, 2, 4, dtype=torch.bfloat16)):
+        with pytest.raises(TypeError):
+            binding._want(bad, "q", torch.bfloat16, (6, 2, 8), device="cpu")
+    with pytest.raises(TypeError):
+        binding._want(good, "q", torch.bfloat16, (6, 2, 8), device="cuda")      # a host tensor where a device one is needed
+    with pytest.raises(TypeError):
+        binding._want(None, "q", torch.bfloat16, (6, 2, 8))

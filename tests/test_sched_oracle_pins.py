@@ -95,5 +95,4 @@ def test_genetic_matches_brute_force_on_tiny_and_never_gets_worse():
     inst = inputs.cascade_instance(1, n_samples=10)
     args = (inst["K"], inst["L"], inst["feasible"], inst["preds"], inst["N"])
     T, ch, s, e, hist = so.genetic(*args, p=32, G=25, mu=0.1, eps=2, seed=1)
-    assert T <= hist[0] and T < hist[0] * 0.999 or T == hist[0]
     assert T <= hist[0]
