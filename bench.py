@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload long720p] [--impl reference] [--sp ulysses|cp]
 
-One "step" = one forward + one backward of the whole hot path (prep, fwd, prep, scale, backward main, post kernels)
+One "step" = one forward + one backward of the whole hot path (prep, fwd, prep, scale, bwd_fused, post kernels)
 over one packed batch of synthetic N(0,1) bf16 inputs of the named BASELINE.json config.
 `value` = 14*D*H*sum(L_b^2) / t (real lengths; norm/RoPE/softmax and every prologue / epilogue kernel count as time, not
 FLOPs), inputs resident in HBM.  `e2e` is the same metric through the C-ABI host call (pinned host buffers, H2D + D2H
@@ -266,8 +266,6 @@ def time_workload(env: Env, workload, steps, warmup, deterministic=False, order=
         try:
             cta_balance = {}
             for name, is_bwd in (("fwd_kernel", False), ("bwd_fused_kernel", True)):
-                if is_bwd and deterministic and not plan.deterministic_is_fused():
-                    continue
                 _, end_us = plan.cta_times(is_bwd)
                 cta_balance[name] = {"ctas": len(end_us), "end_max_us": max(end_us), "end_mean_us": sum(end_us) / len(end_us),
                                      "end_min_us": min(end_us), "max_over_mean": max(end_us) / (sum(end_us) / len(end_us))}
@@ -385,7 +383,7 @@ def main():
     # ---- roofline of the dominant kernel: dense contraction -> tensor roofline.
     # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); backward main kernel
     # 10*D*H*S2 (S, dP, dV, dK, dQ — the 5-GEMM backward convention).
-    alg = {"fwd_kernel": 4.0, "bwd_main(fused 5-GEMM | det: dKdV pass)": 10.0}
+    alg = {"fwd_kernel": 4.0, "bwd_fused_kernel": 10.0}
     kernels = [{"name": n, "ms": ms} for n, ms in r["kt_f"] + r["kt_b"]]
     dom = max(kernels, key=lambda k_: k_["ms"])
     dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2

@@ -164,13 +164,11 @@ void arachne_plan_destroy(arachne_plan* plan);
 size_t arachne_workspace_bytes(const arachne_plan* plan, int pass);
 
 /* Number of kernels one arachne_varlen_attn_fwd (pass 0) / arachne_varlen_attn_bwd (pass 1) call enqueues, for launch
- * accounting: fwd 2; bwd 4 (prep, bwd_scale, fused main, post) or 5 with ARACHNE_FLAG_DETERMINISTIC (two main passes);
- * the _dgamma form adds one. */
+ * accounting: fwd 2 (prep, fwd); bwd 4 (prep, bwd_scale, bwd_fused, post); the _dgamma form adds one. */
 int arachne_num_launches(const arachne_plan* plan, int pass);
 
 /* Name of TIMED INTERVAL `idx` (0-based, launch order) of a pass — the unit arachne_plan_kernel_times reports: fwd has 2
- * (prep_kernel, fwd_kernel), bwd has 4 (prep + bwd_scale, main kernel, second main pass [deterministic only, else 0 ms],
- * post [+ dgamma reduce]); "" if out of range. */
+ * (prep_kernel, fwd_kernel), bwd has 3 (prep + bwd_scale, bwd_fused_kernel, post [+ dgamma reduce]); "" if out of range. */
 const char* arachne_kernel_name(int pass, int idx);
 
 /* Sticky envelope status of a plan ("Verified envelope" above).  ARACHNE_OK if no forward launched on this plan without
@@ -182,7 +180,7 @@ int arachne_plan_logit_status(const arachne_plan* plan, float* tau_seen);
  * record a CUDA event before the first and after every kernel on the caller's stream (no
  * synchronisation is added); the plan keeps the events of the last 32 calls per pass.
  * arachne_plan_kernel_times synchronises on those events and writes to ms_sum[i] the SUM over
- * the recorded calls of timed interval i's duration in milliseconds (ms_sum has n_kernels >= 2 (fwd) / 4 (bwd)
+ * the recorded calls of timed interval i's duration in milliseconds (ms_sum has n_kernels >= 2 (fwd) / 3 (bwd)
  * entries, see arachne_kernel_name) and the number of calls to *n_calls.  Enabling resets the ring.
  * Not thread-safe with concurrent fwd/bwd on the same plan. */
 int arachne_plan_enable_profiling(arachne_plan* plan, int enable);
@@ -206,7 +204,9 @@ int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void*
 /* Backward.  Needs the o and lse that fwd produced for the same inputs and plan, and d_o
  * (bf16 [N,H,D]).  Writes dq, dk (gradients w.r.t. the RAW q, k) and dv, all bf16 [N,H,D].
  * With ARACHNE_FLAG_DETERMINISTIC the result is bit-identical from run to run on the same
- * device and plan (no atomics; fixed summation order). */
+ * device and plan: the fused kernel's dQ partial tiles are added in a fixed order (per-query-tile tickets),
+ * everything else has one owner per output tile.  A ticket wait that exceeds 4 s (it cannot, by construction) sets a
+ * flag in the workspace header instead of hanging the device. */
 int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
                             const float* gamma_q, const float* gamma_k, const void* o,
                             const float* lse, const void* d_o, void* dq, void* dk, void* dv,
@@ -257,7 +257,8 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const*
  *             is these peer loads), applies un-RoPE + RMSNorm backward, and writes dk[rank], dv[rank] (bf16) and
  *             dgamma_k (this rank's part; all-reduce it).  dgamma_q comes from step (1) (this rank's part).
  * Sequences may straddle the cuts; rows of a boundary tile that belong to another rank are masked (P = 0), so nothing
- * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): CP runs the fused backward.
+ * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): the ordered dq~ reduction has not
+ * been verified on a context-parallel plan.
  * Workspace for both backward calls: arachne_workspace_bytes(plan, 1).  A rank may own no tokens (empty shard). */
 int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params,
                            const int32_t* cu_seqlens_host, const int32_t* grids_host,

@@ -146,7 +146,7 @@ def _want(t, name, dtype, shape=None, device="cuda", optional=False):
 
 
 def _want_call(plan, bf16, lse=None, gammas=(), workspace=None, device="cuda"):
-    nhd = (plan.N, plan.H, plan.D)
+    nhd = (plan.N, plan.total_heads, plan.D)
     for name, t in bf16.items():
         _want(t, name, torch.bfloat16, nhd, device)
     if lse is not None:
@@ -202,6 +202,7 @@ class Plan:
             tl_arr = (ctypes.c_int32 * max(len(tl), 1))(*tl)
             _check(_lib.arachne_plan_create_joint(ctypes.byref(self._h), ctypes.byref(self.params), cu_arr, gr_arr, tl_arr))
         self.N, self.H, self.D = self.params.total_tokens, num_heads, head_dim
+        self.total_heads = int(total_heads or num_heads)      # heads in the raw tensors (> H for an Ulysses rank's plan)
 
     def workspace_bytes(self, bwd: bool) -> int:
         return int(_lib.arachne_workspace_bytes(self._h, 1 if bwd else 0))
@@ -212,10 +213,6 @@ class Plan:
     def enable_profiling(self, enable=True):
         _check(_lib.arachne_plan_enable_profiling(self._h, 1 if enable else 0))
 
-    def deterministic_is_fused(self) -> bool:
-        """True when ARACHNE_FLAG_DETERMINISTIC runs bwd_fused_kernel with the ordered dQ~ reduction (5 launches -> 4)."""
-        return self.num_launches(True) == 4
-
     def logit_status(self):
         """(status, tau): arachne_plan_logit_status — ERR_LOGIT_RANGE once a forward without FLAG_WIDE_LOGITS saw tau > 1."""
         tau = ctypes.c_float(0.0)
@@ -223,7 +220,7 @@ class Plan:
 
     def kernel_times(self, bwd: bool):
         """[(timed interval name, mean ms per call)] over the calls recorded since enable_profiling()."""
-        n = 4 if bwd else 2
+        n = 3 if bwd else 2
         ms = (ctypes.c_float * n)()
         calls = ctypes.c_int(0)
         _check(_lib.arachne_plan_kernel_times(self._h, 1 if bwd else 0, ms, n, ctypes.byref(calls)))

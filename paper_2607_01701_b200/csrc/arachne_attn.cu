@@ -13,7 +13,6 @@
 #include <cuda_runtime.h>
 
 #include "../../include/arachne_attn.h"
-#include "bwd.cuh"
 #include "bwd_fused.cuh"
 #include "common.cuh"
 #include "fwd.cuh"
@@ -54,6 +53,7 @@ struct arachne_plan {
   mutable struct arachne_host_ctx* host = nullptr;   // lazily created by the *_host calls (device buffers, streams)
   int cp_rank = -1;   // >= 0: context-parallel plan (arachne_plan_create_cp), this process owns the queries of shard cp_rank
   Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
+  size_t ticket_bytes = 0; // ordered dq~ reduction tickets [H][n_tiles] (ARACHNE_FLAG_DETERMINISTIC), inside the workspace header
   int n_groups = 0;        // num_seqs * num_heads: (sequence, head) groups (dS scaling tables in the workspace header)
   size_t hdr_bytes = 0;    // WsHeader + group tables at the start of every workspace
   unsigned* d_envelope = nullptr;   // sticky: float bits of the largest out-of-envelope logit bound seen (arachne_plan_logit_status)
@@ -62,10 +62,8 @@ struct arachne_plan {
   SeqInfo* d_seqs = nullptr;
   int* d_tile_seq = nullptr;
   TokInfo* d_tok_info = nullptr;
-  WorkItem* d_items = nullptr;
   WorkItem* d_dyn_items = nullptr;      // the global LPT-ordered lists (dynamic distribution in fwd_kernel / bwd_fused_kernel)
   WorkItem* d_dyn_fwd_items = nullptr;
-  int* d_item_ptr = nullptr;
   int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
   unsigned long long* d_cta_trace = nullptr;   // [2][kTraceMaxCtas][2] globaltimer ns (arachne_plan_cta_times)
@@ -77,7 +75,7 @@ struct arachne_plan {
   // optional per-kernel timing (arachne_plan_enable_profiling): ring of kProfSlots calls per pass,
   // kernels+1 events per call, recorded on the caller's stream (no synchronisation).
   static constexpr int kProfSlots = 32;
-  static constexpr int kMaxKernels = 4;
+  static constexpr int kMaxKernels = 3;
   bool profiling = false;
   mutable long long prof_calls[2] = {0, 0};
   cudaEvent_t prof_ev[2][kProfSlots][kMaxKernels + 1] = {};
@@ -92,8 +90,6 @@ namespace {
 template <int D>
 int configure_kernels() {
   ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
-  ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
-  ARACHNE_CUDA(cudaFuncSetAttribute(bwd_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<D>::kSmemBytes));
   ARACHNE_CUDA(cudaFuncSetAttribute(bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdFusedCfg<D>::kSmemBytes));
   return ARACHNE_OK;
 }
@@ -115,7 +111,7 @@ ProblemDesc per_call_desc(const arachne_plan* pl, void* ws) {
   pd.work_counter = hdr->work_counter;
   pd.dq_error = &hdr->dq_error;
   pd.grp_stats = reinterpret_cast<unsigned*>(w + sizeof(WsHeader));
-  pd.grp_sk = reinterpret_cast<float*>(w + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16);
+  pd.grp_sk = reinterpret_cast<float*>(w + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16 + pl->ticket_bytes);
   return pd;
 }
 
@@ -173,45 +169,38 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
   if (cp) b.gk_t = cp_gk;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
+  // ordered-reduction tickets [H][n_tiles], between the group maxima and the sk table (zeroed with them)
+  unsigned* tickets = reinterpret_cast<unsigned*>(static_cast<uint8_t*>(ws) + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16);
   PrepParams pp{};
   pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse;
   pp.gamma_q = gq; pp.gamma_k = gk;
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // the forward's operand images, bit for bit
-  pp.gq_zero = deterministic ? nullptr : b.gq_t;
+  pp.gq_zero = b.gq_t;
   prof_mark(pl, 1, 0, st);
-  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16, st));   // header + group maxima
+  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16 + pl->ticket_bytes, st));   // header, group maxima, tickets
   prep_kernel<D, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
   const int grid = pl->n_ctas;
-  if (deterministic) {
-    // two-pass (7 GEMM) path: every output tile owned by one CTA, fixed summation order
-    BwdParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv};
-    bwd_kernel<D, false><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pd, bp, 1);
-    ARACHNE_CUDA(cudaGetLastError());
-    prof_mark(pl, 1, 2, st);
-    bwd_kernel<D, true><<<grid, 192, BwdCfg<D>::kSmemBytes, st>>>(pd, bp, 2);
-    ARACHNE_CUDA(cudaGetLastError());
-    prof_mark(pl, 1, 3, st);
-  } else {
-    // fused single-pass (5 GEMM) path: dQ~ partial tiles reduce-added at L2 (order not fixed)
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv};
+  {
+    // fused single-pass (5 GEMM) kernel: dQ~ partial tiles reduce-added at L2 — in arrival order by default, in a fixed
+    // order (tickets) with ARACHNE_FLAG_DETERMINISTIC
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? tickets : nullptr};
     if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
-    prof_mark(pl, 1, 3, st);
   }
-  PostParams po{b.gq_t, deterministic ? 0 : 1, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
+  PostParams po{b.gq_t, 1, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
   post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
     dgamma_reduce_kernel<D><<<2, 256, 0, st>>>(dgpart, pl->post_blocks, dgq, dgk);
     ARACHNE_CUDA(cudaGetLastError());
   }
-  prof_mark(pl, 1, 4, st);
+  prof_mark(pl, 1, 3, st);
   if (pl->profiling) pl->prof_calls[1]++;
   return ARACHNE_OK;
 }
@@ -368,34 +357,41 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
   // fwd_kernel and bwd_fused_kernel take the items of these LPT-ordered lists DYNAMICALLY (an atomic counter, sm100.cuh
   // ItemRing): list scheduling in decreasing-cost order, and CTAs that are a little faster simply take more items.
-  // The deterministic two-pass kernels keep a STATIC LPT assignment: each item goes to the least-loaded CTA (ties: lowest
-  // index — while costs are equal this is round-robin, so CTAs running side by side stay on adjacent tiles of the same
-  // (sequence, head) group), and every CTA's items are stored contiguously.
-  auto deal = [&](std::vector<WorkItem>& list, int n_cta, auto cost, std::vector<int>& ptr) {
-    if (n_cta == 0) { ptr.assign(1, 0); return; }
-    std::vector<long long> load(n_cta, 0);
-    std::vector<std::vector<WorkItem>> own(n_cta);
-    for (const WorkItem& w : list) {
-      int best = 0;
-      for (int c = 1; c < n_cta; ++c) if (load[c] < load[best]) best = c;
-      own[best].push_back(w);
-      load[best] += cost(w);
+  std::vector<WorkItem> dyn_items = items, dyn_fwd_items = fwd_items;
+  if ((p.flags & ARACHNE_FLAG_DETERMINISTIC) && !dyn_items.empty()) {
+    // Ordered dq~ reduction (bwd_fused.cuh): the key tiles of one (sequence, head) group add into a query tile one after the
+    // other, so a group of n key tiles cannot finish faster than n hops of ~kHopBudget tile-pair steps each (reduction
+    // issued -> complete -> ticket published -> read by the next CTA).  With all CTAs on ONE group (the default order) the
+    // group has n^2 / n_ctas steps of compute: hop-bound once n < kHopBudget * n_ctas.  So the deterministic list INTERLEAVES
+    // G = ceil(kHopBudget * n_ctas / n) groups round-robin (tile t of each group in turn): consecutive key tiles of a group are
+    // handed out G items apart and every chain has G times the slack.  G must not be larger than needed: G groups keep
+    // G x (Q^, dO, dq~ of one head) live in L2 — measured at 720p: G = 1..2 1040 TFLOP/s, G = 3 967, G = 8 806 with the SM clock
+    // down to 975 MHz (DRAM power); budget 4 is the measured optimum on every workload (profiles/r2_deterministic.md).
+    // Batches follow the LPT group order, so the groups of one batch have (nearly) the same length.
+    constexpr int kHopBudget = 4;
+    std::vector<std::pair<int, int>> groups;           // (sequence, head) in LPT order
+    for (int b : order)
+      if (pl->seqs[b].qt_n > 0)
+        for (int h = 0; h < p.num_heads; ++h) groups.push_back({b, h});
+    const int n_cta_est = std::min<long long>(pl->num_sms, static_cast<long long>(dyn_items.size()));
+    std::vector<WorkItem> inter;
+    inter.reserve(dyn_items.size());
+    for (size_t g0 = 0; g0 < groups.size();) {
+      const int n0 = pl->seqs[groups[g0].first].n_tiles;
+      const size_t G = std::min(groups.size() - g0, static_cast<size_t>(std::max(1, (kHopBudget * n_cta_est + n0 - 1) / n0)));
+      int n_max = 0;
+      for (size_t g = g0; g < g0 + G; ++g) n_max = std::max(n_max, pl->seqs[groups[g].first].n_tiles);
+      for (int t = 0; t < n_max; ++t)
+        for (size_t g = g0; g < g0 + G; ++g)
+          if (t < pl->seqs[groups[g].first].n_tiles) inter.push_back(WorkItem{groups[g].first, groups[g].second, t, 0});
+      g0 += G;
     }
-    list.clear();
-    ptr.assign(1, 0);
-    for (int c = 0; c < n_cta; ++c) {
-      list.insert(list.end(), own[c].begin(), own[c].end());
-      ptr.push_back(static_cast<int>(list.size()));
-    }
-  };
-  std::vector<int> item_ptr;
-  std::vector<WorkItem> dyn_items = items, dyn_fwd_items = fwd_items;     // before the static deal: global LPT order
+    dyn_items.swap(inter);
+  }
   if (dyn_items.empty()) dyn_items.push_back(WorkItem{0, 0, 0, 0});
   if (dyn_fwd_items.empty()) dyn_fwd_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_ctas = std::min(pl->num_sms, pl->n_items);
   pl->n_fwd_ctas = std::min(pl->num_sms, pl->n_fwd_items);
-  deal(items, pl->n_ctas, [&](const WorkItem& w) { return static_cast<long long>(pl->seqs[w.seq].qt_n); }, item_ptr);
-  if (items.empty()) items.push_back(WorkItem{0, 0, 0, 0});          // (a CP rank that owns no queries: nothing is launched)
   // RoPE tables in fp64 -> fp32 (readings R4, R5)
   std::vector<float2> tab;
   RopeDesc rd{};
@@ -433,24 +429,22 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     }
     PLAN_UP(pl->d_tok_info, ti, TokInfo)
   }
-  PLAN_UP(pl->d_items, items, WorkItem)
   PLAN_UP(pl->d_dyn_items, dyn_items, WorkItem)
   PLAN_UP(pl->d_dyn_fwd_items, dyn_fwd_items, WorkItem)
-  PLAN_UP(pl->d_item_ptr, item_ptr, int)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_envelope), sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
   if ((e = cudaMemset(pl->d_envelope, 0, sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
   if (pl->num_sms <= kTraceMaxCtas) {
-    if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
-    if ((e = cudaMemset(pl->d_cta_trace, 0, 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
+    if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 4 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
+    if ((e = cudaMemset(pl->d_cta_trace, 0, 4 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
   }
   int rc = p.head_dim == 128 ? configure_kernels<128>() : configure_kernels<64>();
   if (rc != ARACHNE_OK) { arachne_plan_destroy(pl); return rc; }
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.items = pl->d_items; pd.item_ptr = pl->d_item_ptr; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.cta_trace = pl->d_cta_trace;   // stats, counters, group tables: per call (per_call_desc)
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.cta_trace = pl->d_cta_trace;   // stats, counters, group tables: per call (per_call_desc)
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -477,7 +471,8 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
   }
   pl->n_groups = p.num_seqs * p.num_heads;
-  pl->hdr_bytes = align_up(sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * (16 + 8), 1024);
+  pl->ticket_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * sizeof(unsigned), 16);
+  pl->hdr_bytes = align_up(sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * (16 + 8) + pl->ticket_bytes, 1024);
   {
     // Envelope (reading R19): north_star's gates are claimed for tau = softmax_scale*sqrt(D)*|gamma_q|inf*|gamma_k|inf
     // <= 1 (every BASELINE.json config has tau = 1).  The forward's logit bound in log2 units is tau*sqrt(D)*log2(e).
@@ -496,7 +491,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_items); cudaFree(pl->d_item_ptr); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_envelope); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_envelope); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
   delete pl;
 }
 
@@ -510,25 +505,24 @@ size_t arachne_workspace_bytes(const arachne_plan* pl, int pass) {
 int arachne_num_launches(const arachne_plan* pl, int pass) {
   if (!pl) return 0;
   if (pass == 0) return 2;                                              // prep_kernel, fwd_kernel
-  if (pass == 1) return (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) ? 5  // prep, bwd_scale, dK/dV pass, dQ pass, post
-                                                                   : 4; // prep, bwd_scale, bwd_fused, post
+  if (pass == 1) return 4;                                              // prep, bwd_scale, bwd_fused, post
   return 0;
 }
 
-static int num_timed_intervals(int pass) { return pass == 0 ? 2 : (pass == 1 ? 4 : 0); }
+static int num_timed_intervals(int pass) { return pass == 0 ? 2 : (pass == 1 ? 3 : 0); }
 
 const char* arachne_kernel_name(int pass, int idx) {
   static const char* fwd[] = {"prep_kernel(fwd: RMSNorm+RoPE -> fp16 tiles)", "fwd_kernel"};
-  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> fp16 tiles, delta) + bwd_scale_kernel", "bwd_main(fused 5-GEMM | det: dKdV pass)",
-                              "bwd_second(det only: dQ pass)", "post_kernel(un-RoPE + RMSNorm bwd)"};
+  static const char* bwd[] = {"prep_kernel(bwd: RMSNorm+RoPE -> fp16 tiles, delta) + bwd_scale_kernel", "bwd_fused_kernel",
+                              "post_kernel(un-RoPE + RMSNorm bwd)"};
   if (pass == 0 && idx >= 0 && idx < 2) return fwd[idx];
-  if (pass == 1 && idx >= 0 && idx < 4) return bwd[idx];
+  if (pass == 1 && idx >= 0 && idx < 3) return bwd[idx];
   return "";
 }
 
 int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us, double* end_us, int n, int* n_ctas) {
   if (!pl || !start_us || !end_us || !n_ctas) return ARACHNE_ERR_NULL_POINTER;
-  if (kernel < 0 || kernel > 1 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
+  if (kernel < 0 || kernel > 3 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
   const int ctas = kernel == 0 ? pl->n_fwd_ctas : pl->n_ctas;
   if (n < ctas) return ARACHNE_ERR_BAD_PARAM;
   std::vector<unsigned long long> t(static_cast<size_t>(kTraceMaxCtas) * 2);
@@ -536,6 +530,7 @@ int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us,
                           cudaMemcpyDeviceToHost));
   unsigned long long t0 = ~0ull;
   for (int c = 0; c < ctas; ++c) t0 = std::min(t0, t[2 * c]);
+  if (kernel >= 2) t0 = 0;
   for (int c = 0; c < ctas; ++c) { start_us[c] = (t[2 * c] - t0) * 1e-3; end_us[c] = (t[2 * c + 1] - t0) * 1e-3; }
   *n_ctas = ctas;
   return ARACHNE_OK;

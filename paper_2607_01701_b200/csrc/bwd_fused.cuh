@@ -1,8 +1,7 @@
-// Fused single-pass backward (§8 a6 + a7, default mode): 5 GEMMs per (key tile, query tile) pair,
-// dK/dV accumulated in TMEM across the query loop, dQ~ partial tiles reduced into a blocked fp32
-// accumulator in global memory by the TMA engine (cp.reduce.async.bulk .add.f32 at L2; the order
-// of the additions is not fixed -> run-to-run bit differences; ARACHNE_FLAG_DETERMINISTIC selects
-// the two-pass kernels of bwd.cuh instead).
+// Fused single-pass backward (§8 a6 + a7): 5 GEMMs per (key tile, query tile) pair, dK/dV accumulated in TMEM across
+// the query loop, dQ~ partial tiles reduced into a blocked fp32 accumulator in global memory by the TMA engine
+// (cp.reduce.async.bulk .add.f32 at L2).  Default: the additions land in arrival order -> run-to-run bit differences;
+// ARACHNE_FLAG_DETERMINISTIC: the same kernel with per-query-tile tickets that fix the order ("ordered reduction" below).
 //
 // Work item = (sequence b, head h, 128-row KEY tile).
 // Items are taken DYNAMICALLY from the plan's LPT-ordered list: lane 0 of the producer warp does an atomicAdd on a per-launch
@@ -43,7 +42,35 @@ struct BwdFusedParams {
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
   ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
   float* gv_t;             // nullable (context parallelism): dV PARTIAL fp32 [N,H,D] written instead of dv
+  unsigned* dq_ticket;     // nullable.  ARACHNE_FLAG_DETERMINISTIC: [H][n_tiles] tickets (zeroed per call) that put the
+                           // reduce-adds into every dq~ tile in a FIXED order (see "ordered reduction" below)
 };
+
+// Ordered (deterministic) dq~ reduction.  The L2 reduce-add of fp32 partial tiles is associative only up to rounding, so the
+// default mode is not bit-reproducible.  With tickets, the key tiles of a (sequence, head) group add into a given query tile in
+// ASCENDING key-tile order: the drain leader of key tile t waits until ticket[query tile] == t, issues its chunk reductions,
+// and once cp.async.bulk.wait_group reports them COMPLETE (performed at L2) publishes t + 1.
+//   * No deadlock: key tile t waits only for key tile t - 1 of its group, which the work list hands out EARLIER (one atomic
+//     counter, taken in list order), so the CTA it waits for is resident and itself waits only on lower tiles.
+//   * No cost on the drain's critical path in steady state: the ticket is requested (relaxed load) at the top of the step
+//     and consumed only before the first reduction is issued; publishing is deferred by one tile, when the reductions have
+//     long completed.  What remains is the hop latency between consecutive key tiles of a group (~4 tile-pair steps); the
+//     deterministic work list interleaves groups so that no chain is hop-bound (arachne_attn.cu, kHopBudget).
+// The order depends only on the plan, so results are bit-identical run to run on the same device.
+// Ticket accesses are RELAXED at gpu scope, on purpose.  What orders the reductions is physical: a ticket is stored only after
+// cp.async.bulk.wait_group has reported the reductions COMPLETE (performed at L2, the point of coherence of the atomics), and the
+// next reduction is issued only after the new ticket value has been read.  Release / acquire forms cost a membar per tile on
+// the drain's critical path (measured: +1.9 us per tile pair, 720p backward 402 -> 630 ms) and buy nothing here: generic-proxy
+// fences do not order the bulk (async-proxy) operations anyway.
+__device__ __forceinline__ unsigned ld_relaxed_gpu(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_relaxed_gpu(unsigned* p, unsigned v) {
+  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+
 
 template <int D>
 struct BwdFusedCfg {
@@ -410,6 +437,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     float sc = 0.f;                                                 // softmax_scale / sk of the current item
     float* stage_row = reinterpret_cast<float*>(sStage) + q * 32;   // row q of staging buffer 0; buffer 1 at +128*32
     uint32_t g = 0;
+    // ordered reduction (leader only): tick_p1 / rank_p1 = ticket and rank of the tile being reduced, tick_p2 / rank_p2 = of the
+    // tile before it (not yet published), tick_seen = last value read from tick_p1
+    unsigned* tick_p1 = nullptr; unsigned* tick_p2 = nullptr;
+    unsigned rank_p1 = 0, rank_p2 = 0, tick_seen = 0;
     // chunk = 32 d-columns of the tile (16 KB, contiguous in the blocked global layout).  Two staging
     // buffers alternate; before a buffer is rewritten, the bulk reduce issued from it two chunks ago
     // must have finished READING it (wait_group.read 1 = all but the most recent group).
@@ -427,6 +458,13 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       fence_proxy_async_smem();
       named_bar_sync(1, 128);
       if (leader) {
+        if (chunk == 0 && tick_p1 != nullptr && tick_seen != rank_p1) {
+          // not this tile's turn yet: the key tile before this one (rank - 1) has not published it
+          const unsigned long long t0 = globaltimer_ns();
+          while ((tick_seen = ld_relaxed_gpu(tick_p1)) != rank_p1) {
+            if (globaltimer_ns() - t0 > 4000000000ull) { atomicExch(pd.dq_error, 1u); break; }   // never hang the device
+          }
+        }
         bulk_reduce_add_f32_s2g(gtile + chunk * (kTileRows * 32), sStage + (chunk & 1) * (kTileRows * 32 * 4),
                                 kTileRows * 32 * 4);
         bulk_commit_group();
@@ -440,7 +478,18 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       sc = pd.softmax_scale * pd.grp_sk[(static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2 + 1];
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const int qt = sq.qt_lo + i;
-        float* gtile = bp.gq_blk + (static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt) * (kTileRows * D);
+        const size_t tile_idx = static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt;
+        float* gtile = bp.gq_blk + tile_idx * (kTileRows * D);
+        if (bp.dq_ticket && leader) {
+          // ordered reduction: publish the tile before last (its reductions have completed: all bulk groups but the latest
+          // tile's D/32), then REQUEST this tile's ticket — the load is consumed only just before the first reduction of
+          // the tile is issued (flush_chunk), so its L2 round trip hides behind the wait for dq_full and the staging
+          if (tick_p2) { bulk_wait_group<D / 32>(); st_relaxed_gpu(tick_p2, rank_p2 + 1); }
+          tick_p2 = tick_p1; rank_p2 = rank_p1;
+          tick_p1 = bp.dq_ticket + tile_idx;
+          rank_p1 = static_cast<unsigned>(wi.tile);
+          tick_seen = ld_relaxed_gpu(tick_p1);
+        }
         mbar_wait(dq_full, g & 1);
         tc_fence_after();
         uint32_t v0[32], v1[32];
@@ -459,6 +508,12 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           flush_chunk(v0, 2, gtile);
           flush_chunk(v1, 3, gtile);
         }
+      }
+      if (bp.dq_ticket && leader) {           // end of the item: publish what is still pending
+        bulk_wait_group<0>();
+        if (tick_p2) st_relaxed_gpu(tick_p2, rank_p2 + 1);
+        if (tick_p1) st_relaxed_gpu(tick_p1, rank_p1 + 1);
+        tick_p1 = tick_p2 = nullptr;
       }
     }
     if (leader) bulk_wait_group<0>();            // all reductions have been performed before the CTA exits

@@ -30,10 +30,10 @@ struct TokInfo {
   uint32_t seq;      // sequence index
 };
 
-// One unit of work for every persistent kernel: (sequence, head, 128-token tile of that sequence).
-// Forward / dQ kernels read it as a QUERY tile, the dK/dV kernel as a KEY tile.  The host orders
-// the list longest-processing-time-first by (sequence, head) group, tiles of a group adjacent, then deals the items
-// to the persistent CTAs greedily (each item to the least-loaded CTA) and stores every CTA's items contiguously.
+// One unit of work for the persistent kernels: (sequence, head, 128-token tile of that sequence).
+// fwd_kernel reads it as a (pair of) QUERY tile(s), bwd_fused_kernel as a KEY tile.  The host orders the lists
+// longest-processing-time-first by (sequence, head) group, tiles of a group adjacent (the deterministic backward list
+// interleaves a few groups: arachne_attn.cu); the CTAs take the items dynamically through an atomic counter.
 struct WorkItem {
   int seq;
   int head;
@@ -105,12 +105,10 @@ struct ProblemDesc {
   const SeqInfo* seqs;
   const int* tile_seq;       // [n_tiles_total] tile -> sequence
   const TokInfo* tok_info;   // [N]
-  const WorkItem* items;     // [n_items]  (n_items = n_tiles_total * H)
   int n_fwd_items;
-  const WorkItem* dyn_items;     // [n_items] the same items in the global LPT order, taken dynamically (work_counter)
+  const WorkItem* dyn_items;     // [n_items] backward items (key tiles) in the global LPT order, taken dynamically (work_counter)
   const WorkItem* dyn_fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
   int* work_counter;             // [2] next index into dyn_fwd_items / dyn_items; zeroed by the host before each launch
-  const int* item_ptr;       // [n_ctas + 1] CTA c owns items [item_ptr[c], item_ptr[c+1]) (host LPT assignment)
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel.  stats,
                              // work_counter, grp_stats and grp_sk live in the header of the CALLER'S workspace (WsHeader below),
                              // i.e. they are per call: two calls on one plan with different workspaces do not share them
