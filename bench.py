@@ -210,7 +210,7 @@ class Env:
         return float(tt.item())
 
 
-def time_workload(env: Env, workload, steps, warmup, deterministic=False, order="listed", seed_offset=0, heads=0, keep=False):
+def time_workload(env: Env, workload, steps, warmup, deterministic=False, order="listed", seed_offset=0, heads=0, keep=False, extra_flags=0):
     """W untimed + K timed steps of `workload` (device-resident inputs; every rank its own batch of the same structure).
     Returns the measurement dict (and, with keep, the live objects for the e2e / cpu_baseline legs)."""
     torch = env.torch
@@ -223,7 +223,7 @@ def time_workload(env: Env, workload, steps, warmup, deterministic=False, order=
     t = {k: inputs.randn_bf16((st["N"], st["H"], st["D"]), inputs.BASE_SEED + 16 * st["index"] + tid + 1000 * env.rank, env.dev)
          for tid, k in ((1, "q"), (2, "k"), (3, "v"), (4, "dO"))}
     t_plan = time.perf_counter()
-    plan = binding.plan_for(st, flags=binding.FLAG_DETERMINISTIC if deterministic else 0)
+    plan = binding.plan_for(st, flags=(binding.FLAG_DETERMINISTIC if deterministic else 0) | extra_flags)
     plan_ms = 1e3 * (time.perf_counter() - t_plan)      # host: validation, work lists, LPT order, RoPE / token tables, upload (not in the step)
     ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device=env.dev)
     o = torch.empty_like(t["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device=env.dev)
@@ -302,6 +302,7 @@ def main():
     ap.add_argument("--no-targets", action="store_true", help="skip the extra legs (heavytail, deterministic) of config.targets")
     ap.add_argument("--order", default="listed", choices=["listed", "reversed", "shuffled"])
     ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC backward as the main measurement")
+    ap.add_argument("--fwd-pairs", action="store_true", help="ARACHNE_FLAG_FWD_CTA_PAIRS: the CTA-pair (cta_group::2) forward kernel (A/B)")
     ap.add_argument("--heads", type=int, default=0, help="override the head count: the per-rank share of a Ulysses group of degree H/heads")
     ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
     ap.add_argument("--sp", default="none", choices=["none", "ulysses", "cp"],
@@ -324,7 +325,8 @@ def main():
     # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
     # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
     r = time_workload(env, args.workload, args.steps, args.warmup, deterministic=args.deterministic, order=args.order,
-                      seed_offset=args.seed_offset, heads=args.heads, keep=True)
+                      seed_offset=args.seed_offset, heads=args.heads, keep=True,
+                      extra_flags=binding.FLAG_FWD_CTA_PAIRS if args.fwd_pairs else 0)
     r["world"] = env.world
     st, plan, t, flops = r["st"], r["plan"], r["t"], r["flops"]
     s2 = flops / (14.0 * st["D"] * st["H"])

@@ -66,6 +66,9 @@ struct arachne_plan {
   WorkItem* d_dyn_fwd_items = nullptr;
   int n_ctas = 0, n_fwd_ctas = 0;
   int n_fwd_items = 0;
+  WorkItem* d_dyn_fwd_pair_items = nullptr;   // forward, CTA-pair form: items of up to four query tiles
+  int n_fwd_pair_items = 0, n_fwd_pair_ctas = 0;
+  bool fwd_pairs = false;               // D = 128 and ARACHNE_FLAG_FWD_CTA_PAIRS: fwd_pair_kernel
   unsigned long long* d_cta_trace = nullptr;   // [2][kTraceMaxCtas][2] globaltimer ns (arachne_plan_cta_times)
   float2* d_rope = nullptr;
   ProblemDesc pd{};
@@ -90,6 +93,8 @@ namespace {
 template <int D>
 int configure_kernels() {
   ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
+  if constexpr (D == 128)
+    ARACHNE_CUDA(cudaFuncSetAttribute(fwd_pair_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D, true>::kSmemBytes));
   ARACHNE_CUDA(cudaFuncSetAttribute(bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdFusedCfg<D>::kSmemBytes));
   return ARACHNE_OK;
 }
@@ -139,6 +144,16 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
   FwdParams fp{f.qt, f.kt, f.vt, o, lse, pl->d_envelope, pl->bound_limit};
+  if constexpr (D == 128) {
+    if (pl->fwd_pairs) {      // CTA-pair form (cluster of 2, cta_group::2): grid = 2 CTAs per pair
+      if (pl->n_fwd_pair_ctas > 0)
+        fwd_pair_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, true>::kThreads, FwdCfg<D, true>::kSmemBytes, st>>>(pd, fp);
+      ARACHNE_CUDA(cudaGetLastError());
+      prof_mark(pl, 0, 2, st);
+      if (pl->profiling) pl->prof_calls[0]++;
+      return ARACHNE_OK;
+    }
+  }
   const int grid = pl->n_fwd_ctas;
   if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp);   // (a CP rank may own no queries)
   ARACHNE_CUDA(cudaGetLastError());
@@ -281,7 +296,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
   if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
-      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~15))
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~31))
     return ARACHNE_ERR_BAD_PARAM;
   {
     // envelope (reading R19): an explicit softmax_scale above 1/sqrt(D) widens the logits beyond what the gates are claimed for
@@ -353,6 +368,16 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     for (int h = 0; h < p.num_heads; ++h)
       for (int t = pl->seqs[b].qt_lo; t < pl->seqs[b].qt_lo + pl->seqs[b].qt_n; t += 2)
         fwd_items.push_back(WorkItem{b, h, t, std::min(2, pl->seqs[b].qt_lo + pl->seqs[b].qt_n - t)});
+  // CTA-pair forward: items of up to FOUR adjacent query tiles (two per CTA of the pair), same group order
+  std::vector<WorkItem> fwd_pair_items;
+  for (int b : order)
+    for (int h = 0; h < p.num_heads; ++h)
+      for (int t = pl->seqs[b].qt_lo; t < pl->seqs[b].qt_lo + pl->seqs[b].qt_n; t += 4)
+        fwd_pair_items.push_back(WorkItem{b, h, t, std::min(4, pl->seqs[b].qt_lo + pl->seqs[b].qt_n - t)});
+  pl->n_fwd_pair_items = static_cast<int>(fwd_pair_items.size());
+  pl->n_fwd_pair_ctas = 2 * std::min(pl->num_sms / 2, pl->n_fwd_pair_items);
+  pl->fwd_pairs = p.head_dim == 128 && (p.flags & ARACHNE_FLAG_FWD_CTA_PAIRS) != 0;
+  if (fwd_pair_items.empty()) fwd_pair_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_items = static_cast<int>(items.size());
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
   // fwd_kernel and bwd_fused_kernel take the items of these LPT-ordered lists DYNAMICALLY (an atomic counter, sm100.cuh
@@ -431,20 +456,21 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   PLAN_UP(pl->d_dyn_items, dyn_items, WorkItem)
   PLAN_UP(pl->d_dyn_fwd_items, dyn_fwd_items, WorkItem)
+  PLAN_UP(pl->d_dyn_fwd_pair_items, fwd_pair_items, WorkItem)
   PLAN_UP(pl->d_rope, tab, float2)
 #undef PLAN_UP
   if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_envelope), sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMalloc");
   if ((e = cudaMemset(pl->d_envelope, 0, sizeof(unsigned))) != cudaSuccess) return fail(e, "cudaMemset");
   if (pl->num_sms <= kTraceMaxCtas) {
-    if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 4 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
-    if ((e = cudaMemset(pl->d_cta_trace, 0, 4 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
+    if ((e = cudaMalloc(reinterpret_cast<void**>(&pl->d_cta_trace), 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMalloc");
+    if ((e = cudaMemset(pl->d_cta_trace, 0, 2 * kTraceMaxCtas * 2 * sizeof(unsigned long long))) != cudaSuccess) return fail(e, "cudaMemset");
   }
   int rc = p.head_dim == 128 ? configure_kernels<128>() : configure_kernels<64>();
   if (rc != ARACHNE_OK) { arachne_plan_destroy(pl); return rc; }
 
   rd.tab = pl->d_rope;
   ProblemDesc& pd = pl->pd;
-  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.cta_trace = pl->d_cta_trace;   // stats, counters, group tables: per call (per_call_desc)
+  pd.seqs = pl->d_seqs; pd.tile_seq = pl->d_tile_seq; pd.tok_info = pl->d_tok_info; pd.dyn_items = pl->d_dyn_items; pd.dyn_fwd_items = pl->d_dyn_fwd_items; pd.n_fwd_items = pl->n_fwd_items; pd.dyn_fwd_pair_items = pl->d_dyn_fwd_pair_items; pd.n_fwd_pair_items = pl->n_fwd_pair_items; pd.cta_trace = pl->d_cta_trace;   // stats, counters, group tables: per call (per_call_desc)
   pd.n_items = pl->n_items; pd.n_tiles_total = pl->n_tiles_total; pd.num_seqs = p.num_seqs;
   pd.N = p.total_tokens; pd.H = p.num_heads;
   pd.eps = p.rms_eps; pd.softmax_scale = pl->p.softmax_scale;
@@ -491,7 +517,7 @@ void arachne_plan_destroy(arachne_plan* pl) {
     for (auto& slot : pass)
       for (cudaEvent_t ev : slot)
         if (ev) cudaEventDestroy(ev);
-  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_envelope); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
+  cudaFree(pl->d_seqs); cudaFree(pl->d_tile_seq); cudaFree(pl->d_tok_info); cudaFree(pl->d_dyn_items); cudaFree(pl->d_dyn_fwd_items); cudaFree(pl->d_dyn_fwd_pair_items); cudaFree(pl->d_envelope); cudaFree(pl->d_cta_trace); cudaFree(pl->d_rope);
   delete pl;
 }
 
@@ -522,15 +548,14 @@ const char* arachne_kernel_name(int pass, int idx) {
 
 int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us, double* end_us, int n, int* n_ctas) {
   if (!pl || !start_us || !end_us || !n_ctas) return ARACHNE_ERR_NULL_POINTER;
-  if (kernel < 0 || kernel > 3 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
-  const int ctas = kernel == 0 ? pl->n_fwd_ctas : pl->n_ctas;
+  if (kernel < 0 || kernel > 1 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
+  const int ctas = kernel == 0 ? (pl->fwd_pairs ? pl->n_fwd_pair_ctas : pl->n_fwd_ctas) : pl->n_ctas;
   if (n < ctas) return ARACHNE_ERR_BAD_PARAM;
   std::vector<unsigned long long> t(static_cast<size_t>(kTraceMaxCtas) * 2);
   ARACHNE_CUDA(cudaMemcpy(t.data(), pl->d_cta_trace + static_cast<size_t>(kernel) * kTraceMaxCtas * 2, t.size() * sizeof(unsigned long long),
                           cudaMemcpyDeviceToHost));
   unsigned long long t0 = ~0ull;
   for (int c = 0; c < ctas; ++c) t0 = std::min(t0, t[2 * c]);
-  if (kernel >= 2) t0 = 0;
   for (int c = 0; c < ctas; ++c) { start_us[c] = (t[2 * c] - t0) * 1e-3; end_us[c] = (t[2 * c + 1] - t0) * 1e-3; }
   *n_ctas = ctas;
   return ARACHNE_OK;

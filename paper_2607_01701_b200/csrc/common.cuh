@@ -108,6 +108,8 @@ struct ProblemDesc {
   int n_fwd_items;
   const WorkItem* dyn_items;     // [n_items] backward items (key tiles) in the global LPT order, taken dynamically (work_counter)
   const WorkItem* dyn_fwd_items; // [n_fwd_items] forward: pairs of query tiles; .tile = first tile, .pad = tiles in the item (1|2)
+  const WorkItem* dyn_fwd_pair_items;  // [n_fwd_pair_items] forward, CTA-pair form: up to FOUR query tiles (.pad = 1..4)
+  int n_fwd_pair_items;
   int* work_counter;             // [2] next index into dyn_fwd_items / dyn_items; zeroed by the host before each launch
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel.  stats,
                              // work_counter, grp_stats and grp_sk live in the header of the CALLER'S workspace (WsHeader below),

@@ -35,12 +35,21 @@ struct FwdParams {
   float bound_limit;      // logit bound (log2 units) the gates are claimed for; +inf with ARACHNE_FLAG_WIDE_LOGITS
 };
 
-template <int D>
+// kPair = true: the CTA-PAIR form of the kernel (cluster of 2, tcgen05 cta_group::2; D = 128 only).  A pair takes items of up
+// to FOUR query tiles — CTA r of the pair owns tiles 2r, 2r+1 of the item — and shares every K^/V tile: each CTA loads and
+// holds only HALF of it (K^: its 64 keys x D; V: all 128 keys x its 64 d-columns), the leader CTA's MMA warp issues M = 256
+// instructions that cover the same-numbered query tile of both CTAs, and completion is multicast to the barriers of both.
+// Per SM this halves the K/V traffic from L2 and the B-operand reads from shared memory (the S GEMM, both operands in shared
+// memory, is otherwise pinned at the 128 B/clk shared-memory limit: DESIGN.md §7).  The peer CTA's warp 9 has no MMAs to
+// issue; it relays "my half has landed" to the leader.  Softmax / epilogue warps are the same code in both forms.
+template <int D, bool kPair = false>
 struct FwdCfg {
+  static_assert(!kPair || D == 128, "the CTA-pair forward is built for head_dim 128 (V's d-halves must be whole 128-byte swizzle blocks)");
   static constexpr int kTileBytes = kTileRows * D * 2;
-  static constexpr int kRing = (D == 128) ? 5 : 8;       // K/V ring slots (K_j, V_j alternate)
-  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * kItemRing;
-  static constexpr int kSmemBytes = kTileBytes * (2 + kRing) + 8 * kNumBars + 16 + 4 * kItemRing;
+  static constexpr int kSlotBytes = kPair ? kTileBytes / 2 : kTileBytes;   // one ring slot: a K^ or V tile (pair: this CTA's half)
+  static constexpr int kRing = kPair ? 8 : ((D == 128) ? 5 : 8);           // K/V ring slots (K_j, V_j alternate)
+  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * kItemRing + (kPair ? 1 + kRing : 0);
+  static constexpr int kSmemBytes = 2 * kTileBytes + kRing * kSlotBytes + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 320;
   // every 4th exp2 on the FMA pipe (ex2_poly3) instead of MUFU: pays at D = 64, where MUFU (16 ex2/clk/SM) is the
   // busiest unit (cogvideox fwd 13.0 vs 14.7 ms); at D = 128 the loop is tensor/power-bound and the extra FMA-pipe
@@ -53,15 +62,16 @@ struct FwdCfg {
 // largest logit bound (log2 units) for which the forward takes the static-max softmax
 constexpr float kStaticMaxBound = 32.0f;
 
-template <int D>
-__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp) {
-  using Cfg = FwdCfg<D>;
+template <int D, bool kPair>
+__device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp) {
+  using Cfg = FwdCfg<D, kPair>;
   constexpr int TILE = Cfg::kTileBytes;
+  constexpr int SLOT = Cfg::kSlotBytes;
   constexpr int RING = Cfg::kRing;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint8_t* sQ = smem;                     // 2 tiles
-  uint8_t* sKV = sQ + 2 * TILE;           // RING tiles
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + RING * TILE);
+  uint8_t* sKV = sQ + 2 * TILE;           // RING slots
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + RING * SLOT);
   uint64_t* q_full = bars;            // producer -> MMA
   uint64_t* q_empty = bars + 1;       // MMA (commit) -> producer
   uint64_t* kv_full = bars + 2;       // [RING]
@@ -72,29 +82,76 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
   uint64_t* o_free = pv_done + 2;        // [2] softmax epilogue (128 arrivals) -> MMA
   uint64_t* it_full = o_free + 2;        // [kItemRing] work-item ring (sm100.cuh): items are taken dynamically
   uint64_t* it_empty = it_full + kItemRing;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(it_empty + kItemRing);
+  uint64_t* peer_q_full = it_empty + kItemRing;        // pair, LEADER only: the peer's Q^ tiles / K,V halves have landed
+  uint64_t* peer_kv_full = peer_q_full + 1;            //   [RING]  (arrived remotely by the peer's relay warp)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(it_empty + kItemRing + (kPair ? 1 + RING : 0));
   int* sItem = reinterpret_cast<int*>(tmem_slot + 1);
   const ItemRing item_ring{sItem, it_full, it_empty};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = kPair ? cluster_ctarank() : 0u;      // 0 = leader (issues the MMAs, owns the barriers the MMA warp waits on)
+  // arrivals of the softmax / epilogue warps on a barrier the MMA warp waits on: 1-CTA form = every thread arrives (count 128);
+  // pair form = one arrival per warp on the LEADER's barrier (count 4 local + 4 remote warps)
+  constexpr uint32_t kArrivals = kPair ? 8 : 128;
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();   // tile images need 1024-byte alignment (128B swizzle atoms)
     mbar_init(q_full, 1); mbar_init(q_empty, 1);
     for (int s = 0; s < RING; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
     for (int t = 0; t < 2; ++t) {
-      mbar_init(&s_full[t], 1); mbar_init(&p_full[t], 128);
-      mbar_init(&pv_done[t], 1); mbar_init(&o_free[t], 128);
+      mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kArrivals);
+      mbar_init(&pv_done[t], 1); mbar_init(&o_free[t], kArrivals);
     }
-    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], 9); }   // consumers: MMA + 8 softmax warps
+    // item ring consumers: MMA + 8 softmax warps; pair: + the peer's producer, relay and 8 softmax warps (remote arrivals)
+    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], kPair ? 19 : 9); }
+    if constexpr (kPair) {
+      mbar_init(peer_q_full, 1);
+      for (int s = 0; s < RING; ++s) mbar_init(&peer_kv_full[s], 1);
+    }
     fence_mbar_init();
   }
-  if (warp == 9) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
+  if (warp == 9) {
+    if constexpr (kPair) { tmem_alloc2(tmem_slot, 512); tmem_relinquish2(); }
+    else { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
+  }
   tc_fence_before();
-  __syncthreads();
+  if constexpr (kPair) cluster_sync_all(); else __syncthreads();      // (pair: barrier inits visible to the peer's remote arrivals)
   if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2] = globaltimer_ns();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
   const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
+  const WorkItem* item_list = kPair ? pd.dyn_fwd_pair_items : pd.dyn_fwd_items;
+  const int n_list = kPair ? pd.n_fwd_pair_items : pd.n_fwd_items;
+  auto wait = [](uint64_t* bar, uint32_t parity) { if constexpr (kPair) mbar_wait_wd(bar, parity); else mbar_wait(bar, parity); };
+  // item hand-out.  1-CTA: sm100.cuh ItemRing.  Pair: the LEADER's producer takes the index and publishes it to both CTAs'
+  // rings; every consumer warp of both CTAs releases the slot on the LEADER's `empty` barrier.
+  auto fetch_producer = [&](uint32_t it) -> int {
+    if constexpr (!kPair) return item_fetch_producer(item_ring, it, pd.work_counter, n_list, lane);
+    const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
+    int item = 0;
+    if (lane == 0) {
+      mbar_wait_wd(&it_empty[s], ph ^ 1);
+      item = atomicAdd(pd.work_counter, 1);
+      if (item >= n_list) item = -1;
+      sItem[s] = item;
+      st_cluster_u32(mapa_u32(smem_u32(&sItem[s]), 1), static_cast<uint32_t>(item));
+      mbar_arrive(&it_full[s]);
+      mbar_arrive_cluster(mapa_u32(smem_u32(&it_full[s]), 1));     // release.cluster: the peer sees the slot write
+    }
+    return __shfl_sync(0xffffffffu, item, 0);
+  };
+  auto fetch_consumer = [&](uint32_t it) -> int {
+    if constexpr (!kPair) return item_fetch_consumer(item_ring, it, lane);
+    const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
+    mbar_wait_wd(&it_full[s], ph);
+    const int item = sItem[s];
+    __syncwarp();
+    if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&it_empty[s]), 0));
+    return item;
+  };
+  // number of query tiles each CTA works on in this item (pair: both CTAs run the same count; tiles beyond the item's
+  // last one are PHANTOMS — a copy of the last real tile whose rows are never stored — because an M = 256 instruction always
+  // covers both CTAs)
+  auto tiles_per_cta = [](const WorkItem& wi) { return kPair ? min(2, wi.pad) : wi.pad; };
 
   if (warp == 8) {
     // ------------------------------------------------------------------ producer
@@ -105,89 +162,129 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     }
     uint32_t it = 0, ring = 0;
     for (;; ++it) {
-      const int item = item_fetch_producer(item_ring, it, pd.work_counter, pd.n_fwd_items, lane);
+      const int item = (rank == 0) ? fetch_producer(it) : fetch_consumer(it);
       if (item < 0) break;
-      const WorkItem wi = pd.dyn_fwd_items[item];
+      const WorkItem wi = item_list[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      const int n_q = wi.pad;
+      const int n_q = tiles_per_cta(wi);
       const uint8_t* hbase_q = fp.qt + wi.head * head_stride;
       const uint8_t* hbase_k = fp.kt + wi.head * head_stride;
       const uint8_t* hbase_v = fp.vt + wi.head * head_stride;
-      mbar_wait(q_empty, (it & 1) ^ 1);
+      wait(q_empty, (it & 1) ^ 1);
       if (lane == 0) {
         mbar_expect_tx(q_full, n_q * TILE);
-        bulk_g2s(sQ, hbase_q + static_cast<size_t>(sq.tile_base + wi.tile) * TILE, n_q * TILE, q_full);
+        if constexpr (!kPair) {
+          bulk_g2s(sQ, hbase_q + static_cast<size_t>(sq.tile_base + wi.tile) * TILE, n_q * TILE, q_full);
+        } else {
+          for (int t = 0; t < n_q; ++t) {      // this CTA's tiles 2*rank + t of the item; phantoms read the item's last tile
+            const int qt = wi.tile + min(static_cast<int>(2 * rank) + t, wi.pad - 1);
+            bulk_g2s(sQ + t * TILE, hbase_q + static_cast<size_t>(sq.tile_base + qt) * TILE, TILE, q_full);
+          }
+        }
       }
       for (int j = 0; j < sq.n_tiles; ++j) {
         const size_t off = static_cast<size_t>(sq.tile_base + j) * TILE;
 #pragma unroll
         for (int kv = 0; kv < 2; ++kv, ++ring) {
           const uint32_t st = ring % RING, ph = (ring / RING) & 1;
-          mbar_wait(&kv_empty[st], ph ^ 1);
+          wait(&kv_empty[st], ph ^ 1);
           if (lane == 0) {
-            mbar_expect_tx(&kv_full[st], TILE);
-            bulk_g2s(sKV + st * TILE, (kv == 0 ? hbase_k : hbase_v) + off, TILE, &kv_full[st]);
+            mbar_expect_tx(&kv_full[st], SLOT);
+            if constexpr (!kPair) {
+              bulk_g2s(sKV + st * SLOT, (kv == 0 ? hbase_k : hbase_v) + off, TILE, &kv_full[st]);
+            } else if (kv == 0) {
+              // K^: this CTA's 64 keys (rows 64*rank..) of each 64-element block -> [D/64][64 rows][128 B]
+#pragma unroll
+              for (int c = 0; c < D / 64; ++c)
+                bulk_g2s(sKV + st * SLOT + c * 8192, hbase_k + off + c * (kTileRows * 128) + rank * 8192, 8192, &kv_full[st]);
+            } else {
+              // V: all 128 keys, this CTA's 64 d-columns = block `rank` of the image (contiguous)
+              bulk_g2s(sKV + st * SLOT, hbase_v + off + rank * (kTileRows * 128), kTileRows * 128, &kv_full[st]);
+            }
           }
         }
         __syncwarp();
+      }
+    }
+  } else if (warp == 9 && rank != 0) {
+    // ------------------------------------------------------------------ pair form, peer CTA: relay "my half has landed"
+    if constexpr (kPair) {
+      uint32_t it = 0, ring = 0;
+      for (;; ++it) {
+        const int item = fetch_consumer(it);
+        if (item < 0) break;
+        const int n_kv = pd.seqs[item_list[item].seq].n_tiles;
+        mbar_wait_wd(q_full, it & 1);
+        if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(peer_q_full), 0));
+        for (int s2 = 0; s2 < 2 * n_kv; ++s2, ++ring) {
+          const uint32_t st = ring % RING, ph = (ring / RING) & 1;
+          mbar_wait_wd(&kv_full[st], ph);
+          if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&peer_kv_full[st]), 0));
+        }
       }
     }
   } else if (warp == 9) {
     // ------------------------------------------------------------------ MMA issuer
     // The whole warp runs the loop convergently (uniform descriptors -> plain UTCHMMA issue, no
     // per-instruction election loop); one elected lane issues the tcgen05 instructions.
-    constexpr uint32_t idesc_s = make_idesc(128, 128, FMT_F16, FMT_F16, MAJOR_K, MAJOR_K);
-    constexpr uint32_t idesc_o = make_idesc(128, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+    constexpr uint32_t M = kPair ? 256 : 128;
+    constexpr uint32_t idesc_s = make_idesc(M, 128, FMT_F16, FMT_F16, MAJOR_K, MAJOR_K);
+    constexpr uint32_t idesc_o = make_idesc(M, D, FMT_BF16, FMT_BF16, MAJOR_K, MAJOR_MN);
+    constexpr uint32_t KBLK = kPair ? 64 * 128 : kTileRows * 128;     // bytes of one 64-element block of a K^ slot
     const uint32_t aQ = smem_u32(sQ), aKV = smem_u32(sKV);
+    auto mma_ss = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) { if constexpr (kPair) umma_ss2(d, a, b, idesc, acc); else umma_ss(d, a, b, idesc, acc); };
+    auto mma_ts = [](uint32_t d, uint32_t a, uint64_t b, uint32_t idesc, uint32_t acc) { if constexpr (kPair) umma_ts2(d, a, b, idesc, acc); else umma_ts(d, a, b, idesc, acc); };
+    auto commit = [](uint64_t* bar) { if constexpr (kPair) umma_commit2(bar); else umma_commit(bar); };
     uint32_t it = 0, ring = 0;      // ring: slot counter at K_0 of the current item (K_j = ring+2j, V_j = ring+2j+1)
     uint32_t cnt[2] = {0, 0};       // per query tile: number of PV tiles issued so far
     for (;; ++it) {
-      const int item = item_fetch_consumer(item_ring, it, lane);
+      const int item = fetch_consumer(it);
       if (item < 0) break;
-      const WorkItem wi = pd.dyn_fwd_items[item];
+      const WorkItem wi = item_list[item];
       const int n_kv = pd.seqs[wi.seq].n_tiles;
-      const int n_q = wi.pad;
+      const int n_q = tiles_per_cta(wi);
       // S_t,j : waits K_j on first use, releases the slot (and Q^ after the last tile) on last use
       auto issue_s = [&](int t, int j) {
         const uint32_t r = ring + 2 * j, st = r % RING, ph = (r / RING) & 1;
-        if (t == 0) mbar_wait(&kv_full[st], ph);
+        if (t == 0) { wait(&kv_full[st], ph); if constexpr (kPair) mbar_wait_wd(&peer_kv_full[st], ph); }
         tc_fence_after();
         if (elect_one()) {
           const uint32_t tS = tbase + Cfg::kColS + t * 128;
 #pragma unroll
           for (int kk = 0; kk < D / 16; ++kk) {
             const uint32_t koff = (kk >> 2) * (kTileRows * 128) + (kk & 3) * 32;
-            umma_ss(tS, make_sdesc(aQ + t * TILE + koff, 16, 1024), make_sdesc(aKV + st * TILE + koff, 16, 1024),
-                    idesc_s, kk > 0);
+            const uint32_t boff = (kk >> 2) * KBLK + (kk & 3) * 32;
+            mma_ss(tS, make_sdesc(aQ + t * TILE + koff, 16, 1024), make_sdesc(aKV + st * SLOT + boff, 16, 1024), idesc_s, kk > 0);
           }
-          umma_commit(&s_full[t]);
+          commit(&s_full[t]);
           if (t == n_q - 1) {
-            umma_commit(&kv_empty[st]);
-            if (j == n_kv - 1) umma_commit(q_empty);
+            commit(&kv_empty[st]);
+            if (j == n_kv - 1) commit(q_empty);
           }
         }
         __syncwarp();
       };
       auto issue_pv = [&](int t, int j) {
         const uint32_t r = ring + 2 * j + 1, st = r % RING, ph = (r / RING) & 1;
-        if (t == 0) mbar_wait(&kv_full[st], ph);
-        if (j == 0) mbar_wait(&o_free[t], (it & 1) ^ 1);        // previous item's epilogue has drained O_t
-        mbar_wait(&p_full[t], cnt[t] & 1);
+        if (t == 0) { wait(&kv_full[st], ph); if constexpr (kPair) mbar_wait_wd(&peer_kv_full[st], ph); }
+        if (j == 0) wait(&o_free[t], (it & 1) ^ 1);        // previous item's epilogue has drained O_t
+        wait(&p_full[t], cnt[t] & 1);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t tP = tbase + Cfg::kColS + t * 128, tO = tbase + Cfg::kColO + t * D;
 #pragma unroll
           for (int kk = 0; kk < kTileRows / 16; ++kk) {
-            umma_ts(tO, tP + kk * 8, make_sdesc(aKV + st * TILE + kk * 2048, kTileRows * 128, 1024), idesc_o,
-                    (j > 0 || kk > 0) ? 1u : 0u);
+            mma_ts(tO, tP + kk * 8, make_sdesc(aKV + st * SLOT + kk * 2048, kTileRows * 128, 1024), idesc_o,
+                   (j > 0 || kk > 0) ? 1u : 0u);
           }
-          umma_commit(&pv_done[t]);
-          if (t == n_q - 1) umma_commit(&kv_empty[st]);
+          commit(&pv_done[t]);
+          if (t == n_q - 1) commit(&kv_empty[st]);
         }
         __syncwarp();
         ++cnt[t];
       };
-      mbar_wait(q_full, it & 1);
+      wait(q_full, it & 1);
+      if constexpr (kPair) mbar_wait_wd(peer_q_full, it & 1);
       for (int t = 0; t < n_q; ++t) issue_s(t, 0);
       for (int j = 0; j < n_kv; ++j) {
         for (int t = 0; t < n_q; ++t) {
@@ -212,14 +309,19 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
     // range.  Anything larger (no_norm debug flag, huge gamma) takes the online-softmax path below.
     const float bound = sqrtf(__uint_as_float(pd.stats[0])) * sqrtf(__uint_as_float(pd.stats[1]));
     const bool static_max = bound <= kStaticMaxBound;     // false for NaN / inf
+    // arrival on a barrier the MMA warp waits on, after this thread's TMEM traffic has been fenced
+    auto arrive_mma = [&](uint64_t* bar) {
+      if constexpr (!kPair) { mbar_arrive(bar); }
+      else { __syncwarp(); if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(bar), 0)); }
+    };
     for (;; ++it) {
-      const int item = item_fetch_consumer(item_ring, it, lane);
+      const int item = fetch_consumer(it);
       if (item < 0) break;
-      const WorkItem wi = pd.dyn_fwd_items[item];
+      const WorkItem wi = item_list[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      if (t >= wi.pad) {
+      if (t >= tiles_per_cta(wi)) {
         // odd trailing tile: warps 4-7 sit this item out, but keep the o_free phase in step with `it`
-        mbar_arrive(&o_free[t]);
+        arrive_mma(&o_free[t]);
         continue;
       }
       float m = 0.f, l = 0.f;
@@ -229,7 +331,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
         // (Cfg::kPolyExp; MUFU: 16 ex2/clk/SM = 1024 clk per 128x128 tile).
         float rs0 = 0.f, rs1 = 0.f;
         for (int j = 0; j < sq.n_tiles; ++j, ++g) {
-          mbar_wait(&s_full[t], g & 1);
+          wait(&s_full[t], g & 1);
           tc_fence_after();
           const int valid = sq.len - j * kTileRows;    // keys of this tile that exist
           uint32_t sa[32], sb[32];
@@ -263,13 +365,13 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
           }
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(&p_full[t]);
+          arrive_mma(&p_full[t]);
         }
         l = rs0 + rs1;
       } else {
         m = -INFINITY;
         for (int j = 0; j < sq.n_tiles; ++j, ++g) {
-          mbar_wait(&s_full[t], g & 1);
+          wait(&s_full[t], g & 1);
           tc_fence_after();
           uint32_t su[128];
 #pragma unroll
@@ -307,7 +409,7 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
           l = l * alpha + (rs0 + rs1);
           if (j > 0 && __any_sync(0xffffffffu, bump)) {
             // O += P V of tile g-1 must have completed before O is rescaled
-            mbar_wait(&pv_done[t], (g - 1) & 1);
+            wait(&pv_done[t], (g - 1) & 1);
             tc_fence_after();
 #pragma unroll
             for (int c = 0; c < D / 32; ++c) {
@@ -321,15 +423,16 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
           }
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(&p_full[t]);
+          arrive_mma(&p_full[t]);
         }
       }
       // ---- epilogue: O / l -> bf16, LSE (natural log, reading R9)
-      mbar_wait(&pv_done[t], (g - 1) & 1);
+      wait(&pv_done[t], (g - 1) & 1);
       tc_fence_after();
-      const int n = (wi.tile + t) * kTileRows + row;     // token inside the sequence
+      const int t_item = (kPair ? 2 * static_cast<int>(rank) : 0) + t;     // this tile's place in the item (pair: phantoms beyond wi.pad)
+      const int n = (wi.tile + t_item) * kTileRows + row;     // token inside the sequence
       const int tok_g = sq.tok_start + n;
-      const bool valid_row = n < sq.len && tok_g >= pd.cp_lo && tok_g < pd.cp_hi;   // CP: only this rank's query rows
+      const bool valid_row = t_item < wi.pad && n < sq.len && tok_g >= pd.cp_lo && tok_g < pd.cp_hi;   // CP: only this rank's query rows
       const float inv_l = 1.0f / l;
       __nv_bfloat16* orow = valid_row ? raw_row<__nv_bfloat16>(pd.sh, fp.o, sq.tok_start + n, wi.head, D) : nullptr;
 #pragma unroll
@@ -352,13 +455,25 @@ __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams f
       if (valid_row)
         fp.lse[static_cast<size_t>(wi.head) * pd.N + sq.tok_start + n] = (m + log2f(l)) * 0.6931471805599453f;
       tc_fence_before();
-      mbar_arrive(&o_free[t]);
+      arrive_mma(&o_free[t]);
     }
   }
   tc_fence_before();
-  __syncthreads();
+  if constexpr (kPair) cluster_sync_all(); else __syncthreads();   // (pair: no remote arrival may target a CTA that has exited)
   if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2 + 1] = globaltimer_ns();
-  if (warp == 9) tmem_dealloc(tbase, 512);
+  if (warp == 9) {
+    if constexpr (kPair) tmem_dealloc2(tbase, 512); else tmem_dealloc(tbase, 512);
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp) {
+  fwd_body<D, false>(pd, fp);
+}
+// CTA-pair form: grid = 2 x (number of pairs), static cluster of 2 (the two SMs of a TPC)
+template <int D>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_pair_kernel(ProblemDesc pd, FwdParams fp) {
+  fwd_body<D, true>(pd, fp);
 }
 
 }  // namespace arachne
