@@ -69,3 +69,25 @@ def test_two_processes_one_gpu_ipc_shards(tmp_path, mode):
     port = _free_port()
     mp.spawn(_worker, args=(2, port, mode, str(tmp_path)), nprocs=2, join=True)
     assert (tmp_path / f"ok_{mode}_0").read_text() == "ok" and (tmp_path / f"ok_{mode}_1").read_text() == "ok"
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("sp", ["ulysses", "cp"])
+def test_bench_sp_mode_two_ranks_on_one_gpu(sp):
+    """`bench.py --gpus 2 --sp ulysses|cp` launched the way the driver launches multi-GPU runs (torch.distributed.run).  With one
+    GPU on the box the two ranks share it (gloo barriers, CUDA IPC shards: config.emulated) — a functional check of the
+    strong-scaling mode, not a scaling number."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.join(root, "bench.py"), "--gpus", "2", "--sp", sp, "--workload", "bucket256",
+           "--steps", "2", "--warmup", "3"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=500, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [x for x in out.stdout.splitlines() if x.startswith("{")][-1]
+    d = json.loads(line)
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["value"] > 0
+    assert d["config"]["parallelism"] == f"{sp}2" and d["config"]["emulated"] == (torch.cuda.device_count() < 2)
+    print(sp, round(d["value"], 1), "TFLOP/s", d["config"])

@@ -331,3 +331,19 @@ def test_one_plan_serves_two_streams_with_separate_workspaces():
         assert torch.equal(outs[i]["dk"], ref[i][3]), i
         num = torch.linalg.vector_norm(outs[i]["dq"].float() - ref[i][2].float())
         assert float(num / torch.linalg.vector_norm(ref[i][2].float())) <= 1e-3, i   # dQ: L2 reduce order is free
+
+
+# ------------------------------------------------------------------ the CTA-pair (cta_group::2) forward kernel (opt-in, A/B)
+def test_forward_cta_pairs_against_oracle_and_default(orc):
+    """ARACHNE_FLAG_FWD_CTA_PAIRS: items of up to four query tiles over a cluster of two CTAs that share every K/V tile.
+    Packs with 1, 2, 3, 4 and 5+ query tiles per sequence exercise full pairs, a peer CTA with one real + one phantom tile,
+    and a peer CTA with only phantoms; every output is held to the oracle gates, and O / LSE must equal the one-CTA
+    kernel's bit for bit (same per-row arithmetic; only the instruction shape differs)."""
+    from paper_2607_01701_b200 import binding
+    for grids, H in (([(1, 10, 10), (1, 16, 16), (3, 10, 13), (2, 16, 16), (5, 11, 13)], 3),      # 100, 256, 390, 512, 715 tokens
+                     ([(9, 16, 16), (1, 1, 1), (1, 3, 43)], 2)):                                    # 2304 (18 tiles), 1, 129
+        st = inputs.pack(grids, H, 128, index=4)
+        w, got, t = _full_case(orc, st, flags=binding.FLAG_FWD_CTA_PAIRS)
+        base = pu.run_gpu(st, t, with_bwd=False)
+        assert torch.equal(got["O"], base["O"]) and torch.equal(got["LSE"], base["LSE"])
+        print("fwd pairs:", grids, w)
