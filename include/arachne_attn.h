@@ -66,11 +66,15 @@ enum {
   ARACHNE_FLAG_NO_NORM = 2,          /* debug: skip RMSNorm (x^ = x)                         */
   ARACHNE_FLAG_NO_ROPE = 4,          /* debug: skip RoPE (x~ = x^)                           */
   ARACHNE_FLAG_WIDE_LOGITS = 8,      /* the caller accepts logits outside the verified envelope (below) */
-  ARACHNE_FLAG_FWD_CTA_PAIRS = 16    /* A-B: run the forward as CTA pairs (cluster of 2, tcgen05 cta_group::2; head_dim 128
+  ARACHNE_FLAG_FWD_CTA_PAIRS = 16,   /* A-B: run the forward as CTA pairs (cluster of 2, tcgen05 cta_group::2; head_dim 128
                                         only, ignored otherwise).  Correct (same parity tests) but SLOWER than the default
                                         one-CTA kernel — 720p forward 176 vs 150 ms: the forward loop is bound by the
                                         softmax <-> MMA hand-off latency, which the cross-CTA hops lengthen, not by the
                                         shared-memory operand bandwidth the pairing relieves           */
+  ARACHNE_FLAG_IMAGE_COPIES = 32     /* A-B: the prologue copies V (and dO) into tile images in the workspace, as round 1
+                                        did, instead of the main kernels reading them from the caller's tensors by
+                                        tensor-map TMA (the default for one-shard plans).  Same results
+                                        bit for bit; more HBM traffic and a larger workspace                          */
 };
 
 /* Verified envelope (reading R19).  Q^ and K^ enter the tensor cores as fp16 — the most precise 16-bit

@@ -10,6 +10,7 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "../../include/arachne_attn.h"
@@ -17,6 +18,7 @@
 #include "common.cuh"
 #include "fwd.cuh"
 #include "prep.cuh"
+#include "rawtile.cuh"
 
 using namespace arachne;
 
@@ -69,6 +71,9 @@ struct arachne_plan {
   WorkItem* d_dyn_fwd_pair_items = nullptr;   // forward, CTA-pair form: items of up to four query tiles
   int n_fwd_pair_items = 0, n_fwd_pair_ctas = 0;
   bool fwd_pairs = false;               // D = 128 and ARACHNE_FLAG_FWD_CTA_PAIRS: fwd_pair_kernel
+  bool raw_fwd = false, raw_bwd = false;   // V (fwd) / V and dO (bwd) tiles are read from the raw tensors by tensor-map TMA
+                                           // (rawtile.cuh) instead of being copied into tile images by the prologue
+  int n_img_fwd = 3, n_img_bwd = 4;        // tile-image regions in the forward / backward workspace
   unsigned long long* d_cta_trace = nullptr;   // [2][kTraceMaxCtas][2] globaltimer ns (arachne_plan_cta_times)
   float2* d_rope = nullptr;
   ProblemDesc pd{};
@@ -102,8 +107,44 @@ int configure_kernels() {
 struct FwdWs { uint8_t *qt, *kt, *vt; };
 struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
 
-size_t fwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + 3 * pl->img_bytes; }
-size_t bwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + 4 * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
+size_t fwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + pl->n_img_fwd * pl->img_bytes; }
+size_t bwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
+
+// Tensor maps over a raw [tokens, H_total, D] bf16 tensor (rawtile.cuh): encoded on the host per call (the base pointer is a
+// call argument), ~1 us each, passed to the kernel as __grid_constant__ parameters.  cuTensorMapEncodeTiled is taken from
+// the driver at run time (no link-time dependency on libcuda).
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+int make_raw_maps(const arachne_plan* pl, const void* base, RawMaps* out, RawTensor* rt) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) { g_last_error = "cuTensorMapEncodeTiled not available from the driver"; return ARACHNE_ERR_CUDA; }
+  const cuuint64_t D = static_cast<cuuint64_t>(pl->p.head_dim), Ht = static_cast<cuuint64_t>(pl->sh.H_total);
+  const cuuint64_t dims[3] = {D, Ht, static_cast<cuuint64_t>(pl->p.total_tokens)};
+  const cuuint64_t strides[2] = {D * 2, Ht * D * 2};                 // bytes, dims 1 and 2
+  const cuuint32_t estr[3] = {1, 1, 1};
+  for (int i = 0; i < 2; ++i) {
+    const cuuint32_t box[3] = {64, 1, i == 0 ? static_cast<cuuint32_t>(kTileRows) : 8u};
+    const CUresult r = enc(i == 0 ? &out->tile : &out->rows8, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims,
+                           strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { g_last_error = "cuTensorMapEncodeTiled failed (" + std::to_string(static_cast<int>(r)) + ")"; return ARACHNE_ERR_CUDA; }
+  }
+  rt->base = static_cast<const __nv_bfloat16*>(base);
+  rt->tok_stride = static_cast<long long>(Ht * D);
+  rt->head0 = pl->sh.head_offset;
+  return ARACHNE_OK;
+}
 
 // The first hdr_bytes of every workspace hold the per-call mutable words of the kernels (WsHeader: logit bound, dynamic
 // work counters) and, for the backward, the per-(sequence, head) dS-scaling tables: the plan itself carries no per-launch
@@ -130,8 +171,14 @@ template <int D>
 int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k, const ShardedPtr& v, const float* gq,
                const float* gk, const ShardedPtr& o, float* lse, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws) + pl->hdr_bytes;
-  FwdWs f{w, w + pl->img_bytes, w + 2 * pl->img_bytes};
+  FwdWs f{w, w + pl->img_bytes, pl->raw_fwd ? nullptr : w + 2 * pl->img_bytes};
   const ProblemDesc pd = per_call_desc(pl, ws);
+  RawMaps vmaps{};
+  RawTensor v_raw{};
+  if (pl->raw_fwd) {
+    const int rc = make_raw_maps(pl, v.p[0], &vmaps, &v_raw);
+    if (rc != ARACHNE_OK) return rc;
+  }
   PrepParams pp{};
   pp.q = q; pp.k = k; pp.v = v;
   pp.gamma_q = gq; pp.gamma_k = gk;
@@ -140,14 +187,15 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.stats = pd.stats;
   prof_mark(pl, 0, 0, st);
   ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader), st));
-  prep_kernel<D, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
+  if (pl->raw_fwd) prep_kernel<D, false, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
+  else prep_kernel<D, false, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
-  FwdParams fp{f.qt, f.kt, f.vt, o, lse, pl->d_envelope, pl->bound_limit};
+  FwdParams fp{f.qt, f.kt, f.vt, v_raw, o, lse, pl->d_envelope, pl->bound_limit};
   if constexpr (D == 128) {
     if (pl->fwd_pairs) {      // CTA-pair form (cluster of 2, cta_group::2): grid = 2 CTAs per pair
       if (pl->n_fwd_pair_ctas > 0)
-        fwd_pair_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, true>::kThreads, FwdCfg<D, true>::kSmemBytes, st>>>(pd, fp);
+        fwd_pair_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, true>::kThreads, FwdCfg<D, true>::kSmemBytes, st>>>(pd, fp, vmaps);
       ARACHNE_CUDA(cudaGetLastError());
       prof_mark(pl, 0, 2, st);
       if (pl->profiling) pl->prof_calls[0]++;
@@ -155,7 +203,7 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
     }
   }
   const int grid = pl->n_fwd_ctas;
-  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp);   // (a CP rank may own no queries)
+  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp, vmaps);   // (a CP rank may own no queries)
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
   if (pl->profiling) pl->prof_calls[0]++;
@@ -175,8 +223,17 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   BwdWs b{};
   b.qt = w; w += pl->img_bytes;
   b.kt = w; w += pl->img_bytes;
-  b.vt = w; w += pl->img_bytes;
-  b.dot = w; w += pl->img_bytes;
+  if (!pl->raw_bwd) {
+    b.vt = w; w += pl->img_bytes;
+    b.dot = w; w += pl->img_bytes;
+  }
+  RawMaps vmaps{}, domaps{};
+  RawTensor v_raw{}, do_raw{};
+  if (pl->raw_bwd) {
+    int rc;
+    if ((rc = make_raw_maps(pl, v.p[0], &vmaps, &v_raw)) != ARACHNE_OK || (rc = make_raw_maps(pl, d_o.p[0], &domaps, &do_raw)) != ARACHNE_OK)
+      return rc;
+  }
   b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.delta_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.gk_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
@@ -194,7 +251,8 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.gq_zero = b.gq_t;
   prof_mark(pl, 1, 0, st);
   ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16 + pl->ticket_bytes, st));   // header, group maxima, tickets
-  prep_kernel<D, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
+  if (pl->raw_bwd) prep_kernel<D, true, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
+  else prep_kernel<D, true, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t);
   ARACHNE_CUDA(cudaGetLastError());
@@ -203,8 +261,8 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   {
     // fused single-pass (5 GEMM) kernel: dQ~ partial tiles reduce-added at L2 — in arrival order by default, in a fixed
     // order (tickets) with ARACHNE_FLAG_DETERMINISTIC
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? tickets : nullptr};
-    if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp);
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, v_raw, do_raw, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? tickets : nullptr};
+    if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp, vmaps, domaps);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
   }
@@ -296,7 +354,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
   if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
-      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~31))
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~63))
     return ARACHNE_ERR_BAD_PARAM;
   {
     // envelope (reading R19): an explicit softmax_scale above 1/sqrt(D) widens the logits beyond what the gates are claimed for
@@ -377,6 +435,15 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->n_fwd_pair_items = static_cast<int>(fwd_pair_items.size());
   pl->n_fwd_pair_ctas = 2 * std::min(pl->num_sms / 2, pl->n_fwd_pair_items);
   pl->fwd_pairs = p.head_dim == 128 && (p.flags & ARACHNE_FLAG_FWD_CTA_PAIRS) != 0;
+  // V / dO by tensor-map TMA from the raw tensors: plain (one-shard) plans.  Token-range-sharded tensors (Ulysses, CP) have
+  // tiles that straddle shards and stay on the prologue's gather; so does the CTA-pair forward (it holds half tiles).
+  {
+    const bool raw_ok = num_shards == 1 && !(p.flags & ARACHNE_FLAG_IMAGE_COPIES);
+    pl->raw_fwd = raw_ok && !pl->fwd_pairs;
+    pl->raw_bwd = raw_ok;
+    pl->n_img_fwd = pl->raw_fwd ? 2 : 3;
+    pl->n_img_bwd = pl->raw_bwd ? 2 : 4;
+  }
   if (fwd_pair_items.empty()) fwd_pair_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_items = static_cast<int>(items.size());
   pl->n_fwd_items = static_cast<int>(fwd_items.size());
@@ -720,7 +787,7 @@ template <int D>
 int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const ShardedPtr& gvp, const ShardedPtr& k, const float* gk,
                      const ShardedPtr& dk, const ShardedPtr& dv, float* dgk, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
-  w += pl->hdr_bytes + 4 * pl->img_bytes + 2 * pl->rowvec_bytes;   // same carving as launch_bwd: gk_t, gq_t, dgamma partials
+  w += pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 2 * pl->rowvec_bytes;   // same carving as launch_bwd: gk_t, gq_t, dgamma partials
   float* gk_sum = reinterpret_cast<float*>(w); w += pl->grad_bytes + pl->gradblk_bytes;
   float* dgpart = dgk ? reinterpret_cast<float*>(w) : nullptr;
   const int lo = pl->pd.cp_lo, hi = pl->pd.cp_hi;

@@ -26,6 +26,7 @@
 // reduce-add); 12 producer (cp.async.bulk); 13 MMA issuer (whole warp convergent, elected lane issues).
 #pragma once
 #include "common.cuh"
+#include "rawtile.cuh"
 #include "sm100.cuh"
 
 namespace arachne {
@@ -33,8 +34,9 @@ namespace arachne {
 struct BwdFusedParams {
   const uint8_t* qt;       // Q^' fp16 images (q~ * softmax_scale * log2e)   [H][n_tiles][TILE]
   const uint8_t* kt;       // K^ fp16 images
-  const uint8_t* vt;       // V  bf16 images
-  const uint8_t* dot;      // dO bf16 images
+  const uint8_t* vt;       // V  bf16 images   (only when v_raw.base == nullptr)
+  const uint8_t* dot;      // dO bf16 images   (only when do_raw.base == nullptr)
+  RawTensor v_raw, do_raw; // base != nullptr: V / dO tiles come straight from the raw tensors by tensor-map TMA (rawtile.cuh)
   const float* lse2_t;     // [H][n_tiles][128]  lse*log2e, +inf on pad rows
   const float* delta_t;    // [H][n_tiles][128]
   float* gq_blk;           // in/out: dl/dq~ fp32, blocked [H][n_tiles][D/32][128][32], 16-byte pieces
@@ -112,7 +114,8 @@ __device__ __forceinline__ void bulk_wait_group() {
 }
 
 template <int D>
-__global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFusedParams bp) {
+__global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFusedParams bp, const __grid_constant__ RawMaps vmaps,
+                                                            const __grid_constant__ RawMaps domaps) {
   using Cfg = BwdFusedCfg<D>;
   constexpr int TILE = Cfg::kTileBytes;
   constexpr int QS = Cfg::kQStages, DS = Cfg::kDOStages;
@@ -182,11 +185,17 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       const SeqInfo sq = pd.seqs[wi.seq];
       const size_t hoff = wi.head * head_stride;
       mbar_wait(kv_free, (it & 1) ^ 1);
-      if (lane == 0) {
+      {
         const size_t xoff = hoff + static_cast<size_t>(sq.tile_base + wi.tile) * TILE;
-        mbar_expect_tx(kv_full, 2 * TILE);
-        bulk_g2s(sK, bp.kt + xoff, TILE, kv_full);
-        bulk_g2s(sV, bp.vt + xoff, TILE, kv_full);
+        const bool raw = bp.v_raw.base != nullptr;
+        const int valid = min(kTileRows, sq.len - wi.tile * kTileRows), tok0 = sq.tok_start + wi.tile * kTileRows;
+        const uint32_t vbytes = raw ? raw_tile_stage<D>(sV, bp.v_raw, wi.head, tok0, valid, lane) : TILE;
+        if (lane == 0) {
+          mbar_expect_tx(kv_full, TILE + vbytes);
+          bulk_g2s(sK, bp.kt + xoff, TILE, kv_full);
+          if (raw) raw_tile_issue<D>(sV, vmaps, bp.v_raw, wi.head, tok0, valid, kv_full);
+          else bulk_g2s(sV, bp.vt + xoff, TILE, kv_full);
+        }
       }
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const int qt = sq.qt_lo + i;
@@ -201,7 +210,14 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           bulk_g2s(sDelta + qs * 128, bp.delta_t + roff, 512, &q_full[qs]);
         }
         mbar_wait(&do_empty[ds], dph ^ 1);
-        if (lane == 0) {
+        if (bp.do_raw.base != nullptr) {
+          const int valid = min(kTileRows, sq.len - qt * kTileRows), tok0 = sq.tok_start + qt * kTileRows;
+          const uint32_t bytes = raw_tile_stage<D>(sdO + ds * TILE, bp.do_raw, wi.head, tok0, valid, lane);
+          if (lane == 0) {
+            mbar_expect_tx(&do_full[ds], bytes);
+            raw_tile_issue<D>(sdO + ds * TILE, domaps, bp.do_raw, wi.head, tok0, valid, &do_full[ds]);
+          }
+        } else if (lane == 0) {
           mbar_expect_tx(&do_full[ds], TILE);
           bulk_g2s(sdO + ds * TILE, bp.dot + yoff, TILE, &do_full[ds]);
         }
@@ -343,12 +359,17 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           tmem_wait_ld();
           uint32_t pk[16];
 #pragma unroll
-          for (int c = 0; c < 32; c += 2) {
-            const float2 l2 = *reinterpret_cast<const float2*>(&lse_s[half * 32 + c]);
-            const float p0 = ex2_approx(__uint_as_float(sv[c]) - l2.x);       // S^T is already in the exp2 domain (Q^')
-            const float p1 = ex2_approx(__uint_as_float(sv[c + 1]) - l2.y);
-            p[half * 32 + c] = p0; p[half * 32 + c + 1] = p1;
+          for (int c = 0; c < 32; c += 4) {
+            // lse2 / delta are the same for every thread (broadcast reads): 16-byte loads keep the shared-memory data pipe,
+            // which the tensor core's operand reads already load to ~60 %, as free as possible (profiles/r2_ncu.md)
+            const float4 l4 = *reinterpret_cast<const float4*>(&lse_s[half * 32 + c]);
+            const float p0 = ex2_approx(__uint_as_float(sv[c]) - l4.x);       // S^T is already in the exp2 domain (Q^')
+            const float p1 = ex2_approx(__uint_as_float(sv[c + 1]) - l4.y);
+            const float p2 = ex2_approx(__uint_as_float(sv[c + 2]) - l4.z);
+            const float p3 = ex2_approx(__uint_as_float(sv[c + 3]) - l4.w);
+            p[half * 32 + c] = p0; p[half * 32 + c + 1] = p1; p[half * 32 + c + 2] = p2; p[half * 32 + c + 3] = p3;
             pk[c >> 1] = pack_bf16x2(p0, p1);
+            pk[(c >> 1) + 1] = pack_bf16x2(p2, p3);
           }
           tmem_st16(tS + half * 16, pk);         // P^T (bf16 pairs) over the already-read S^T columns
         }
@@ -368,12 +389,15 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           for (int c8 = 0; c8 < 4; ++c8) {
             uint32_t w[4];
 #pragma unroll
-            for (int e = 0; e < 8; e += 2) {
+            for (int e = 0; e < 8; e += 4) {
               const int c = c8 * 8 + e;
-              const float2 d2 = *reinterpret_cast<const float2*>(&dl_s[half * 32 + c]);
-              const float ds0 = p[half * 32 + c] * fmaf(__uint_as_float(dpv[c]), sk, -d2.x);
-              const float ds1 = p[half * 32 + c + 1] * fmaf(__uint_as_float(dpv[c + 1]), sk, -d2.y);
+              const float4 d4 = *reinterpret_cast<const float4*>(&dl_s[half * 32 + c]);
+              const float ds0 = p[half * 32 + c] * fmaf(__uint_as_float(dpv[c]), sk, -d4.x);
+              const float ds1 = p[half * 32 + c + 1] * fmaf(__uint_as_float(dpv[c + 1]), sk, -d4.y);
+              const float ds2 = p[half * 32 + c + 2] * fmaf(__uint_as_float(dpv[c + 2]), sk, -d4.z);
+              const float ds3 = p[half * 32 + c + 3] * fmaf(__uint_as_float(dpv[c + 3]), sk, -d4.w);
               w[e >> 1] = pack_f16x2(ds0, ds1);
+              w[(e >> 1) + 1] = pack_f16x2(ds2, ds3);
             }
             const uint32_t chunk = half * 4 + c8;
             *reinterpret_cast<uint4*>(dS_row + ((chunk ^ (r & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);

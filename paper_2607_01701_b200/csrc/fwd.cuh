@@ -21,6 +21,7 @@
 // error floor at ~2e-4 instead of ~1.5e-3 for bf16.  P and V are bf16.
 #pragma once
 #include "common.cuh"
+#include "rawtile.cuh"
 #include "sm100.cuh"
 
 namespace arachne {
@@ -28,12 +29,28 @@ namespace arachne {
 struct FwdParams {
   const uint8_t* qt;      // [H][n_tiles][TILE_BYTES]  Q^ fp16 images
   const uint8_t* kt;      // K^ fp16 images
-  const uint8_t* vt;      // V bf16 images
+  const uint8_t* vt;      // V bf16 images (only when v_raw.base == nullptr)
+  RawTensor v_raw;        // base != nullptr: V tiles come straight from the raw tensor by tensor-map TMA (rawtile.cuh)
   ShardedPtr o;           // [N,H_total,D] bf16, possibly sharded by token range (common.cuh)
   float* lse;             // [H,N]
   unsigned* envelope;     // plan-owned sticky word: float bits of the largest logit bound that exceeded bound_limit
   float bound_limit;      // logit bound (log2 units) the gates are claimed for; +inf with ARACHNE_FLAG_WIDE_LOGITS
 };
+
+// A/B switches (profiles/r2_fwd_handoff.md).  kSplitP = number of pieces (1, 2 or 4) in which the softmax hands a tile of P to
+// the MMA warp: with more than one, the first pieces of O += P V run on the tensor pipe while the rest of the row is still
+// being exponentiated (the MUFU time of a tile, 1024 clk, is as long as its two GEMMs; every cycle of the
+// S -> exp -> PV -> S chain that is not overlapped is lost on both units).  kWarpArrive: one mbarrier arrival per softmax
+// WARP (after __syncwarp) instead of one per thread.
+#ifndef ARACHNE_FWD_SPLIT_P
+#define ARACHNE_FWD_SPLIT_P 2
+#endif
+#ifndef ARACHNE_FWD_WARP_ARRIVE
+#define ARACHNE_FWD_WARP_ARRIVE 0
+#endif
+constexpr int kSplitP = ARACHNE_FWD_SPLIT_P;
+static_assert(kSplitP == 1 || kSplitP == 2 || kSplitP == 4, "P is handed over in 1, 2 or 4 pieces of 128 / kSplitP keys");
+constexpr bool kWarpArrive = ARACHNE_FWD_WARP_ARRIVE != 0;
 
 // kPair = true: the CTA-PAIR form of the kernel (cluster of 2, tcgen05 cta_group::2; D = 128 only).  A pair takes items of up
 // to FOUR query tiles — CTA r of the pair owns tiles 2r, 2r+1 of the item — and shares every K^/V tile: each CTA loads and
@@ -48,7 +65,7 @@ struct FwdCfg {
   static constexpr int kTileBytes = kTileRows * D * 2;
   static constexpr int kSlotBytes = kPair ? kTileBytes / 2 : kTileBytes;   // one ring slot: a K^ or V tile (pair: this CTA's half)
   static constexpr int kRing = kPair ? 8 : ((D == 128) ? 5 : 8);           // K/V ring slots (K_j, V_j alternate)
-  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * kItemRing + (kPair ? 1 + kRing : 0);
+  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * (kSplitP - 1) + 2 * kItemRing + (kPair ? 1 + kRing : 0);
   static constexpr int kSmemBytes = 2 * kTileBytes + kRing * kSlotBytes + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 320;
   // every 4th exp2 on the FMA pipe (ex2_poly3) instead of MUFU: pays at D = 64, where MUFU (16 ex2/clk/SM) is the
@@ -63,7 +80,7 @@ struct FwdCfg {
 constexpr float kStaticMaxBound = 32.0f;
 
 template <int D, bool kPair>
-__device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp) {
+__device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp, const RawMaps& vm) {
   using Cfg = FwdCfg<D, kPair>;
   constexpr int TILE = Cfg::kTileBytes;
   constexpr int SLOT = Cfg::kSlotBytes;
@@ -78,7 +95,8 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   uint64_t* kv_empty = kv_full + RING;
   uint64_t* s_full = kv_empty + RING;    // [2] MMA (commit) -> softmax of tile t
   uint64_t* p_full = s_full + 2;         // [2] softmax (128 arrivals) -> MMA
-  uint64_t* pv_done = p_full + 2;        // [2] MMA (commit) -> softmax: one phase per PV
+  uint64_t* pa_full = p_full + 2;        // [2][kSplitP - 1] softmax -> MMA: piece i of P (keys [i, i+1) * 128 / kSplitP) is in TMEM
+  uint64_t* pv_done = pa_full + 2 * (kSplitP - 1);   // [2] MMA (commit) -> softmax: one phase per PV
   uint64_t* o_free = pv_done + 2;        // [2] softmax epilogue (128 arrivals) -> MMA
   uint64_t* it_full = o_free + 2;        // [kItemRing] work-item ring (sm100.cuh): items are taken dynamically
   uint64_t* it_empty = it_full + kItemRing;
@@ -92,13 +110,14 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   const uint32_t rank = kPair ? cluster_ctarank() : 0u;      // 0 = leader (issues the MMAs, owns the barriers the MMA warp waits on)
   // arrivals of the softmax / epilogue warps on a barrier the MMA warp waits on: 1-CTA form = every thread arrives (count 128);
   // pair form = one arrival per warp on the LEADER's barrier (count 4 local + 4 remote warps)
-  constexpr uint32_t kArrivals = kPair ? 8 : 128;
+  constexpr uint32_t kArrivals = kPair ? 8 : (kWarpArrive ? 4 : 128);
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();   // tile images need 1024-byte alignment (128B swizzle atoms)
     mbar_init(q_full, 1); mbar_init(q_empty, 1);
     for (int s = 0; s < RING; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
     for (int t = 0; t < 2; ++t) {
       mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kArrivals);
+      for (int i = 0; i < kSplitP - 1; ++i) mbar_init(&pa_full[t * (kSplitP - 1) + i], kArrivals);
       mbar_init(&pv_done[t], 1); mbar_init(&o_free[t], kArrivals);
     }
     // item ring consumers: MMA + 8 softmax warps; pair: + the peer's producer, relay and 8 softmax warps (remote arrivals)
@@ -188,6 +207,18 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
         for (int kv = 0; kv < 2; ++kv, ++ring) {
           const uint32_t st = ring % RING, ph = (ring / RING) & 1;
           wait(&kv_empty[st], ph ^ 1);
+          if constexpr (!kPair) {
+            if (kv == 1 && fp.v_raw.base != nullptr) {      // V_j straight from the raw tensor (rawtile.cuh)
+              const int valid = min(kTileRows, sq.len - j * kTileRows);
+              const int tok0 = sq.tok_start + j * kTileRows;
+              const uint32_t bytes = raw_tile_stage<D>(sKV + st * SLOT, fp.v_raw, wi.head, tok0, valid, lane);
+              if (lane == 0) {
+                mbar_expect_tx(&kv_full[st], bytes);
+                raw_tile_issue<D>(sKV + st * SLOT, vm, fp.v_raw, wi.head, tok0, valid, &kv_full[st]);
+              }
+              continue;
+            }
+          }
           if (lane == 0) {
             mbar_expect_tx(&kv_full[st], SLOT);
             if constexpr (!kPair) {
@@ -268,19 +299,25 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
         const uint32_t r = ring + 2 * j + 1, st = r % RING, ph = (r / RING) & 1;
         if (t == 0) { wait(&kv_full[st], ph); if constexpr (kPair) mbar_wait_wd(&peer_kv_full[st], ph); }
         if (j == 0) wait(&o_free[t], (it & 1) ^ 1);        // previous item's epilogue has drained O_t
-        wait(&p_full[t], cnt[t] & 1);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint32_t tP = tbase + Cfg::kColS + t * 128, tO = tbase + Cfg::kColO + t * D;
+        const uint32_t tP = tbase + Cfg::kColS + t * 128, tO = tbase + Cfg::kColO + t * D;
+        constexpr int KPP = (kTileRows / 16) / kSplitP;          // K = 16 steps per piece
 #pragma unroll
-          for (int kk = 0; kk < kTileRows / 16; ++kk) {
-            mma_ts(tO, tP + kk * 8, make_sdesc(aKV + st * SLOT + kk * 2048, kTileRows * 128, 1024), idesc_o,
-                   (j > 0 || kk > 0) ? 1u : 0u);
+        for (int piece = 0; piece < kSplitP; ++piece) {
+          // pieces before the last: those keys of P have been stored; their share of O += P V runs while the softmax
+          // finishes the row
+          wait(piece < kSplitP - 1 ? &pa_full[t * (kSplitP - 1) + piece] : &p_full[t], cnt[t] & 1);
+          tc_fence_after();
+          if (elect_one()) {
+#pragma unroll
+            for (int kk = piece * KPP; kk < (piece + 1) * KPP; ++kk)
+              mma_ts(tO, tP + kk * 8, make_sdesc(aKV + st * SLOT + kk * 2048, kTileRows * 128, 1024), idesc_o, (j > 0 || kk > 0) ? 1u : 0u);
+            if (piece == kSplitP - 1) {
+              commit(&pv_done[t]);
+              if (t == n_q - 1) commit(&kv_empty[st]);
+            }
           }
-          commit(&pv_done[t]);
-          if (t == n_q - 1) commit(&kv_empty[st]);
+          __syncwarp();
         }
-        __syncwarp();
         ++cnt[t];
       };
       wait(q_full, it & 1);
@@ -311,8 +348,9 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
     const bool static_max = bound <= kStaticMaxBound;     // false for NaN / inf
     // arrival on a barrier the MMA warp waits on, after this thread's TMEM traffic has been fenced
     auto arrive_mma = [&](uint64_t* bar) {
-      if constexpr (!kPair) { mbar_arrive(bar); }
-      else { __syncwarp(); if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(bar), 0)); }
+      if constexpr (kPair) { __syncwarp(); if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(bar), 0)); }
+      else if constexpr (kWarpArrive) { __syncwarp(); if (lane == 0) mbar_arrive(bar); }
+      else { mbar_arrive(bar); }
     };
     for (;; ++it) {
       const int item = fetch_consumer(it);
@@ -361,6 +399,11 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
               }
             }
             tmem_st16(tS + c * 16, pk);      // P (bf16 pairs) over S columns that have already been read
+            if (kSplitP > 1 && c < 3 && ((c + 1) * kSplitP) % 4 == 0) {      // a piece of P is complete: hand it to the MMA warp now
+              tmem_wait_st();
+              tc_fence_before();
+              arrive_mma(&pa_full[t * (kSplitP - 1) + (c + 1) * kSplitP / 4 - 1]);
+            }
             if (c < 3) tmem_wait_ld();
           }
           tmem_wait_st();
@@ -423,6 +466,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
           }
           tmem_wait_st();
           tc_fence_before();
+          for (int i = 0; i < kSplitP - 1; ++i) arrive_mma(&pa_full[t * (kSplitP - 1) + i]);   // (O may have been rescaled above: no early hand-off on this path)
           arrive_mma(&p_full[t]);
         }
       }
@@ -467,13 +511,14 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
 }
 
 template <int D>
-__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp) {
-  fwd_body<D, false>(pd, fp);
+__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp, const __grid_constant__ RawMaps vmaps) {
+  fwd_body<D, false>(pd, fp, vmaps);
 }
 // CTA-pair form: grid = 2 x (number of pairs), static cluster of 2 (the two SMs of a TPC)
 template <int D>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_pair_kernel(ProblemDesc pd, FwdParams fp) {
-  fwd_body<D, true>(pd, fp);
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_pair_kernel(ProblemDesc pd, FwdParams fp,
+                                                                                         const __grid_constant__ RawMaps vmaps) {
+  fwd_body<D, true>(pd, fp, vmaps);      // (the pair form reads V images; the maps are unused)
 }
 
 }  // namespace arachne

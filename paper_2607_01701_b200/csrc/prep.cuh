@@ -22,8 +22,8 @@ struct PrepParams {
   const float* gamma_k;
   uint8_t* qt;                 // [H][n_tiles][128*D*2]
   uint8_t* kt;
-  uint8_t* vt;
-  uint8_t* dot;                // nullable
+  uint8_t* vt;                 // nullable: no V image (the main kernels read V by tensor-map TMA, rawtile.cuh)
+  uint8_t* dot;                // nullable: forward, or no dO image (same)
   float* lse2_t;               // [H][n_tiles][128]  lse * log2(e); +inf on pad rows
   float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
   float* gq_zero;              // nullable: blocked dq~ accumulator [H][n_tiles][128*D] to clear (fused backward)
@@ -102,7 +102,9 @@ __device__ __forceinline__ float norm_rope8(float (&x)[8], const float (&gam)[8]
   return nrm;
 }
 
-template <int D, bool kBwd>
+// kCopy: also write V (and, backward, dO) tile images — the path of token-range-sharded plans and of ARACHNE_FLAG_IMAGE_COPIES;
+// otherwise the main kernels read those tiles from the raw tensors by tensor-map TMA (rawtile.cuh) and pp.vt / pp.dot are null.
+template <int D, bool kBwd, bool kCopy>
 __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams pp) {
   constexpr int LPR = D / 8, RPW = 32 / LPR;
   constexpr int TILE_BYTES = kTileRows * D * 2;
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     if (valid) {
       if (q_side) uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
       uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src);
-      uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);
+      if (kBwd || kCopy) uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);   // (bwd: |V|^2 bound)
       if (kBwd && q_side) {
         ug = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src);
         uo = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.o, shard) + src);
@@ -159,7 +161,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     const uint32_t ioff = image_off(r, d0);
     if (q_side) *reinterpret_cast<uint4*>(pp.qt + img_off + ioff) = valid ? pack8(xq, FMT_F16) : zero4;   // (eps = 0: 0 * inf)
     *reinterpret_cast<uint4*>(pp.kt + img_off + ioff) = valid ? pack8(xk, FMT_F16) : zero4;
-    *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
+    if (kCopy) *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
     // row norms are only needed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, seg_sum<LPR>(qs)); kn = fmaxf(kn, seg_sum<LPR>(ks)); }
     if (kBwd) {
@@ -170,7 +172,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
       vn = fmaxf(vn, seg_sum<LPR>(v2));
     }
     if (kBwd && q_side) {
-      *reinterpret_cast<uint4*>(pp.dot + img_off + ioff) = ug;
+      if (kCopy) *reinterpret_cast<uint4*>(pp.dot + img_off + ioff) = ug;
       float g[8], oo[8];
       unpack_bf16x8(ug, g);
       unpack_bf16x8(uo, oo);

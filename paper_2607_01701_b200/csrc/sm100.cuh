@@ -114,6 +114,19 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
       "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
       : "memory");
 }
+// Tensor-map TMA: one box of a 3-D tensor map (dims: head_dim elements, heads, tokens) -> shared memory, 128-byte swizzle
+// applied by the engine, completion on an mbarrier.  `tmap` is the generic address of a CUtensorMap (a __grid_constant__
+// kernel parameter here).
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const void* tmap, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n" ::
+          "r"(smem_u32(smem_dst)),
+      "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
+  asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");
+}
 // shared -> global with fp32 add performed at L2 (used for dQ partial tiles)
 __device__ __forceinline__ void bulk_reduce_add_f32_s2g(void* gmem_dst, const void* smem_src,
                                                         uint32_t bytes) {

@@ -347,3 +347,36 @@ def test_forward_cta_pairs_against_oracle_and_default(orc):
         base = pu.run_gpu(st, t, with_bwd=False)
         assert torch.equal(got["O"], base["O"]) and torch.equal(got["LSE"], base["LSE"])
         print("fwd pairs:", grids, w)
+
+
+# ------------------------------------------------------------------ V / dO by tensor-map TMA (default) vs tile-image copies
+@pytest.mark.parametrize("D", [64, 128])
+def test_raw_tma_tiles_equal_image_copies(orc, D):
+    """Default one-shard plans read V (forward, backward) and dO (backward) tiles from the caller's tensors by tensor-map TMA
+    (csrc/rawtile.cuh); ARACHNE_FLAG_IMAGE_COPIES is the round-1 path (the prologue copies them into zero-padded tile images).
+    The bytes that reach shared memory must be the same, so every output must be bit-identical (deterministic backward) —
+    on tails of 5, 2, 8, 123, 127 and 0 rows (whole tiles), i.e. tails below 8 rows, multiples of 8, and both — and a
+    neighbouring sequence full of NaN must not leak into a tail tile.  One case is also held to the oracle."""
+    from paper_2607_01701_b200 import binding
+    grids = [(1, 1, 5), (1, 10, 13), (1, 8, 17), (1, 3, 41), (1, 16, 16), (1, 15, 17)]     # 5, 130, 136, 123, 256, 255 tokens
+    st = inputs.pack(grids, 2, D, index=5)
+    t = inputs.make_inputs(st, device="cuda")
+    raw = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC)
+    img = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC | binding.FLAG_IMAGE_COPIES)
+    assert raw["plan"].workspace_bytes(True) < img["plan"].workspace_bytes(True)      # no V / dO images in the workspace
+    for k in ("O", "LSE", "dQ", "dK", "dV"):
+        assert torch.equal(raw[k], img[k]), k
+    a = _np(t)
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], rope_dims=st["rope_dims"])
+    pu.check_full(st, raw, ref)
+    # NaN in every other sequence's V and dO: the remaining sequences are untouched, bit for bit
+    cu = st["cu_seqlens"]
+    p = {k: v.clone() for k, v in t.items()}
+    for b in (0, 2, 4):
+        p["v"][cu[b]:cu[b + 1]] = float("nan")
+        p["dO"][cu[b]:cu[b + 1]] = float("nan")
+    pois = pu.run_gpu(st, p, flags=binding.FLAG_DETERMINISTIC)
+    for b in (1, 3, 5):
+        for k in ("O", "dQ", "dK", "dV"):
+            assert torch.equal(pois[k][cu[b]:cu[b + 1]], raw[k][cu[b]:cu[b + 1]]), (k, b)
+        assert torch.equal(pois["LSE"][:, cu[b]:cu[b + 1]], raw["LSE"][:, cu[b]:cu[b + 1]]), b
