@@ -107,12 +107,18 @@ typedef struct {
   float rms_eps;          /* added to the mean square, inside the sqrt; 1e-6               */
   float softmax_scale;    /* 0 => 1/sqrt(head_dim)                                         */
   int32_t flags;          /* ARACHNE_FLAG_*                                                */
+  int64_t q_stride;       /* elements between consecutive TOKENS of Q / K / V; 0 => num_heads * head_dim   */
+  int64_t k_stride;       /* (contiguous).  The heads of a token stay adjacent (head stride = head_dim),    */
+  int64_t v_stride;       /* which covers the strided producers there are: a fused QKV projection           */
+                          /* [N, 3, H, D] is three base pointers with stride 3*H*D.  Each must be a         */
+                          /* multiple of 8 and >= num_heads * head_dim; one-shard plans only (sharded       */
+                          /* plans: 0).  O, LSE, dO and the gradients are always contiguous.                */
 } arachne_attn_params;
 
-/* The tensors are CONTIGUOUS [N, H, D]: SURVEY §8(b) sketched optional q/k/v token and head strides; they are not part of
- * this ABI because every raw row is read exactly once by the in-call prologue (prep_kernel), so a strided caller loses
- * nothing by making the tensors contiguous first, and the sharded entry points below already cover the one strided
- * layout the method needs (a head range of a wider [n, total_heads, D] tensor). */
+/* Q, K, V may be token-strided views (q_stride, k_stride, v_stride above): Q and K rows are read once by the
+ * in-call prologue and once by the backward epilogue, V tiles by tensor-map TMA whose token stride is simply the map's.
+ * Everything the library writes (O, LSE, dQ, dK, dV) and dO are contiguous [N, H, D]; the sharded entry points below cover
+ * the other strided layout the method needs (a head range of a wider [n, total_heads, D] tensor). */
 
 typedef struct arachne_plan arachne_plan;
 

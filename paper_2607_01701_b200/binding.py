@@ -39,6 +39,7 @@ class AttnParams(ctypes.Structure):
         ("num_seqs", ctypes.c_int32), ("total_tokens", ctypes.c_int32), ("num_heads", ctypes.c_int32),
         ("head_dim", ctypes.c_int32), ("rope_dims", ctypes.c_int32 * 3), ("rope_theta", ctypes.c_float),
         ("rms_eps", ctypes.c_float), ("softmax_scale", ctypes.c_float), ("flags", ctypes.c_int32),
+        ("q_stride", ctypes.c_int64), ("k_stride", ctypes.c_int64), ("v_stride", ctypes.c_int64),
     ]
 
 
@@ -128,7 +129,7 @@ def _ptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
 
 
-def _want(t, name, dtype, shape=None, device="cuda", optional=False):
+def _want(t, name, dtype, shape=None, device="cuda", optional=False, tok_stride=0):
     """The C side can only check alignment: a non-contiguous view (a slice of a fused QKV projection), a wrong dtype or a
     CPU tensor would silently give wrong results or fault, so the marshalling layer refuses them here."""
     if t is None:
@@ -139,8 +140,12 @@ def _want(t, name, dtype, shape=None, device="cuda", optional=False):
         raise TypeError(f"{name}: expected a {device} tensor, got {t.device}")
     if t.dtype != dtype:
         raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
-    if not t.is_contiguous():
-        raise TypeError(f"{name}: must be contiguous (the ABI takes contiguous [N, H, D] tensors; call .contiguous())")
+    if tok_stride:
+        # a token-strided view declared at plan creation (q_stride / k_stride / v_stride): heads and head_dim stay dense
+        if shape is None or len(shape) != 3 or tuple(t.stride()) != (tok_stride, shape[2], 1):
+            raise TypeError(f"{name}: expected strides ({tok_stride}, D, 1) as declared to the plan, got {tuple(t.stride())}")
+    elif not t.is_contiguous():
+        raise TypeError(f"{name}: must be contiguous (or declare its token stride to the plan: q_stride / k_stride / v_stride)")
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise TypeError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
 
@@ -148,7 +153,7 @@ def _want(t, name, dtype, shape=None, device="cuda", optional=False):
 def _want_call(plan, bf16, lse=None, gammas=(), workspace=None, device="cuda"):
     nhd = (plan.N, plan.total_heads, plan.D)
     for name, t in bf16.items():
-        _want(t, name, torch.bfloat16, nhd, device)
+        _want(t, name, torch.bfloat16, nhd, device, tok_stride=getattr(plan, "in_strides", {}).get(name, 0))
     if lse is not None:
         _want(lse, "lse", torch.float32, (plan.H, plan.N), device)
     for name, t in gammas:
@@ -164,7 +169,8 @@ class Plan:
     is then the LOCAL head count."""
 
     def __init__(self, cu_seqlens, grids, num_heads, head_dim, rope_dims, rope_theta=10000.0, rms_eps=1e-6,
-                 softmax_scale=0.0, flags=0, text_lens=None, shard_starts=None, total_heads=None, head_offset=0, cp_rank=None):
+                 softmax_scale=0.0, flags=0, text_lens=None, shard_starts=None, total_heads=None, head_offset=0, cp_rank=None,
+                 q_stride=0, k_stride=0, v_stride=0):
         cu = [int(x) for x in cu_seqlens]
         gr = [int(x) for g in grids for x in g]
         self.params = AttnParams()
@@ -177,6 +183,9 @@ class Plan:
         self.params.rms_eps = rms_eps
         self.params.softmax_scale = softmax_scale
         self.params.flags = flags
+        # token strides (elements) of strided Q / K / V views, e.g. slices of a fused [N, 3, H, D] projection; 0 = contiguous
+        self.params.q_stride, self.params.k_stride, self.params.v_stride = int(q_stride), int(k_stride), int(v_stride)
+        self.in_strides = {"q": int(q_stride), "k": int(k_stride), "v": int(v_stride)}
         self._h = _vp()
         cu_arr = (ctypes.c_int32 * len(cu))(*cu)
         gr_arr = (ctypes.c_int32 * max(len(gr), 1))(*gr)

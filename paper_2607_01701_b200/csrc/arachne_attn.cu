@@ -126,12 +126,12 @@ EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-int make_raw_maps(const arachne_plan* pl, const void* base, RawMaps* out, RawTensor* rt) {
+int make_raw_maps(const arachne_plan* pl, const void* base, long long tok_stride, RawMaps* out, RawTensor* rt) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) { g_last_error = "cuTensorMapEncodeTiled not available from the driver"; return ARACHNE_ERR_CUDA; }
   const cuuint64_t D = static_cast<cuuint64_t>(pl->p.head_dim), Ht = static_cast<cuuint64_t>(pl->sh.H_total);
   const cuuint64_t dims[3] = {D, Ht, static_cast<cuuint64_t>(pl->p.total_tokens)};
-  const cuuint64_t strides[2] = {D * 2, Ht * D * 2};                 // bytes, dims 1 and 2
+  const cuuint64_t strides[2] = {D * 2, static_cast<cuuint64_t>(tok_stride) * 2};      // bytes, dims 1 (heads) and 2 (tokens)
   const cuuint32_t estr[3] = {1, 1, 1};
   for (int i = 0; i < 2; ++i) {
     const cuuint32_t box[3] = {64, 1, i == 0 ? static_cast<cuuint32_t>(kTileRows) : 8u};
@@ -141,7 +141,7 @@ int make_raw_maps(const arachne_plan* pl, const void* base, RawMaps* out, RawTen
     if (r != CUDA_SUCCESS) { g_last_error = "cuTensorMapEncodeTiled failed (" + std::to_string(static_cast<int>(r)) + ")"; return ARACHNE_ERR_CUDA; }
   }
   rt->base = static_cast<const __nv_bfloat16*>(base);
-  rt->tok_stride = static_cast<long long>(Ht * D);
+  rt->tok_stride = tok_stride;
   rt->head0 = pl->sh.head_offset;
   return ARACHNE_OK;
 }
@@ -176,7 +176,7 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   RawMaps vmaps{};
   RawTensor v_raw{};
   if (pl->raw_fwd) {
-    const int rc = make_raw_maps(pl, v.p[0], &vmaps, &v_raw);
+    const int rc = make_raw_maps(pl, v.p[0], pl->pd.in_stride[2], &vmaps, &v_raw);
     if (rc != ARACHNE_OK) return rc;
   }
   PrepParams pp{};
@@ -231,7 +231,8 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   RawTensor v_raw{}, do_raw{};
   if (pl->raw_bwd) {
     int rc;
-    if ((rc = make_raw_maps(pl, v.p[0], &vmaps, &v_raw)) != ARACHNE_OK || (rc = make_raw_maps(pl, d_o.p[0], &domaps, &do_raw)) != ARACHNE_OK)
+    if ((rc = make_raw_maps(pl, v.p[0], pl->pd.in_stride[2], &vmaps, &v_raw)) != ARACHNE_OK ||
+        (rc = make_raw_maps(pl, d_o.p[0], static_cast<long long>(pl->sh.H_total) * pl->p.head_dim, &domaps, &do_raw)) != ARACHNE_OK)
       return rc;
   }
   b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
@@ -361,6 +362,14 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     const float sc = p.softmax_scale == 0.f ? 1.0f / std::sqrt(static_cast<float>(p.head_dim)) : p.softmax_scale;
     if (sc * std::sqrt(static_cast<float>(p.head_dim)) > 1.0001f && !(p.flags & (ARACHNE_FLAG_WIDE_LOGITS | ARACHNE_FLAG_NO_NORM)))
       return ARACHNE_ERR_LOGIT_RANGE;
+  }
+  {
+    // token strides of Q, K, V: one-shard plans over a tensor of exactly num_heads heads; 16-byte rows; no overlap
+    const long long hd = static_cast<long long>(p.num_heads) * p.head_dim;
+    for (long long sx : {static_cast<long long>(p.q_stride), static_cast<long long>(p.k_stride), static_cast<long long>(p.v_stride)}) {
+      if (sx == 0) continue;
+      if (num_shards != 1 || total_heads != p.num_heads || sx < hd || (sx % 8) != 0) return ARACHNE_ERR_BAD_PARAM;
+    }
   }
   if (cu[0] != 0) return ARACHNE_ERR_BAD_CU_SEQLENS;
   for (int b = 0; b < p.num_seqs; ++b)
@@ -550,6 +559,12 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->sh.H_total = total_heads;
   pl->sh.head_offset = head_offset;
   pd.sh = pl->sh;
+  {
+    const long long contiguous = static_cast<long long>(total_heads) * p.head_dim;
+    pd.in_stride[0] = p.q_stride ? p.q_stride : contiguous;
+    pd.in_stride[1] = p.k_stride ? p.k_stride : contiguous;
+    pd.in_stride[2] = p.v_stride ? p.v_stride : contiguous;
+  }
   pd.cp_lo = cp_rank >= 0 ? pl->sh.start[cp_rank] : 0;
   pd.cp_hi = cp_rank >= 0 ? pl->sh.start[cp_rank + 1] : p.total_tokens;
   pl->tile_bytes = static_cast<size_t>(kTileRows) * p.head_dim * 2;
@@ -944,6 +959,7 @@ static int run_host(const arachne_plan* pl, bool with_bwd, const void* q_h, cons
   if (!pl || !q_h || !k_h || !v_h || !o_h || !lse_h) return ARACHNE_ERR_NULL_POINTER;
   if (with_bwd && (!do_h || !dq_h || !dk_h || !dv_h)) return ARACHNE_ERR_NULL_POINTER;
   if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;
+  if (pl->p.q_stride || pl->p.k_stride || pl->p.v_stride) return ARACHNE_ERR_BAD_PARAM;     // host buffers are dense [N, H, D]
   arachne_host_ctx* c = nullptr;
   int rc = host_ctx(pl, with_bwd, &c);
   if (rc) return rc;

@@ -65,8 +65,9 @@ struct Sharding {
 struct ShardedPtr {
   void* p[kMaxShards];
 };
-// element offset of (global token tok, local head h, 0) inside its shard; r_out = the shard
-__device__ __forceinline__ size_t raw_off(const Sharding& sh, int tok, int h, int D, int& r_out) {
+// element offset of (global token tok, local head h, 0) inside its shard; r_out = the shard.  tok_stride = elements between
+// consecutive tokens of THIS tensor (H_total * D unless the caller passed a strided Q, K or V: ProblemDesc::in_stride)
+__device__ __forceinline__ size_t raw_off(const Sharding& sh, long long tok_stride, int tok, int h, int D, int& r_out) {
   int r = 0;
   if (sh.n_shards > 1) {      // uniform branch: the plain single-tensor case pays nothing
 #pragma unroll
@@ -74,7 +75,7 @@ __device__ __forceinline__ size_t raw_off(const Sharding& sh, int tok, int h, in
       if (i < sh.n_shards && tok >= sh.start[i]) r = i;
   }
   r_out = r;
-  return (static_cast<size_t>(tok - sh.start[r]) * sh.H_total + sh.head_offset + h) * D;
+  return static_cast<size_t>(tok - sh.start[r]) * static_cast<size_t>(tok_stride) + static_cast<size_t>(sh.head_offset + h) * D;
 }
 // t.p[r] with constant indices only (a dynamic index would make ptxas copy the kernel parameter to local memory)
 template <typename T>
@@ -87,10 +88,11 @@ __device__ __forceinline__ T* shard_base(const ShardedPtr& t, int r) {
   }
   return static_cast<T*>(b);
 }
+// row of a CONTIGUOUS tensor (everything the library writes, dO, O)
 template <typename T>
 __device__ __forceinline__ T* raw_row(const Sharding& sh, const ShardedPtr& t, int tok, int h, int D) {
   int r;
-  const size_t off = raw_off(sh, tok, h, D, r);
+  const size_t off = raw_off(sh, static_cast<long long>(sh.H_total) * D, tok, h, D, r);
   return shard_base<T>(t, r) + off;
 }
 
@@ -127,6 +129,7 @@ struct ProblemDesc {
   int no_norm, no_rope;
   RopeDesc rope;
   Sharding sh;
+  long long in_stride[3];    // token stride (elements) of the raw Q, K, V (arachne_attn_params::q_stride ...; H_total * D if contiguous)
   unsigned long long* cta_trace;   // nullable: [kernel 0 fwd | 1 bwd_fused][gridDim.x][2] globaltimer ns at CTA start / end
   int cp_lo, cp_hi;          // context parallelism: this process owns the QUERY tokens [cp_lo, cp_hi) (0, N otherwise)
 };

@@ -140,12 +140,14 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     const TokInfo ti = pd.tok_info[tok];
     const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);   // R21: trailing text tokens are normed, not rotated
     int shard = 0;
-    const size_t src = raw_off(pd.sh, tok, h, D, shard) + d0;
+    const long long dense = static_cast<long long>(pd.sh.H_total) * D;
+    const size_t src = raw_off(pd.sh, dense, tok, h, D, shard) + d0;          // row in a contiguous tensor (dO, O)
+    const long long trow = tok - pd.sh.start[shard];                            // Q, K, V may be token-strided (ProblemDesc::in_stride)
     uint4 uq = zero4, uk = zero4, uv = zero4, ug = zero4, uo = zero4;
     if (valid) {
-      if (q_side) uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src);
-      uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src);
-      if (kBwd || kCopy) uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src);   // (bwd: |V|^2 bound)
+      if (q_side) uq = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.q, shard) + src + trow * (pd.in_stride[0] - dense));
+      uk = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.k, shard) + src + trow * (pd.in_stride[1] - dense));
+      if (kBwd || kCopy) uv = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.v, shard) + src + trow * (pd.in_stride[2] - dense));   // (bwd: |V|^2 bound)
       if (kBwd && q_side) {
         ug = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.d_o, shard) + src);
         uo = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(pp.o, shard) + src);
@@ -317,8 +319,10 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
     const TokInfo ti = pd.tok_info[tok];
     const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);     // R21: text tokens were not rotated
     int shard;
-    const size_t roff = raw_off(pd.sh, tok, h, D, shard) + d0;
-    const uint4 ux = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(xraw_s, shard) + roff);
+    const long long dense = static_cast<long long>(pd.sh.H_total) * D;
+    const size_t roff = raw_off(pd.sh, dense, tok, h, D, shard) + d0;                                           // output row (contiguous)
+    const size_t xoff = roff + static_cast<long long>(tok - pd.sh.start[shard]) * (pd.in_stride[is_k ? 1 : 0] - dense);   // raw Q / K row (may be token-strided)
+    const uint4 ux = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(xraw_s, shard) + xoff);
     float4 f0, f1;
     if (blocked) {
       // blocked layout [H][tile][D/32][128 rows][32], 16-byte pieces XOR-swizzled with (row & 7) (bwd_fused.cuh)

@@ -380,3 +380,28 @@ def test_raw_tma_tiles_equal_image_copies(orc, D):
         for k in ("O", "dQ", "dK", "dV"):
             assert torch.equal(pois[k][cu[b]:cu[b + 1]], raw[k][cu[b]:cu[b + 1]]), (k, b)
         assert torch.equal(pois["LSE"][:, cu[b]:cu[b + 1]], raw["LSE"][:, cu[b]:cu[b + 1]]), b
+
+
+def test_token_strided_qkv_views_of_a_fused_projection():
+    """arachne_attn_params::q_stride / k_stride / v_stride (SURVEY §8(b)): Q, K, V as the three [:, i] slices of one fused
+    [N, 3, H, D] projection output, no .contiguous() — bit-identical to the same data in dense tensors (deterministic
+    backward), for both head dims; a stride the plan cannot take is refused."""
+    from paper_2607_01701_b200 import binding
+    for D in (64, 128):
+        st = inputs.pack([(1, 10, 13), (2, 9, 11), (1, 3, 41)], 3, D, index=6)
+        t = inputs.make_inputs(st, device="cuda")
+        fused = torch.stack([t["q"], t["k"], t["v"]], dim=1).contiguous()            # [N, 3, H, D]
+        views = dict(q=fused[:, 0], k=fused[:, 1], v=fused[:, 2], dO=t["dO"])
+        assert not views["q"].is_contiguous()
+        s3 = 3 * st["H"] * D
+        dense = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC)
+        strided = pu.run_gpu(st, views, flags=binding.FLAG_DETERMINISTIC, plan_kw=dict(q_stride=s3, k_stride=s3, v_stride=s3))
+        for k in ("O", "LSE", "dQ", "dK", "dV"):
+            assert torch.equal(dense[k], strided[k]), (D, k)
+            assert strided[k].is_contiguous()
+        with pytest.raises(TypeError):                                               # undeclared stride: refused by the binding
+            pu.run_gpu(st, views, with_bwd=False)
+        for bad in (s3 + 4, st["H"] * D - 8):                                         # not a multiple of 8 / overlapping rows
+            with pytest.raises(binding.ArachneError) as ei:
+                binding.plan_for(st, q_stride=bad)
+            assert ei.value.status == 12
