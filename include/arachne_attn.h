@@ -71,6 +71,9 @@ enum {
                                         one-CTA kernel — 720p forward 176 vs 150 ms: the forward loop is bound by the
                                         softmax <-> MMA hand-off latency, which the cross-CTA hops lengthen, not by the
                                         shared-memory operand bandwidth the pairing relieves           */
+  ARACHNE_FLAG_FWD_MULTICAST = 64,   /* forward as clusters of 2 CTAs that share the K^/V stream: each CTA fetches half of
+                                        every tile and the TMA engine multicasts it into both (head_dim 128 only, ignored
+                                        otherwise); halves the L2 -> SM traffic of the forward         */
   ARACHNE_FLAG_IMAGE_COPIES = 32     /* A-B: the prologue copies V (and dO) into tile images in the workspace, as round 1
                                         did, instead of the main kernels reading them from the caller's tensors by
                                         tensor-map TMA (the default for one-shard plans).  Same results

@@ -71,6 +71,7 @@ struct arachne_plan {
   WorkItem* d_dyn_fwd_pair_items = nullptr;   // forward, CTA-pair form: items of up to four query tiles
   int n_fwd_pair_items = 0, n_fwd_pair_ctas = 0;
   bool fwd_pairs = false;               // D = 128 and ARACHNE_FLAG_FWD_CTA_PAIRS: fwd_pair_kernel
+  bool fwd_mcast = false;               // D = 128 and ARACHNE_FLAG_FWD_MULTICAST: fwd_mc_kernel
   bool raw_fwd = false, raw_bwd = false;   // V (fwd) / V and dO (bwd) tiles are read from the raw tensors by tensor-map TMA
                                            // (rawtile.cuh) instead of being copied into tile images by the prologue
   int n_img_fwd = 3, n_img_bwd = 4;        // tile-image regions in the forward / backward workspace
@@ -99,7 +100,9 @@ template <int D>
 int configure_kernels() {
   ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
   if constexpr (D == 128)
-    ARACHNE_CUDA(cudaFuncSetAttribute(fwd_pair_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D, true>::kSmemBytes));
+    ARACHNE_CUDA(cudaFuncSetAttribute(fwd_pair_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D, kFwdPair>::kSmemBytes));
+  if constexpr (D == 128)
+    ARACHNE_CUDA(cudaFuncSetAttribute(fwd_mc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D, kFwdMcast>::kSmemBytes));
   ARACHNE_CUDA(cudaFuncSetAttribute(bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdFusedCfg<D>::kSmemBytes));
   return ARACHNE_OK;
 }
@@ -195,7 +198,17 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   if constexpr (D == 128) {
     if (pl->fwd_pairs) {      // CTA-pair form (cluster of 2, cta_group::2): grid = 2 CTAs per pair
       if (pl->n_fwd_pair_ctas > 0)
-        fwd_pair_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, true>::kThreads, FwdCfg<D, true>::kSmemBytes, st>>>(pd, fp, vmaps);
+        fwd_pair_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, kFwdPair>::kThreads, FwdCfg<D, kFwdPair>::kSmemBytes, st>>>(pd, fp, vmaps);
+      ARACHNE_CUDA(cudaGetLastError());
+      prof_mark(pl, 0, 2, st);
+      if (pl->profiling) pl->prof_calls[0]++;
+      return ARACHNE_OK;
+    }
+  }
+  if constexpr (D == 128) {
+    if (pl->fwd_mcast) {      // multicast form (cluster of 2 sharing the K^/V stream): grid = 2 CTAs per cluster
+      if (pl->n_fwd_pair_ctas > 0)
+        fwd_mc_kernel<D><<<pl->n_fwd_pair_ctas, FwdCfg<D, kFwdMcast>::kThreads, FwdCfg<D, kFwdMcast>::kSmemBytes, st>>>(pd, fp, vmaps);
       ARACHNE_CUDA(cudaGetLastError());
       prof_mark(pl, 0, 2, st);
       if (pl->profiling) pl->prof_calls[0]++;
@@ -355,7 +368,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
   if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
-      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~63))
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~127))
     return ARACHNE_ERR_BAD_PARAM;
   {
     // envelope (reading R19): an explicit softmax_scale above 1/sqrt(D) widens the logits beyond what the gates are claimed for
@@ -444,6 +457,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->n_fwd_pair_items = static_cast<int>(fwd_pair_items.size());
   pl->n_fwd_pair_ctas = 2 * std::min(pl->num_sms / 2, pl->n_fwd_pair_items);
   pl->fwd_pairs = p.head_dim == 128 && (p.flags & ARACHNE_FLAG_FWD_CTA_PAIRS) != 0;
+  pl->fwd_mcast = p.head_dim == 128 && !pl->fwd_pairs && (p.flags & ARACHNE_FLAG_FWD_MULTICAST) != 0;
   // V / dO by tensor-map TMA from the raw tensors: plain (one-shard) plans.  Token-range-sharded tensors (Ulysses, CP) have
   // tiles that straddle shards and stay on the prologue's gather; so does the CTA-pair forward (it holds half tiles).
   {
@@ -631,7 +645,7 @@ const char* arachne_kernel_name(int pass, int idx) {
 int arachne_plan_cta_times(const arachne_plan* pl, int kernel, double* start_us, double* end_us, int n, int* n_ctas) {
   if (!pl || !start_us || !end_us || !n_ctas) return ARACHNE_ERR_NULL_POINTER;
   if (kernel < 0 || kernel > 1 || !pl->d_cta_trace) return ARACHNE_ERR_BAD_PARAM;
-  const int ctas = kernel == 0 ? (pl->fwd_pairs ? pl->n_fwd_pair_ctas : pl->n_fwd_ctas) : pl->n_ctas;
+  const int ctas = kernel == 0 ? ((pl->fwd_pairs || pl->fwd_mcast) ? pl->n_fwd_pair_ctas : pl->n_fwd_ctas) : pl->n_ctas;
   if (n < ctas) return ARACHNE_ERR_BAD_PARAM;
   std::vector<unsigned long long> t(static_cast<size_t>(kTraceMaxCtas) * 2);
   ARACHNE_CUDA(cudaMemcpy(t.data(), pl->d_cta_trace + static_cast<size_t>(kernel) * kTraceMaxCtas * 2, t.size() * sizeof(unsigned long long),

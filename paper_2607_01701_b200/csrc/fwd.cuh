@@ -59,9 +59,16 @@ constexpr bool kWarpArrive = ARACHNE_FWD_WARP_ARRIVE != 0;
 // Per SM this halves the K/V traffic from L2 and the B-operand reads from shared memory (the S GEMM, both operands in shared
 // memory, is otherwise pinned at the 128 B/clk shared-memory limit: DESIGN.md §7).  The peer CTA's warp 9 has no MMAs to
 // issue; it relays "my half has landed" to the leader.  Softmax / epilogue warps are the same code in both forms.
-template <int D, bool kPair = false>
+// kMode 2: the MULTICAST form (cluster of 2, D = 128).  The two CTAs of a cluster are two ordinary one-CTA kernels (their own
+// cta_group::1 MMAs, softmax and barriers) that work on the same (sequence, head) — the same 4-tile items as the pair form — and
+// SHARE THE K^/V STREAM: each CTA fetches half of every tile and multicasts it into both CTAs' ring slots, so the L2 -> SM
+// traffic of the pair halves (profiles/r2_fwd_handoff.md: the loop is sensitive to it).  A slot is refilled once BOTH CTAs'
+// tensor cores are done with it (the releasing commits are multicast too: kv_empty counts 2).
+enum : int { kFwdSingle = 0, kFwdPair = 1, kFwdMcast = 2 };
+template <int D, int kMode = kFwdSingle>
 struct FwdCfg {
-  static_assert(!kPair || D == 128, "the CTA-pair forward is built for head_dim 128 (V's d-halves must be whole 128-byte swizzle blocks)");
+  static constexpr bool kPair = kMode == kFwdPair;
+  static_assert(kMode == kFwdSingle || D == 128, "the CTA-pair forward is built for head_dim 128 (V's d-halves must be whole 128-byte swizzle blocks)");
   static constexpr int kTileBytes = kTileRows * D * 2;
   static constexpr int kSlotBytes = kPair ? kTileBytes / 2 : kTileBytes;   // one ring slot: a K^ or V tile (pair: this CTA's half)
   static constexpr int kRing = kPair ? 8 : ((D == 128) ? 5 : 8);           // K/V ring slots (K_j, V_j alternate)
@@ -79,9 +86,12 @@ struct FwdCfg {
 // largest logit bound (log2 units) for which the forward takes the static-max softmax
 constexpr float kStaticMaxBound = 32.0f;
 
-template <int D, bool kPair>
+template <int D, int kMode>
 __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp, const RawMaps& vm) {
-  using Cfg = FwdCfg<D, kPair>;
+  using Cfg = FwdCfg<D, kMode>;
+  constexpr bool kPair = kMode == kFwdPair;      // cta_group::2 MMAs issued by the leader for both CTAs
+  constexpr bool kMc = kMode == kFwdMcast;       // independent CTAs sharing the K^/V stream by multicast
+  constexpr bool kCl = kMode != kFwdSingle;      // any cluster form: 4-tile items handed out by the leader
   constexpr int TILE = Cfg::kTileBytes;
   constexpr int SLOT = Cfg::kSlotBytes;
   constexpr int RING = Cfg::kRing;
@@ -107,21 +117,21 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   const ItemRing item_ring{sItem, it_full, it_empty};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = kPair ? cluster_ctarank() : 0u;      // 0 = leader (issues the MMAs, owns the barriers the MMA warp waits on)
+  const uint32_t rank = kCl ? cluster_ctarank() : 0u;      // 0 = leader (issues the MMAs, owns the barriers the MMA warp waits on)
   // arrivals of the softmax / epilogue warps on a barrier the MMA warp waits on: 1-CTA form = every thread arrives (count 128);
   // pair form = one arrival per warp on the LEADER's barrier (count 4 local + 4 remote warps)
   constexpr uint32_t kArrivals = kPair ? 8 : (kWarpArrive ? 4 : 128);
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();   // tile images need 1024-byte alignment (128B swizzle atoms)
     mbar_init(q_full, 1); mbar_init(q_empty, 1);
-    for (int s = 0; s < RING; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
+    for (int s = 0; s < RING; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], kMc ? 2 : 1); }
     for (int t = 0; t < 2; ++t) {
       mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kArrivals);
       for (int i = 0; i < kSplitP - 1; ++i) mbar_init(&pa_full[t * (kSplitP - 1) + i], kArrivals);
       mbar_init(&pv_done[t], 1); mbar_init(&o_free[t], kArrivals);
     }
     // item ring consumers: MMA + 8 softmax warps; pair: + the peer's producer, relay and 8 softmax warps (remote arrivals)
-    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], kPair ? 19 : 9); }
+    for (int s = 0; s < kItemRing; ++s) { mbar_init(&it_full[s], 1); mbar_init(&it_empty[s], kCl ? 19 : 9); }
     if constexpr (kPair) {
       mbar_init(peer_q_full, 1);
       for (int s = 0; s < RING; ++s) mbar_init(&peer_kv_full[s], 1);
@@ -133,18 +143,18 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
     else { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
   }
   tc_fence_before();
-  if constexpr (kPair) cluster_sync_all(); else __syncthreads();      // (pair: barrier inits visible to the peer's remote arrivals)
+  if constexpr (kCl) cluster_sync_all(); else __syncthreads();      // (cluster: barrier inits visible to the peer's remote arrivals)
   if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2] = globaltimer_ns();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
   const size_t head_stride = static_cast<size_t>(pd.n_tiles_total) * TILE;
-  const WorkItem* item_list = kPair ? pd.dyn_fwd_pair_items : pd.dyn_fwd_items;
-  const int n_list = kPair ? pd.n_fwd_pair_items : pd.n_fwd_items;
-  auto wait = [](uint64_t* bar, uint32_t parity) { if constexpr (kPair) mbar_wait_wd(bar, parity); else mbar_wait(bar, parity); };
+  const WorkItem* item_list = kCl ? pd.dyn_fwd_pair_items : pd.dyn_fwd_items;
+  const int n_list = kCl ? pd.n_fwd_pair_items : pd.n_fwd_items;
+  auto wait = [](uint64_t* bar, uint32_t parity) { if constexpr (kCl) mbar_wait_wd(bar, parity); else mbar_wait(bar, parity); };
   // item hand-out.  1-CTA: sm100.cuh ItemRing.  Pair: the LEADER's producer takes the index and publishes it to both CTAs'
   // rings; every consumer warp of both CTAs releases the slot on the LEADER's `empty` barrier.
   auto fetch_producer = [&](uint32_t it) -> int {
-    if constexpr (!kPair) return item_fetch_producer(item_ring, it, pd.work_counter, n_list, lane);
+    if constexpr (!kCl) return item_fetch_producer(item_ring, it, pd.work_counter, n_list, lane);
     const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
     int item = 0;
     if (lane == 0) {
@@ -159,7 +169,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
     return __shfl_sync(0xffffffffu, item, 0);
   };
   auto fetch_consumer = [&](uint32_t it) -> int {
-    if constexpr (!kPair) return item_fetch_consumer(item_ring, it, lane);
+    if constexpr (!kCl) return item_fetch_consumer(item_ring, it, lane);
     const uint32_t s = it % kItemRing, ph = (it / kItemRing) & 1;
     mbar_wait_wd(&it_full[s], ph);
     const int item = sItem[s];
@@ -170,7 +180,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   // number of query tiles each CTA works on in this item (pair: both CTAs run the same count; tiles beyond the item's
   // last one are PHANTOMS — a copy of the last real tile whose rows are never stored — because an M = 256 instruction always
   // covers both CTAs)
-  auto tiles_per_cta = [](const WorkItem& wi) { return kPair ? min(2, wi.pad) : wi.pad; };
+  auto tiles_per_cta = [](const WorkItem& wi) { return kCl ? min(2, wi.pad) : wi.pad; };
 
   if (warp == 8) {
     // ------------------------------------------------------------------ producer
@@ -192,7 +202,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
       wait(q_empty, (it & 1) ^ 1);
       if (lane == 0) {
         mbar_expect_tx(q_full, n_q * TILE);
-        if constexpr (!kPair) {
+        if constexpr (!kCl) {
           bulk_g2s(sQ, hbase_q + static_cast<size_t>(sq.tile_base + wi.tile) * TILE, n_q * TILE, q_full);
         } else {
           for (int t = 0; t < n_q; ++t) {      // this CTA's tiles 2*rank + t of the item; phantoms read the item's last tile
@@ -214,14 +224,19 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
               const uint32_t bytes = raw_tile_stage<D>(sKV + st * SLOT, fp.v_raw, wi.head, tok0, valid, lane);
               if (lane == 0) {
                 mbar_expect_tx(&kv_full[st], bytes);
-                raw_tile_issue<D>(sKV + st * SLOT, vm, fp.v_raw, wi.head, tok0, valid, &kv_full[st]);
+                if constexpr (kMc) raw_tile_issue_mc<D>(sKV + st * SLOT, vm, fp.v_raw, wi.head, tok0, valid, &kv_full[st], rank);
+                else raw_tile_issue<D>(sKV + st * SLOT, vm, fp.v_raw, wi.head, tok0, valid, &kv_full[st]);
               }
               continue;
             }
           }
           if (lane == 0) {
             mbar_expect_tx(&kv_full[st], SLOT);
-            if constexpr (!kPair) {
+            if constexpr (kMc) {
+              // this CTA's half of the tile image, into BOTH CTAs' slots
+              bulk_g2s_mc(sKV + st * SLOT + rank * (TILE / 2), (kv == 0 ? hbase_k : hbase_v) + off + rank * (TILE / 2), TILE / 2,
+                          &kv_full[st], 3);
+            } else if constexpr (!kPair) {
               bulk_g2s(sKV + st * SLOT, (kv == 0 ? hbase_k : hbase_v) + off, TILE, &kv_full[st]);
             } else if (kv == 0) {
               // K^: this CTA's 64 keys (rows 64*rank..) of each 64-element block -> [D/64][64 rows][128 B]
@@ -237,7 +252,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
         __syncwarp();
       }
     }
-  } else if (warp == 9 && rank != 0) {
+  } else if (warp == 9 && kPair && rank != 0) {
     // ------------------------------------------------------------------ pair form, peer CTA: relay "my half has landed"
     if constexpr (kPair) {
       uint32_t it = 0, ring = 0;
@@ -266,6 +281,8 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
     auto mma_ss = [](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) { if constexpr (kPair) umma_ss2(d, a, b, idesc, acc); else umma_ss(d, a, b, idesc, acc); };
     auto mma_ts = [](uint32_t d, uint32_t a, uint64_t b, uint32_t idesc, uint32_t acc) { if constexpr (kPair) umma_ts2(d, a, b, idesc, acc); else umma_ts(d, a, b, idesc, acc); };
     auto commit = [](uint64_t* bar) { if constexpr (kPair) umma_commit2(bar); else umma_commit(bar); };
+    // releasing a K/V ring slot: in the multicast form the slot is written by BOTH CTAs' producers, so both must hear it
+    auto commit_slot = [&](uint64_t* bar) { if constexpr (kMc) umma_commit_mc(bar, 3); else commit(bar); };
     uint32_t it = 0, ring = 0;      // ring: slot counter at K_0 of the current item (K_j = ring+2j, V_j = ring+2j+1)
     uint32_t cnt[2] = {0, 0};       // per query tile: number of PV tiles issued so far
     for (;; ++it) {
@@ -289,7 +306,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
           }
           commit(&s_full[t]);
           if (t == n_q - 1) {
-            commit(&kv_empty[st]);
+            commit_slot(&kv_empty[st]);
             if (j == n_kv - 1) commit(q_empty);
           }
         }
@@ -313,7 +330,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
               mma_ts(tO, tP + kk * 8, make_sdesc(aKV + st * SLOT + kk * 2048, kTileRows * 128, 1024), idesc_o, (j > 0 || kk > 0) ? 1u : 0u);
             if (piece == kSplitP - 1) {
               commit(&pv_done[t]);
-              if (t == n_q - 1) commit(&kv_empty[st]);
+              if (t == n_q - 1) commit_slot(&kv_empty[st]);
             }
           }
           __syncwarp();
@@ -473,7 +490,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
       // ---- epilogue: O / l -> bf16, LSE (natural log, reading R9)
       wait(&pv_done[t], (g - 1) & 1);
       tc_fence_after();
-      const int t_item = (kPair ? 2 * static_cast<int>(rank) : 0) + t;     // this tile's place in the item (pair: phantoms beyond wi.pad)
+      const int t_item = (kCl ? 2 * static_cast<int>(rank) : 0) + t;     // this tile's place in the item (cluster forms: phantoms beyond wi.pad)
       const int n = (wi.tile + t_item) * kTileRows + row;     // token inside the sequence
       const int tok_g = sq.tok_start + n;
       const bool valid_row = t_item < wi.pad && n < sq.len && tok_g >= pd.cp_lo && tok_g < pd.cp_hi;   // CP: only this rank's query rows
@@ -503,7 +520,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
     }
   }
   tc_fence_before();
-  if constexpr (kPair) cluster_sync_all(); else __syncthreads();   // (pair: no remote arrival may target a CTA that has exited)
+  if constexpr (kCl) cluster_sync_all(); else __syncthreads();   // (cluster: no remote arrival or multicast may target a CTA that has exited)
   if (pd.cta_trace && threadIdx.x == 0) pd.cta_trace[(0 * kTraceMaxCtas + blockIdx.x) * 2 + 1] = globaltimer_ns();
   if (warp == 9) {
     if constexpr (kPair) tmem_dealloc2(tbase, 512); else tmem_dealloc(tbase, 512);
@@ -512,13 +529,19 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
 
 template <int D>
 __global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp, const __grid_constant__ RawMaps vmaps) {
-  fwd_body<D, false>(pd, fp, vmaps);
+  fwd_body<D, kFwdSingle>(pd, fp, vmaps);
 }
 // CTA-pair form: grid = 2 x (number of pairs), static cluster of 2 (the two SMs of a TPC)
 template <int D>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_pair_kernel(ProblemDesc pd, FwdParams fp,
                                                                                          const __grid_constant__ RawMaps vmaps) {
-  fwd_body<D, true>(pd, fp, vmaps);      // (the pair form reads V images; the maps are unused)
+  fwd_body<D, kFwdPair>(pd, fp, vmaps);      // (the pair form reads V images; the maps are unused)
+}
+// Multicast form: grid = 2 x (number of clusters), static cluster of 2
+template <int D>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_mc_kernel(ProblemDesc pd, FwdParams fp,
+                                                                                       const __grid_constant__ RawMaps vmaps) {
+  fwd_body<D, kFwdMcast>(pd, fp, vmaps);
 }
 
 }  // namespace arachne

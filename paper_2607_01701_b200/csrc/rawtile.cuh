@@ -71,4 +71,18 @@ __device__ __forceinline__ void raw_tile_issue(uint8_t* dst, const RawMaps& m, c
   }
 }
 
+// Multicast form (cluster of 2, D = 128): CTA `rank` fetches the 64-element block `rank` of the tile and multicasts it into
+// both CTAs' slots; each CTA has staged the generic-proxy rows of a ragged tile itself.
+template <int D>
+__device__ __forceinline__ void raw_tile_issue_mc(uint8_t* dst, const RawMaps& m, const RawTensor& rt, int head, int tok0, int valid,
+                                                  uint64_t* bar, uint32_t rank) {
+  static_assert(D == 128, "two 64-element blocks, one per CTA of the cluster");
+  const int h = rt.head0 + head, c = static_cast<int>(rank);
+  if (valid >= kTileRows) {
+    tma_load_3d_mc(dst + c * (kTileRows * 128), &m.tile, 64 * c, h, tok0, bar, 3);
+  } else {
+    for (int r = 0; r + 8 <= valid; r += 8) tma_load_3d_mc(dst + c * (kTileRows * 128) + r * 128, &m.rows8, 64 * c, h, tok0 + r, bar, 3);
+  }
+}
+
 }  // namespace arachne

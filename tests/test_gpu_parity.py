@@ -334,19 +334,24 @@ def test_one_plan_serves_two_streams_with_separate_workspaces():
 
 
 # ------------------------------------------------------------------ the CTA-pair (cta_group::2) forward kernel (opt-in, A/B)
-def test_forward_cta_pairs_against_oracle_and_default(orc):
-    """ARACHNE_FLAG_FWD_CTA_PAIRS: items of up to four query tiles over a cluster of two CTAs that share every K/V tile.
-    Packs with 1, 2, 3, 4 and 5+ query tiles per sequence exercise full pairs, a peer CTA with one real + one phantom tile,
-    and a peer CTA with only phantoms; every output is held to the oracle gates, and O / LSE must equal the one-CTA
-    kernel's bit for bit (same per-row arithmetic; only the instruction shape differs)."""
+@pytest.mark.parametrize("form", ["pairs", "multicast", "multicast+images"])
+def test_forward_cluster_forms_against_oracle_and_default(orc, form):
+    """The two cluster forms of the forward (head_dim 128): ARACHNE_FLAG_FWD_CTA_PAIRS (cta_group::2 MMAs over a pair that
+    holds half of every K/V tile each) and ARACHNE_FLAG_FWD_MULTICAST (two independent CTAs, every K^/V tile fetched half by
+    each and multicast into both; with and without the tensor-map path for V).  Items of up to four query tiles: packs
+    with 1, 2, 3, 4 and 5+ query tiles per sequence exercise full clusters, a peer CTA with one real + one phantom tile, and a
+    peer CTA with only phantoms; ragged last key tiles exercise the multicast of a partial V tile.  Every output is held to
+    the oracle gates, and O / LSE must equal the one-CTA kernel's bit for bit (same per-row arithmetic)."""
     from paper_2607_01701_b200 import binding
+    flags = {"pairs": binding.FLAG_FWD_CTA_PAIRS, "multicast": binding.FLAG_FWD_MULTICAST,
+             "multicast+images": binding.FLAG_FWD_MULTICAST | binding.FLAG_IMAGE_COPIES}[form]
     for grids, H in (([(1, 10, 10), (1, 16, 16), (3, 10, 13), (2, 16, 16), (5, 11, 13)], 3),      # 100, 256, 390, 512, 715 tokens
                      ([(9, 16, 16), (1, 1, 1), (1, 3, 43)], 2)):                                    # 2304 (18 tiles), 1, 129
         st = inputs.pack(grids, H, 128, index=4)
-        w, got, t = _full_case(orc, st, flags=binding.FLAG_FWD_CTA_PAIRS)
+        w, got, t = _full_case(orc, st, flags=flags)
         base = pu.run_gpu(st, t, with_bwd=False)
         assert torch.equal(got["O"], base["O"]) and torch.equal(got["LSE"], base["LSE"])
-        print("fwd pairs:", grids, w)
+        print("fwd", form, grids, w)
 
 
 # ------------------------------------------------------------------ V / dO by tensor-map TMA (default) vs tile-image copies
