@@ -75,9 +75,11 @@ struct FwdCfg {
   static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * (kSplitP - 1) + 2 * kItemRing + (kPair ? 1 + kRing : 0);
   static constexpr int kSmemBytes = 2 * kTileBytes + kRing * kSlotBytes + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 320;
-  // every 4th exp2 on the FMA pipe (ex2_poly3) instead of MUFU: pays at D = 64, where MUFU (16 ex2/clk/SM) is the
-  // busiest unit (cogvideox fwd 13.0 vs 14.7 ms); at D = 128 the loop is tensor/power-bound and the extra FMA-pipe
-  // instructions cost more than they save (720p fwd 148.0 ms without vs 152.7 ms with; profiles/r1_notes.md §10)
+  // every other PAIR of exp2 on the FMA pipe (ex2_poly3_x2: packed FADD2 / FFMA2, 4 issue slots per element) instead of MUFU:
+  // pays at D = 64, where MUFU (16 ex2/clk/SM) is the busiest unit (cogvideox fwd 12.6 ms vs 12.9 with every 4th exp2 as a scalar
+  // polynomial, 14.7 all-MUFU); at D = 128 every variant — scalar or packed, 1/16 to all — is SLOWER than all-MUFU (720p fwd
+  // 147.9 / 153.2 / 156.1 / 162.3 ms for 0 / 1/4 / 1/2 / all packed): the softmax warps are bound by their own in-order
+  // instruction stream, not by the MUFU pipe (profiles/r2_fwd_handoff.md)
   static constexpr bool kPolyExp = (D == 64);
   // TMEM columns: S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [256+D,256+2D)
   static constexpr uint32_t kColS = 0, kColO = 256;
@@ -401,8 +403,9 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
             if (valid >= kTileRows) {
 #pragma unroll
               for (int i = 0; i < 32; i += 2) {
-                const float p0 = ex2_approx(__uint_as_float(cur[i]));
-                const float p1 = (Cfg::kPolyExp && (i & 2)) ? ex2_poly3(__uint_as_float(cur[i + 1])) : ex2_approx(__uint_as_float(cur[i + 1]));
+                float p0, p1;
+                if (Cfg::kPolyExp && (i & 2)) ex2_poly3_x2(__uint_as_float(cur[i]), __uint_as_float(cur[i + 1]), p0, p1);
+                else { p0 = ex2_approx(__uint_as_float(cur[i])); p1 = ex2_approx(__uint_as_float(cur[i + 1])); }
                 rs0 += p0; rs1 += p1;
                 pk[i >> 1] = pack_bf16x2(p0, p1);
               }

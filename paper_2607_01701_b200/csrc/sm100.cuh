@@ -381,6 +381,31 @@ __device__ __forceinline__ float ex2_poly3(float x) {
   p = fmaf(p, f, 0.9999280572f);
   return __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));
 }
+// Two exp2 at once with the packed fp32x2 instructions of sm_100 (FADD2 / FFMA2: one issue slot per pair): same Cody-Waite split
+// and degree-3 polynomial as ex2_poly3.
+__device__ __forceinline__ void ex2_poly3_x2(float x0, float x1, float& y0, float& y1) {
+  uint64_t v, t, f, p;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x0), "f"(x1));
+  asm("{\n\t.reg .b64 m, c3, c2, c1, c0, u;\n\t"
+      "mov.b64 m, {0f4B400000, 0f4B400000};\n\t"          // 1.5 * 2^23
+      "mov.b64 c3, {0f3D61FBF4, 0f3D61FBF4};\n\t"         // 0.0551716685
+      "mov.b64 c2, {0f3E786F0D, 0f3E786F0D};\n\t"         // 0.2426111251
+      "mov.b64 c1, {0f3F31798D, 0f3F31798D};\n\t"         // 0.6932609677
+      "mov.b64 c0, {0f3F7FFB49, 0f3F7FFB49};\n\t"         // 0.9999280572
+      "add.rn.f32x2 %0, %3, m;\n\t"
+      "sub.rn.f32x2 u, %0, m;\n\t"
+      "sub.rn.f32x2 %1, %3, u;\n\t"
+      "fma.rn.f32x2 %2, c3, %1, c2;\n\t"
+      "fma.rn.f32x2 %2, %2, %1, c1;\n\t"
+      "fma.rn.f32x2 %2, %2, %1, c0;\n\t}\n"
+      : "=&l"(t), "=&l"(f), "=&l"(p)
+      : "l"(v));
+  float p0, p1, t0, t1;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(p));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(t0), "=f"(t1) : "l"(t));
+  y0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
+  y1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
+}
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;\n" : "=r"(r) : "f"(hi), "f"(lo));
