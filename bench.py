@@ -304,6 +304,7 @@ def main():
     ap.add_argument("--deterministic", action="store_true", help="ARACHNE_FLAG_DETERMINISTIC backward as the main measurement")
     ap.add_argument("--fwd-pairs", action="store_true", help="ARACHNE_FLAG_FWD_CTA_PAIRS: the CTA-pair (cta_group::2) forward kernel (A/B)")
     ap.add_argument("--fwd-mcast", action="store_true", help="ARACHNE_FLAG_FWD_MULTICAST: forward as clusters of 2 sharing the K/V stream by TMA multicast (A/B)")
+    ap.add_argument("--fused-q", action="store_true", help="ARACHNE_FLAG_FWD_FUSED_Q: RMSNorm + RoPE of the query tiles inside fwd_kernel instead of the prologue (A/B)")
     ap.add_argument("--image-copies", action="store_true", help="ARACHNE_FLAG_IMAGE_COPIES: the prologue copies V / dO into tile images (round-1 path) instead of tensor-map TMA from the raw tensors (A/B)")
     ap.add_argument("--heads", type=int, default=0, help="override the head count: the per-rank share of a Ulysses group of degree H/heads")
     ap.add_argument("--seed-offset", type=int, default=0, help="heavytail: another batch drawn from the same recipe (R18)")
@@ -328,7 +329,7 @@ def main():
     # structure (weak scaling), no data-path collective; NCCL only for the barrier and the max-time.
     r = time_workload(env, args.workload, args.steps, args.warmup, deterministic=args.deterministic, order=args.order,
                       seed_offset=args.seed_offset, heads=args.heads, keep=True,
-                      extra_flags=(binding.FLAG_FWD_CTA_PAIRS if args.fwd_pairs else 0) | (binding.FLAG_IMAGE_COPIES if args.image_copies else 0) | (binding.FLAG_FWD_MULTICAST if args.fwd_mcast else 0))
+                      extra_flags=(binding.FLAG_FWD_CTA_PAIRS if args.fwd_pairs else 0) | (binding.FLAG_IMAGE_COPIES if args.image_copies else 0) | (binding.FLAG_FWD_MULTICAST if args.fwd_mcast else 0) | (binding.FLAG_FWD_FUSED_Q if args.fused_q else 0))
     r["world"] = env.world
     st, plan, t, flops = r["st"], r["plan"], r["t"], r["flops"]
     s2 = flops / (14.0 * st["D"] * st["H"])

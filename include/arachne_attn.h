@@ -68,12 +68,17 @@ enum {
   ARACHNE_FLAG_WIDE_LOGITS = 8,      /* the caller accepts logits outside the verified envelope (below) */
   ARACHNE_FLAG_FWD_CTA_PAIRS = 16,   /* A-B: run the forward as CTA pairs (cluster of 2, tcgen05 cta_group::2; head_dim 128
                                         only, ignored otherwise).  Correct (same parity tests) but SLOWER than the default
-                                        one-CTA kernel — 720p forward 176 vs 150 ms: the forward loop is bound by the
+                                        one-CTA kernel — 720p forward 180 vs 152 ms: the forward loop is bound by the
                                         softmax <-> MMA hand-off latency, which the cross-CTA hops lengthen, not by the
                                         shared-memory operand bandwidth the pairing relieves           */
   ARACHNE_FLAG_FWD_MULTICAST = 64,   /* forward as clusters of 2 CTAs that share the K^/V stream: each CTA fetches half of
                                         every tile and the TMA engine multicasts it into both (head_dim 128 only, ignored
                                         otherwise); halves the L2 -> SM traffic of the forward         */
+  ARACHNE_FLAG_FWD_FUSED_Q = 128,    /* A-B of SURVEY §7.2 "measure both": the forward loads its RAW query tiles and applies
+                                        RMSNorm + RoPE + scale to them inside fwd_kernel (once per work item) instead of
+                                        reading Q^ tile images written by the in-call prologue; same bytes reach the
+                                        tensor core.  One-CTA form, one-shard plans, RMSNorm on; ignored otherwise.
+                                        Slower on short sequences                                        */
   ARACHNE_FLAG_IMAGE_COPIES = 32     /* A-B: the prologue copies V (and dO) into tile images in the workspace, as round 1
                                         did, instead of the main kernels reading them from the caller's tensors by
                                         tensor-map TMA (the default for one-shard plans).  Same results

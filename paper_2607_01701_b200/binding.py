@@ -18,7 +18,7 @@ if not os.path.exists(_LIB_PATH):
         "(nvcc, sm_100a). There is no CPU fallback.")
 _lib = ctypes.CDLL(_LIB_PATH)
 
-FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE, FLAG_WIDE_LOGITS, FLAG_FWD_CTA_PAIRS, FLAG_IMAGE_COPIES, FLAG_FWD_MULTICAST = 1, 2, 4, 8, 16, 32, 64
+FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE, FLAG_WIDE_LOGITS, FLAG_FWD_CTA_PAIRS, FLAG_IMAGE_COPIES, FLAG_FWD_MULTICAST, FLAG_FWD_FUSED_Q = 1, 2, 4, 8, 16, 32, 64, 128
 ERR_LOGIT_RANGE = 14
 
 EXPORTS = [

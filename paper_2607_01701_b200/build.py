@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libarachne_attn.so")
 SOURCES = ["arachne_attn.cu"]
-HEADERS = ["sm100.cuh", "common.cuh", "rawtile.cuh", "prep.cuh", "fwd.cuh", "bwd_fused.cuh", os.path.join("..", "..", "include", "arachne_attn.h")]
+HEADERS = ["sm100.cuh", "common.cuh", "rawtile.cuh", "normrope.cuh", "prep.cuh", "fwd.cuh", "bwd_fused.cuh", os.path.join("..", "..", "include", "arachne_attn.h")]
 
 
 def _stale() -> bool:

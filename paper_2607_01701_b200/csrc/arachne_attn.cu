@@ -72,6 +72,7 @@ struct arachne_plan {
   int n_fwd_pair_items = 0, n_fwd_pair_ctas = 0;
   bool fwd_pairs = false;               // D = 128 and ARACHNE_FLAG_FWD_CTA_PAIRS: fwd_pair_kernel
   bool fwd_mcast = false;               // D = 128 and ARACHNE_FLAG_FWD_MULTICAST: fwd_mc_kernel
+  bool fwd_fused_q = false;             // ARACHNE_FLAG_FWD_FUSED_Q: fwd_kernel normalises its own raw query tiles (A/B of a1)
   bool raw_fwd = false, raw_bwd = false;   // V (fwd) / V and dO (bwd) tiles are read from the raw tensors by tensor-map TMA
                                            // (rawtile.cuh) instead of being copied into tile images by the prologue
   int n_img_fwd = 3, n_img_bwd = 4;        // tile-image regions in the forward / backward workspace
@@ -99,6 +100,7 @@ namespace {
 template <int D>
 int configure_kernels() {
   ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
+  ARACHNE_CUDA(cudaFuncSetAttribute(fwd_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes));
   if constexpr (D == 128)
     ARACHNE_CUDA(cudaFuncSetAttribute(fwd_pair_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D, kFwdPair>::kSmemBytes));
   if constexpr (D == 128)
@@ -188,13 +190,20 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.qt = f.qt; pp.kt = f.kt; pp.vt = f.vt;
   pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // S leaves the tensor core in the exp2 domain
   pp.stats = pd.stats;
+  pp.skip_q = pl->fwd_fused_q ? 1 : 0;
+  RawMaps qmaps{};
+  RawTensor q_raw{};
+  if (pl->fwd_fused_q) {
+    const int rc = make_raw_maps(pl, q.p[0], pl->pd.in_stride[0], &qmaps, &q_raw);
+    if (rc != ARACHNE_OK) return rc;
+  }
   prof_mark(pl, 0, 0, st);
   ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader), st));
   if (pl->raw_fwd) prep_kernel<D, false, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   else prep_kernel<D, false, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 1, st);
-  FwdParams fp{f.qt, f.kt, f.vt, v_raw, o, lse, pl->d_envelope, pl->bound_limit};
+  FwdParams fp{f.qt, f.kt, f.vt, v_raw, q_raw, gq, pp.q_prescale, o, lse, pl->d_envelope, pl->bound_limit};
   if constexpr (D == 128) {
     if (pl->fwd_pairs) {      // CTA-pair form (cluster of 2, cta_group::2): grid = 2 CTAs per pair
       if (pl->n_fwd_pair_ctas > 0)
@@ -216,7 +225,10 @@ int launch_fwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
     }
   }
   const int grid = pl->n_fwd_ctas;
-  if (grid > 0) fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp, vmaps);   // (a CP rank may own no queries)
+  if (grid > 0) {
+    if (pl->fwd_fused_q) fwd_kernel<D, true><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp, vmaps, qmaps);
+    else fwd_kernel<D><<<grid, FwdCfg<D>::kThreads, FwdCfg<D>::kSmemBytes, st>>>(pd, fp, vmaps, qmaps);
+  }   // (a CP rank may own no queries)
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 0, 2, st);
   if (pl->profiling) pl->prof_calls[0]++;
@@ -368,7 +380,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   }
   if (rsum != p.head_dim) return ARACHNE_ERR_BAD_ROPE_DIMS;
   if (!(p.rope_theta > 0.f) || !std::isfinite(p.rope_theta) || !(p.rms_eps >= 0.f) || !std::isfinite(p.rms_eps) ||
-      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~127))
+      !(p.softmax_scale >= 0.f) || !std::isfinite(p.softmax_scale) || (p.flags & ~255))
     return ARACHNE_ERR_BAD_PARAM;
   {
     // envelope (reading R19): an explicit softmax_scale above 1/sqrt(D) widens the logits beyond what the gates are claimed for
@@ -458,6 +470,9 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->n_fwd_pair_ctas = 2 * std::min(pl->num_sms / 2, pl->n_fwd_pair_items);
   pl->fwd_pairs = p.head_dim == 128 && (p.flags & ARACHNE_FLAG_FWD_CTA_PAIRS) != 0;
   pl->fwd_mcast = p.head_dim == 128 && !pl->fwd_pairs && (p.flags & ARACHNE_FLAG_FWD_MULTICAST) != 0;
+  // fused Q: one-CTA form, one-shard plans (tensor maps), RMSNorm on (without it the logit bound needs a pass over Q anyway)
+  pl->fwd_fused_q = (p.flags & ARACHNE_FLAG_FWD_FUSED_Q) && !pl->fwd_pairs && !pl->fwd_mcast && num_shards == 1 && cp_rank < 0 &&
+                    !(p.flags & ARACHNE_FLAG_NO_NORM);
   // V / dO by tensor-map TMA from the raw tensors: plain (one-shard) plans.  Token-range-sharded tensors (Ulysses, CP) have
   // tiles that straddle shards and stay on the prologue's gather; so does the CTA-pair forward (it holds half tiles).
   {

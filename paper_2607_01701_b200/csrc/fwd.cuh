@@ -21,6 +21,7 @@
 // error floor at ~2e-4 instead of ~1.5e-3 for bf16.  P and V are bf16.
 #pragma once
 #include "common.cuh"
+#include "normrope.cuh"
 #include "rawtile.cuh"
 #include "sm100.cuh"
 
@@ -31,6 +32,11 @@ struct FwdParams {
   const uint8_t* kt;      // K^ fp16 images
   const uint8_t* vt;      // V bf16 images (only when v_raw.base == nullptr)
   RawTensor v_raw;        // base != nullptr: V tiles come straight from the raw tensor by tensor-map TMA (rawtile.cuh)
+  RawTensor q_raw;        // base != nullptr (ARACHNE_FLAG_FWD_FUSED_Q, one-CTA form): the item's RAW query tiles are loaded by
+                          // tensor-map TMA and normalised + rotated + rounded to fp16 in place by the softmax warps ("fused into
+                          // the Q load" in the literal sense; the A/B partner of the prologue)
+  const float* gamma_q;   // fused Q only
+  float q_prescale;       // fused Q only: softmax_scale * log2(e)
   ShardedPtr o;           // [N,H_total,D] bf16, possibly sharded by token range (common.cuh)
   float* lse;             // [H,N]
   unsigned* envelope;     // plan-owned sticky word: float bits of the largest logit bound that exceeded bound_limit
@@ -72,7 +78,7 @@ struct FwdCfg {
   static constexpr int kTileBytes = kTileRows * D * 2;
   static constexpr int kSlotBytes = kPair ? kTileBytes / 2 : kTileBytes;   // one ring slot: a K^ or V tile (pair: this CTA's half)
   static constexpr int kRing = kPair ? 8 : ((D == 128) ? 5 : 8);           // K/V ring slots (K_j, V_j alternate)
-  static constexpr int kNumBars = 2 + 2 * kRing + 8 + 2 * (kSplitP - 1) + 2 * kItemRing + (kPair ? 1 + kRing : 0);
+  static constexpr int kNumBars = 3 + 2 * kRing + 8 + 2 * (kSplitP - 1) + 2 * kItemRing + (kPair ? 1 + kRing : 0);
   static constexpr int kSmemBytes = 2 * kTileBytes + kRing * kSlotBytes + 8 * kNumBars + 16 + 4 * kItemRing;
   static constexpr int kThreads = 320;
   // every other PAIR of exp2 on the FMA pipe (ex2_poly3_x2: packed FADD2 / FFMA2, 4 issue slots per element) instead of MUFU:
@@ -88,8 +94,48 @@ struct FwdCfg {
 // largest logit bound (log2 units) for which the forward takes the static-max softmax
 constexpr float kStaticMaxBound = 32.0f;
 
-template <int D, int kMode>
-__device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp, const RawMaps& vm) {
+// Fused Q (ARACHNE_FLAG_FWD_FUSED_Q): one thread turns one RAW bf16 query row of a tile in shared memory into the fp16 operand
+// row, in place: RMSNorm -> 3D RoPE -> x softmax_scale*log2(e) -> fp16, with the prologue's arithmetic in the prologue's order
+// (normrope.cuh; the chunk sums of squares are combined like prep_kernel's lane butterfly), so the bytes equal the Q^ image's.
+// Rows past the sequence end were zeroed by the producer and stay zero.
+template <int D>
+__device__ __forceinline__ void fused_q_row(const ProblemDesc& pd, const FwdParams& fp, uint8_t* tile, const SeqInfo& sq, int n, int row) {
+  constexpr int NCH = D / 8;
+  if (n >= sq.len) return;
+  const TokInfo ti = pd.tok_info[sq.tok_start + n];
+  const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);
+  float rinv = 1.0f;
+  if (!pd.no_norm) {
+    float c[NCH];
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+      float x[8];
+      unpack_bf16x8(*reinterpret_cast<const uint4*>(tile + image_off(row, ch * 8)), x);
+      c[ch] = sumsq8(x);
+    }
+#pragma unroll
+    for (int o = NCH / 2; o > 0; o >>= 1)
+#pragma unroll
+      for (int j = 0; j < NCH; ++j)
+        if ((j & o) == 0) { const float sum = c[j] + c[j ^ o]; c[j] = sum; c[j ^ o] = sum; }
+    rinv = rsqrtf(c[0] * (1.0f / D) + pd.eps);
+  }
+#pragma unroll 2
+  for (int ch = 0; ch < NCH; ++ch) {
+    uint4* p = reinterpret_cast<uint4*>(tile + image_off(row, ch * 8));
+    float x[8], gam[8];
+    unpack_bf16x8(*p, x);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) gam[i] = fp.gamma_q ? __ldg(&fp.gamma_q[ch * 8 + i]) : 1.0f;
+    float2 cs[4];
+    rope_cs4(pd.rope, ch * 8, ti, rotate, cs);
+    norm_rope_apply8(x, gam, cs, pd.no_norm != 0, rinv, fp.q_prescale);
+    *p = pack8(x, FMT_F16);
+  }
+}
+
+template <int D, int kMode, bool kFusedQ = false>
+__device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams& fp, const RawMaps& vm, const RawMaps& qm) {
   using Cfg = FwdCfg<D, kMode>;
   constexpr bool kPair = kMode == kFwdPair;      // cta_group::2 MMAs issued by the leader for both CTAs
   constexpr bool kMc = kMode == kFwdMcast;       // independent CTAs sharing the K^/V stream by multicast
@@ -103,7 +149,8 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + RING * SLOT);
   uint64_t* q_full = bars;            // producer -> MMA
   uint64_t* q_empty = bars + 1;       // MMA (commit) -> producer
-  uint64_t* kv_full = bars + 2;       // [RING]
+  uint64_t* q_ready = bars + 2;       // fused Q: softmax warps (256 arrivals) -> MMA: the Q^ tiles have been normalised in place
+  uint64_t* kv_full = bars + 3;       // [RING]
   uint64_t* kv_empty = kv_full + RING;
   uint64_t* s_full = kv_empty + RING;    // [2] MMA (commit) -> softmax of tile t
   uint64_t* p_full = s_full + 2;         // [2] softmax (128 arrivals) -> MMA
@@ -125,7 +172,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   constexpr uint32_t kArrivals = kPair ? 8 : (kWarpArrive ? 4 : 128);
   if (threadIdx.x == 0) {
     if (smem_u32(smem) & 1023u) __trap();   // tile images need 1024-byte alignment (128B swizzle atoms)
-    mbar_init(q_full, 1); mbar_init(q_empty, 1);
+    mbar_init(q_full, 1); mbar_init(q_empty, 1); mbar_init(q_ready, 256);
     for (int s = 0; s < RING; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], kMc ? 2 : 1); }
     for (int t = 0; t < 2; ++t) {
       mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kArrivals);
@@ -202,7 +249,25 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
       const uint8_t* hbase_k = fp.kt + wi.head * head_stride;
       const uint8_t* hbase_v = fp.vt + wi.head * head_stride;
       wait(q_empty, (it & 1) ^ 1);
-      if (lane == 0) {
+      bool q_is_raw = false;
+      if constexpr (kFusedQ) {
+        {      // fused Q: RAW query tiles (rawtile.cuh); the softmax warps normalise them in place
+          q_is_raw = true;
+          uint32_t bytes = 0;
+          for (int t = 0; t < n_q; ++t) {
+            const int n0 = (wi.tile + t) * kTileRows;
+            bytes += raw_tile_stage<D>(sQ + t * TILE, fp.q_raw, wi.head, sq.tok_start + n0, min(kTileRows, sq.len - n0), lane);
+          }
+          if (lane == 0) {
+            mbar_expect_tx(q_full, bytes);
+            for (int t = 0; t < n_q; ++t) {
+              const int n0 = (wi.tile + t) * kTileRows;
+              raw_tile_issue<D>(sQ + t * TILE, qm, fp.q_raw, wi.head, sq.tok_start + n0, min(kTileRows, sq.len - n0), q_full);
+            }
+          }
+        }
+      }
+      if (!q_is_raw && lane == 0) {
         mbar_expect_tx(q_full, n_q * TILE);
         if constexpr (!kCl) {
           bulk_g2s(sQ, hbase_q + static_cast<size_t>(sq.tile_base + wi.tile) * TILE, n_q * TILE, q_full);
@@ -340,6 +405,7 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
         ++cnt[t];
       };
       wait(q_full, it & 1);
+      if constexpr (kFusedQ) wait(q_ready, it & 1);      // fused Q: tiles normalised in place
       if constexpr (kPair) mbar_wait_wd(peer_q_full, it & 1);
       for (int t = 0; t < n_q; ++t) issue_s(t, 0);
       for (int j = 0; j < n_kv; ++j) {
@@ -376,6 +442,14 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
       if (item < 0) break;
       const WorkItem wi = item_list[item];
       const SeqInfo sq = pd.seqs[wi.seq];
+      if constexpr (kFusedQ) {
+        {      // fused Q: normalise this thread's row of the raw tile in place, then release the MMA warp
+          wait(q_full, it & 1);
+          if (t < tiles_per_cta(wi)) fused_q_row<D>(pd, fp, sQ + t * TILE, sq, (wi.tile + t) * kTileRows + row, row);
+          fence_proxy_async_smem();
+          mbar_arrive(q_ready);
+        }
+      }
       if (t >= tiles_per_cta(wi)) {
         // odd trailing tile: warps 4-7 sit this item out, but keep the o_free phase in step with `it`
         arrive_mma(&o_free[t]);
@@ -530,21 +604,22 @@ __device__ __forceinline__ void fwd_body(const ProblemDesc& pd, const FwdParams&
   }
 }
 
-template <int D>
-__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp, const __grid_constant__ RawMaps vmaps) {
-  fwd_body<D, kFwdSingle>(pd, fp, vmaps);
+template <int D, bool kFusedQ = false>
+__global__ void __launch_bounds__(320, 1) fwd_kernel(ProblemDesc pd, FwdParams fp, const __grid_constant__ RawMaps vmaps,
+                                                      const __grid_constant__ RawMaps qmaps) {
+  fwd_body<D, kFwdSingle, kFusedQ>(pd, fp, vmaps, qmaps);
 }
 // CTA-pair form: grid = 2 x (number of pairs), static cluster of 2 (the two SMs of a TPC)
 template <int D>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_pair_kernel(ProblemDesc pd, FwdParams fp,
                                                                                          const __grid_constant__ RawMaps vmaps) {
-  fwd_body<D, kFwdPair>(pd, fp, vmaps);      // (the pair form reads V images; the maps are unused)
+  fwd_body<D, kFwdPair>(pd, fp, vmaps, vmaps);      // (the pair form reads V images; the maps are unused)
 }
 // Multicast form: grid = 2 x (number of clusters), static cluster of 2
 template <int D>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) fwd_mc_kernel(ProblemDesc pd, FwdParams fp,
                                                                                        const __grid_constant__ RawMaps vmaps) {
-  fwd_body<D, kFwdMcast>(pd, fp, vmaps);
+  fwd_body<D, kFwdMcast>(pd, fp, vmaps, vmaps);
 }
 
 }  // namespace arachne

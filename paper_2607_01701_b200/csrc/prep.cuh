@@ -10,6 +10,7 @@
 // accesses and per-row index arithmetic; see profiles/r1_notes.md §7.
 #pragma once
 #include "common.cuh"
+#include "normrope.cuh"
 #include "sm100.cuh"
 
 namespace arachne {
@@ -30,77 +31,10 @@ struct PrepParams {
   float q_prescale;            // Q^ is multiplied by softmax_scale*log2(e) before it is rounded to fp16, so that S leaves the
                                // tensor core already in the exp2 domain — in the forward AND in the backward's recompute, which
                                // therefore sees bit-identical operands (P = exp2(S - LSE) consistent with the stored LSE)
+  int skip_q;                  // forward, ARACHNE_FLAG_FWD_FUSED_Q: no Q^ image (fwd_kernel normalises its own query tiles)
   unsigned* stats;             // nullable (forward): [0] = max_i |q~'_i|^2, [1] = max_j |k~_j|^2 as float bits (atomicMax);
                                // the forward kernel derives its logit bound from them (static-max softmax)
 };
-
-// sum over the LPR consecutive lanes that share a row
-template <int LPR>
-__device__ __forceinline__ float seg_sum(float x) {
-#pragma unroll
-  for (int o = LPR / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-  return x;
-}
-
-__device__ __forceinline__ void unpack_bf16x8(const uint4& u, float (&x)[8]) {
-  x[0] = __uint_as_float(u.x << 16); x[1] = __uint_as_float(u.x & 0xffff0000u);
-  x[2] = __uint_as_float(u.y << 16); x[3] = __uint_as_float(u.y & 0xffff0000u);
-  x[4] = __uint_as_float(u.z << 16); x[5] = __uint_as_float(u.z & 0xffff0000u);
-  x[6] = __uint_as_float(u.w << 16); x[7] = __uint_as_float(u.w & 0xffff0000u);
-}
-__device__ __forceinline__ uint4 pack8(const float (&y)[8], int fmt) {
-  uint4 u;
-  if (fmt == FMT_F16) {
-    u.x = pack_f16x2(y[0], y[1]); u.y = pack_f16x2(y[2], y[3]); u.z = pack_f16x2(y[4], y[5]); u.w = pack_f16x2(y[6], y[7]);
-  } else {
-    u.x = pack_bf16x2(y[0], y[1]); u.y = pack_bf16x2(y[2], y[3]); u.z = pack_bf16x2(y[4], y[5]); u.w = pack_bf16x2(y[6], y[7]);
-  }
-  return u;
-}
-
-// (cos, sin) of the 4 RoPE pairs of elements [d0, d0+8) at the token position packed in ti (identity when the token
-// is not rotated: text token, R21, or no_rope)
-__device__ __forceinline__ void rope_cs4(const RopeDesc& rp, int d0, const TokInfo& ti, bool rotate, float2 (&cs)[4]) {
-  const int pos[3] = {static_cast<int>(ti.t_flag & 0x7fffffffu), static_cast<int>(ti.hw >> 16), static_cast<int>(ti.hw & 0xffffu)};
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    int a = 0, p = (d0 >> 1) + i;
-    if (p >= rp.half[0]) { p -= rp.half[0]; a = 1; if (p >= rp.half[1]) { p -= rp.half[1]; a = 2; } }
-    cs[i] = rotate ? __ldg(&rp.tab[rp.off[a] + pos[a] * rp.half[a] + p]) : make_float2(1.f, 0.f);
-  }
-}
-
-// byte offset of the 16-byte chunk holding elements [d0, d0+8) of row r inside a [128][D] tile image
-__device__ __forceinline__ uint32_t image_off(int r, int d0) {
-  return static_cast<uint32_t>(d0 >> 6) * (kTileRows * 128) + swz_off(r, (d0 & 63) >> 3);
-}
-
-// x~ = RoPE(gamma * x * rsqrt(mean(x^2) + eps)) * prescale  (readings R1-R5) on this lane's 8 elements;
-// returns the lane's partial |x~|^2
-template <int D>
-__device__ __forceinline__ float norm_rope8(float (&x)[8], const float (&gam)[8], const float2 (&cs)[4], bool no_norm,
-                                            float eps, float prescale) {
-  constexpr int LPR = D / 8;
-  if (!no_norm) {
-    float ss = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) ss += x[i] * x[i];
-    ss = seg_sum<LPR>(ss);
-    const float rinv = rsqrtf(ss * (1.0f / D) + eps);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) x[i] *= rinv * gam[i];
-  }
-  float nrm = 0.f;
-#pragma unroll
-  for (int i = 0; i < 8; i += 2) {
-    const float2 c = cs[i >> 1];
-    const float x0 = x[i], x1 = x[i + 1];
-    x[i] = (x0 * c.x - x1 * c.y) * prescale;
-    x[i + 1] = (x0 * c.y + x1 * c.x) * prescale;
-    nrm += x[i] * x[i] + x[i + 1] * x[i + 1];
-  }
-  return nrm;
-}
 
 // kCopy: also write V (and, backward, dO) tile images — the path of token-range-sharded plans and of ARACHNE_FLAG_IMAGE_COPIES;
 // otherwise the main kernels read those tiles from the raw tensors by tensor-map TMA (rawtile.cuh) and pp.vt / pp.dot are null.
@@ -120,7 +54,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
   // Context parallelism: K^ / V images are needed for every tile of a sequence this rank touches, the QUERY-side data
   // (Q^ image, dO image, lse2, delta, the dq~ accumulator) only for the tiles that hold some of the rank's own rows.
   const bool touched = sq.qt_n > 0;                              // a sequence without rows of this rank: nothing to prepare
-  const bool q_side = t >= sq.qt_lo && t < sq.qt_lo + sq.qt_n;   // always true without CP
+  const bool q_side = t >= sq.qt_lo && t < sq.qt_lo + sq.qt_n && !pp.skip_q;   // always true without CP / fused Q
   if (pp.gq_zero && q_side) {
     float4* z = reinterpret_cast<float4*>(pp.gq_zero + (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * (kTileRows * D));
     for (int i = threadIdx.x; i < kTileRows * D / 4; i += 256) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);

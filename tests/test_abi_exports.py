@@ -69,7 +69,7 @@ def test_status_strings_and_validation_without_device():
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == binding.ERR_LOGIT_RANGE
     p.flags = binding.FLAG_WIDE_LOGITS
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5
-    p.flags = 128                                                                      # unknown flag bit
+    p.flags = 256                                                                      # unknown flag bit
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 12
 
 

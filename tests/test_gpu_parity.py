@@ -410,3 +410,26 @@ def test_token_strided_qkv_views_of_a_fused_projection():
             with pytest.raises(binding.ArachneError) as ei:
                 binding.plan_for(st, q_stride=bad)
             assert ei.value.status == 12
+
+
+@pytest.mark.parametrize("D", [64, 128])
+def test_forward_fused_q_equals_prologue(orc, D):
+    """ARACHNE_FLAG_FWD_FUSED_Q (the in-kernel variant of §8 a1, SURVEY §7.2 "measure both"): fwd_kernel loads its RAW query
+    tiles and applies RMSNorm + 3D RoPE + scale to them itself.  It runs the prologue's arithmetic in the prologue's order
+    (csrc/normrope.cuh), so O and LSE must equal the default path's bit for bit — ragged tails (5, 130, 136, 123, 256, 255
+    tokens), gamma != 1, and a joint sequence with un-rotated text tokens — and meet the oracle gates."""
+    from paper_2607_01701_b200 import binding
+    grids = [(1, 1, 5), (1, 10, 13), (1, 8, 17), (1, 3, 41), (1, 16, 16), (1, 15, 17)]
+    st = inputs.pack(grids, 2, D, index=7, text_lens=[0, 3, 0, 20, 0, 1])
+    t = inputs.make_inputs(st, device="cuda")
+    rng = np.random.default_rng(7)
+    gq = (1.0 + 0.25 * rng.standard_normal(D)).astype(np.float32)
+    gk = (1.0 + 0.25 * rng.standard_normal(D)).astype(np.float32)
+    base = pu.run_gpu(st, t, gamma_q=gq, gamma_k=gk, with_bwd=False, flags=binding.FLAG_WIDE_LOGITS)
+    fused = pu.run_gpu(st, t, gamma_q=gq, gamma_k=gk, with_bwd=False, flags=binding.FLAG_WIDE_LOGITS | binding.FLAG_FWD_FUSED_Q)
+    assert fused["plan"].workspace_bytes(False) == base["plan"].workspace_bytes(False)
+    assert torch.equal(fused["O"], base["O"]) and torch.equal(fused["LSE"], base["LSE"])
+    a = _np(t)
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], rope_dims=st["rope_dims"], gamma_q=gq, gamma_k=gk,
+                        text_lens=st["text_lens"])
+    pu.check_full(st, fused, ref, with_bwd=False, lse=False)
