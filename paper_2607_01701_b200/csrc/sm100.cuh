@@ -384,21 +384,21 @@ __device__ __forceinline__ float ex2_poly3(float x) {
 // Two exp2 at once with the packed fp32x2 instructions of sm_100 (FADD2 / FFMA2: one issue slot per pair): same Cody-Waite split
 // and degree-3 polynomial as ex2_poly3.
 __device__ __forceinline__ void ex2_poly3_x2(float x0, float x1, float& y0, float& y1) {
-  uint64_t v, t, f, p;
+  uint64_t v, t, p;
   asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x0), "f"(x1));
-  asm("{\n\t.reg .b64 m, c3, c2, c1, c0, u;\n\t"
+  asm("{\n\t.reg .b64 m, c3, c2, c1, c0, u, f;\n\t"
       "mov.b64 m, {0f4B400000, 0f4B400000};\n\t"          // 1.5 * 2^23
-      "mov.b64 c3, {0f3D61FBF4, 0f3D61FBF4};\n\t"         // 0.0551716685
+      "mov.b64 c3, {0f3D61FBB0, 0f3D61FBB0};\n\t"         // 0.0551716685
       "mov.b64 c2, {0f3E786F0D, 0f3E786F0D};\n\t"         // 0.2426111251
       "mov.b64 c1, {0f3F31798D, 0f3F31798D};\n\t"         // 0.6932609677
       "mov.b64 c0, {0f3F7FFB49, 0f3F7FFB49};\n\t"         // 0.9999280572
-      "add.rn.f32x2 %0, %3, m;\n\t"
+      "add.rn.f32x2 %0, %2, m;\n\t"
       "sub.rn.f32x2 u, %0, m;\n\t"
-      "sub.rn.f32x2 %1, %3, u;\n\t"
-      "fma.rn.f32x2 %2, c3, %1, c2;\n\t"
-      "fma.rn.f32x2 %2, %2, %1, c1;\n\t"
-      "fma.rn.f32x2 %2, %2, %1, c0;\n\t}\n"
-      : "=&l"(t), "=&l"(f), "=&l"(p)
+      "sub.rn.f32x2 f, %2, u;\n\t"
+      "fma.rn.f32x2 %1, c3, f, c2;\n\t"
+      "fma.rn.f32x2 %1, %1, f, c1;\n\t"
+      "fma.rn.f32x2 %1, %1, f, c0;\n\t}\n"
+      : "=&l"(t), "=&l"(p)
       : "l"(v));
   float p0, p1, t0, t1;
   asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(p));
