@@ -433,3 +433,41 @@ def test_forward_fused_q_equals_prologue(orc, D):
     ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], rope_dims=st["rope_dims"], gamma_q=gq, gamma_k=gk,
                         text_lens=st["text_lens"])
     pu.check_full(st, fused, ref, with_bwd=False, lse=False)
+
+
+def test_forward_backward_capture_into_a_cuda_graph():
+    """The calls allocate nothing, synchronise nothing and keep all per-launch state in the caller's workspace, so a forward +
+    backward can be captured into a CUDA graph once and replayed (a DiT cascade runs ~60 layers x (2 fwd + 1 bwd) on the same
+    packing).  Replays on NEW input values in the same buffers must equal eager calls bit for bit
+    (deterministic backward); the tensor maps of V / dO are kernel parameters baked into the graph, which is what fixed
+    buffers mean."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(1, 10, 13), (2, 16, 16), (1, 3, 41)], 3, 128, index=8)
+    plan = binding.plan_for(st, flags=binding.FLAG_DETERMINISTIC)
+    t = inputs.make_inputs(st, device="cuda")
+    buf = {k: v.clone() for k, v in t.items()}
+    o = torch.empty_like(buf["q"]); lse = torch.empty((plan.H, plan.N), dtype=torch.float32, device="cuda")
+    dq, dk, dv = (torch.empty_like(buf["q"]) for _ in range(3))
+    ws = torch.empty(max(plan.workspace_bytes(False), plan.workspace_bytes(True)), dtype=torch.uint8, device="cuda")
+
+    def step():
+        binding.arachne_varlen_attn_fwd(plan, buf["q"], buf["k"], buf["v"], o, lse, ws)
+        binding.arachne_varlen_attn_bwd(plan, buf["q"], buf["k"], buf["v"], o, lse, buf["dO"], dq, dk, dv, ws)
+
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        step()                                   # warm-up outside the capture (function attributes are set at plan creation)
+    side.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        step()
+    for seed in (1, 2):
+        new = {k: inputs.randn_bf16(tuple(v.shape), 4242 + 10 * seed + i, v.device) for i, (k, v) in enumerate(t.items())}
+        for k in buf:
+            buf[k].copy_(new[k])
+        g.replay()
+        torch.cuda.synchronize()
+        got = [x.clone() for x in (o, lse, dq, dk, dv)]
+        ref = pu.run_gpu(st, new, flags=binding.FLAG_DETERMINISTIC)
+        for a, k in zip(got, ("O", "LSE", "dQ", "dK", "dV")):
+            assert torch.equal(a, ref[k]), (seed, k)
