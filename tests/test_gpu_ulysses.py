@@ -188,3 +188,18 @@ def test_context_parallel_validation():
     with pytest.raises(binding.ArachneError) as e:       # a CP plan through the Ulysses backward
         binding.arachne_varlen_attn_bwd_sharded(plan, x, x, x, x, lse, x, x, x, x, ws)
     assert e.value.status == 13
+
+
+@pytest.mark.parametrize("D", [64, 128])
+def test_head_range_of_one_unsharded_tensor_uses_the_tensor_map_path(D):
+    """One token shard (the whole tensor) but only a HEAD RANGE per call (total_heads > num_heads, head_offset > 0): such a
+    plan is one-shard, so V and dO tiles come by tensor-map TMA with the head coordinate offset (rawtile.cuh RawTensor::head0).
+    The two head halves together must equal the plain call bit for bit (deterministic backward), ragged tails included."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(1, 10, 13), (1, 3, 41), (2, 16, 16)], 4, D, index=9)       # 130, 123, 512 tokens
+    t = inputs.make_inputs(st, device="cuda")
+    plain = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC)
+    halves = _run_sharded(st, t, 2, flags=binding.FLAG_DETERMINISTIC, starts=[0, st["N"]])
+    for k in ("O", "dQ", "dK", "dV"):
+        assert torch.equal(halves[k], plain[k]), k
+    assert torch.equal(halves["LSE"], plain["LSE"])
