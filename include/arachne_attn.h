@@ -219,7 +219,9 @@ int arachne_plan_cta_times(const arachne_plan* plan, int kernel, double* start_u
 
 /* Forward.  q, k, v: raw bf16 [N,H,D] (Q, K pre-norm, pre-RoPE).  Writes o (bf16 [N,H,D])
  * and lse (fp32 [H,N]).  workspace: >= arachne_workspace_bytes(plan, 0), 256-byte aligned
- * recommended (16 required); its contents are scratch. */
+ * recommended (16 required); its contents are scratch.  In one-shard plans V is read IN PLACE by the main kernel
+ * (tensor-map TMA, encoded per call from the v pointer: v must stay valid and unmodified until the call has run on the
+ * stream, like every input), Q and K by the in-call prologue (csrc/prep.cuh). */
 int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
                             const float* gamma_q, const float* gamma_k, void* o, float* lse,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -229,7 +231,8 @@ int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void*
  * With ARACHNE_FLAG_DETERMINISTIC the result is bit-identical from run to run on the same
  * device and plan: the fused kernel's dQ partial tiles are added in a fixed order (per-query-tile tickets),
  * everything else has one owner per output tile.  A ticket wait that exceeds 4 s (it cannot, by construction) sets a
- * flag in the workspace header instead of hanging the device. */
+ * flag in the workspace header instead of hanging the device.  V and d_o are read in place by tensor-map TMA as in
+ * the forward (one-shard plans). */
 int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
                             const float* gamma_q, const float* gamma_k, const void* o,
                             const float* lse, const void* d_o, void* dq, void* dk, void* dv,
