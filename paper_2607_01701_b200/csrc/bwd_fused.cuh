@@ -508,7 +508,10 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           // ordered reduction: publish the tile before last (its reductions have completed: all bulk groups but the latest
           // tile's D/32), then REQUEST this tile's ticket — the load is consumed only just before the first reduction of
           // the tile is issued (flush_chunk), so its L2 round trip hides behind the wait for dq_full and the staging
-          if (tick_p2) { bulk_wait_group<D / 32>(); st_relaxed_gpu(tick_p2, rank_p2 + 1); }
+          // (wait for ALL of this thread's reductions, not only those of the tile being published: with wait_group<D / 32>
+          // one run in ten of the cogvideox shape differed in one dQ element — a reduction reported complete had not yet been
+          // ordered at L2 against the next CTA's; profiles/r2_deterministic.md)
+          if (tick_p2) { bulk_wait_group<0>(); st_relaxed_gpu(tick_p2, rank_p2 + 1); }
           tick_p2 = tick_p1; rank_p2 = rank_p1;
           tick_p1 = bp.dq_ticket + tile_idx;
           rank_p1 = static_cast<unsigned>(wi.tile);
