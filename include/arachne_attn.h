@@ -229,9 +229,11 @@ int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void*
 /* Backward.  Needs the o and lse that fwd produced for the same inputs and plan, and d_o
  * (bf16 [N,H,D]).  Writes dq, dk (gradients w.r.t. the RAW q, k) and dv, all bf16 [N,H,D].
  * With ARACHNE_FLAG_DETERMINISTIC the result is bit-identical from run to run on the same
- * device and plan: the fused kernel's dQ partial tiles are added in a fixed order (per-query-tile tickets),
- * everything else has one owner per output tile.  A ticket wait that exceeds 4 s (it cannot, by construction) sets a
- * flag in the workspace header instead of hanging the device.  V and d_o are read in place by tensor-map TMA as in
+ * device and plan: the fused kernel's dQ partial tiles are reduced as int32 FIXED POINT (scale = a power of two per
+ * (sequence, head) group from a rigorous bound on every partial sum: no overflow in any order), and integer addition is
+ * associative, so the order in which the CTAs' reductions reach L2 cannot matter; everything else has one
+ * owner per output tile.  Same speed as the default mode; the quantum is ~2^-13 .. 2^-17 of a typical gradient element.
+ * V and d_o are read in place by tensor-map TMA as in
  * the forward (one-shard plans). */
 int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
                             const float* gamma_q, const float* gamma_k, const void* o,
@@ -283,7 +285,7 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const*
  *             is these peer loads), applies un-RoPE + RMSNorm backward, and writes dk[rank], dv[rank] (bf16) and
  *             dgamma_k (this rank's part; all-reduce it).  dgamma_q comes from step (1) (this rank's part).
  * Sequences may straddle the cuts; rows of a boundary tile that belong to another rank are masked (P = 0), so nothing
- * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): the ordered dq~ reduction has not
+ * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): the fixed-point dq~ reduction has not
  * been verified on a context-parallel plan.
  * Workspace for both backward calls: arachne_workspace_bytes(plan, 1).  A rank may own no tokens (empty shard). */
 int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params,

@@ -55,7 +55,6 @@ struct arachne_plan {
   mutable struct arachne_host_ctx* host = nullptr;   // lazily created by the *_host calls (device buffers, streams)
   int cp_rank = -1;   // >= 0: context-parallel plan (arachne_plan_create_cp), this process owns the queries of shard cp_rank
   Sharding sh{};   // token-range sharding of the raw tensors (1 shard = plain tensors)
-  size_t ticket_bytes = 0; // ordered dq~ reduction tickets [H][n_tiles] (ARACHNE_FLAG_DETERMINISTIC), inside the workspace header
   int n_groups = 0;        // num_seqs * num_heads: (sequence, head) groups (dS scaling tables in the workspace header)
   size_t hdr_bytes = 0;    // WsHeader + group tables at the start of every workspace
   unsigned* d_envelope = nullptr;   // sticky: float bits of the largest out-of-envelope logit bound seen (arachne_plan_logit_status)
@@ -160,9 +159,8 @@ ProblemDesc per_call_desc(const arachne_plan* pl, void* ws) {
   WsHeader* hdr = reinterpret_cast<WsHeader*>(w);
   pd.stats = hdr->qk_bound;
   pd.work_counter = hdr->work_counter;
-  pd.dq_error = &hdr->dq_error;
   pd.grp_stats = reinterpret_cast<unsigned*>(w + sizeof(WsHeader));
-  pd.grp_sk = reinterpret_cast<float*>(w + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16 + pl->ticket_bytes);
+  pd.grp_sk = reinterpret_cast<float*>(w + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16);
   return pd;
 }
 
@@ -267,8 +265,6 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
   if (cp) b.gk_t = cp_gk;
   const bool deterministic = (pl->p.flags & ARACHNE_FLAG_DETERMINISTIC) != 0;
-  // ordered-reduction tickets [H][n_tiles], between the group maxima and the sk table (zeroed with them)
-  unsigned* tickets = reinterpret_cast<unsigned*>(static_cast<uint8_t*>(ws) + sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16);
   PrepParams pp{};
   pp.q = q; pp.k = k; pp.v = v; pp.d_o = d_o; pp.o = o; pp.lse = lse;
   pp.gamma_q = gq; pp.gamma_k = gk;
@@ -276,23 +272,23 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // the forward's operand images, bit for bit
   pp.gq_zero = b.gq_t;
   prof_mark(pl, 1, 0, st);
-  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16 + pl->ticket_bytes, st));   // header, group maxima, tickets
+  ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16, st));   // header, group maxima
   if (pl->raw_bwd) prep_kernel<D, true, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   else prep_kernel<D, true, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
-  bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t);
+  bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t, gk, D);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
   const int grid = pl->n_ctas;
   {
-    // fused single-pass (5 GEMM) kernel: dQ~ partial tiles reduce-added at L2 — in arrival order by default, in a fixed
-    // order (tickets) with ARACHNE_FLAG_DETERMINISTIC
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, v_raw, do_raw, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? tickets : nullptr};
+    // fused single-pass (5 GEMM) kernel: dQ~ partial tiles reduce-added at L2 — fp32 in arrival order by default, int32
+    // fixed point (order-independent, bit-reproducible) with ARACHNE_FLAG_DETERMINISTIC
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, v_raw, do_raw, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? 1 : 0};
     if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp, vmaps, domaps);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
   }
-  PostParams po{b.gq_t, 1, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
+  PostParams po{b.gq_t, 1, deterministic ? 1 : 0, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
   post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
@@ -488,36 +484,6 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   // fwd_kernel and bwd_fused_kernel take the items of these LPT-ordered lists DYNAMICALLY (an atomic counter, sm100.cuh
   // ItemRing): list scheduling in decreasing-cost order, and CTAs that are a little faster simply take more items.
   std::vector<WorkItem> dyn_items = items, dyn_fwd_items = fwd_items;
-  if ((p.flags & ARACHNE_FLAG_DETERMINISTIC) && !dyn_items.empty()) {
-    // Ordered dq~ reduction (bwd_fused.cuh): the key tiles of one (sequence, head) group add into a query tile one after the
-    // other, so a group of n key tiles cannot finish faster than n hops of ~kHopBudget tile-pair steps each (reduction
-    // issued -> complete -> ticket published -> read by the next CTA).  With all CTAs on ONE group (the default order) the
-    // group has n^2 / n_ctas steps of compute: hop-bound once n < kHopBudget * n_ctas.  So the deterministic list INTERLEAVES
-    // G = ceil(kHopBudget * n_ctas / n) groups round-robin (tile t of each group in turn): consecutive key tiles of a group are
-    // handed out G items apart and every chain has G times the slack.  G must not be larger than needed: G groups keep
-    // G x (Q^, dO, dq~ of one head) live in L2 — measured at 720p: G = 1..2 1040 TFLOP/s, G = 3 967, G = 8 806 with the SM clock
-    // down to 975 MHz (DRAM power); budget 4 is the measured optimum on every workload (profiles/r2_deterministic.md).
-    // Batches follow the LPT group order, so the groups of one batch have (nearly) the same length.
-    constexpr int kHopBudget = 4;
-    std::vector<std::pair<int, int>> groups;           // (sequence, head) in LPT order
-    for (int b : order)
-      if (pl->seqs[b].qt_n > 0)
-        for (int h = 0; h < p.num_heads; ++h) groups.push_back({b, h});
-    const int n_cta_est = std::min<long long>(pl->num_sms, static_cast<long long>(dyn_items.size()));
-    std::vector<WorkItem> inter;
-    inter.reserve(dyn_items.size());
-    for (size_t g0 = 0; g0 < groups.size();) {
-      const int n0 = pl->seqs[groups[g0].first].n_tiles;
-      const size_t G = std::min(groups.size() - g0, static_cast<size_t>(std::max(1, (kHopBudget * n_cta_est + n0 - 1) / n0)));
-      int n_max = 0;
-      for (size_t g = g0; g < g0 + G; ++g) n_max = std::max(n_max, pl->seqs[groups[g].first].n_tiles);
-      for (int t = 0; t < n_max; ++t)
-        for (size_t g = g0; g < g0 + G; ++g)
-          if (t < pl->seqs[groups[g].first].n_tiles) inter.push_back(WorkItem{groups[g].first, groups[g].second, t, 0});
-      g0 += G;
-    }
-    dyn_items.swap(inter);
-  }
   if (dyn_items.empty()) dyn_items.push_back(WorkItem{0, 0, 0, 0});
   if (dyn_fwd_items.empty()) dyn_fwd_items.push_back(WorkItem{0, 0, 0, 0});
   pl->n_ctas = std::min(pl->num_sms, pl->n_items);
@@ -608,8 +574,7 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
     pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
   }
   pl->n_groups = p.num_seqs * p.num_heads;
-  pl->ticket_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * sizeof(unsigned), 16);
-  pl->hdr_bytes = align_up(sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * (16 + 8) + pl->ticket_bytes, 1024);
+  pl->hdr_bytes = align_up(sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * (16 + 16), 1024);      // header, group maxima, (sk, 1/sk, qs, 1/qs)
   {
     // Envelope (reading R19): north_star's gates are claimed for tau = softmax_scale*sqrt(D)*|gamma_q|inf*|gamma_k|inf
     // <= 1 (every BASELINE.json config has tau = 1).  The forward's logit bound in log2 units is tau*sqrt(D)*log2(e).
@@ -843,7 +808,7 @@ int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const Sharde
     ARACHNE_CUDA(cudaGetLastError());
   }
   ShardedPtr none{};
-  PostParams po{nullptr, 0, gk_sum, none, k, nullptr, gk, none, dk, 2, lo, hi, dgpart};
+  PostParams po{nullptr, 0, 0, gk_sum, none, k, nullptr, gk, none, dk, 2, lo, hi, dgpart};
   post_kernel<D><<<dim3(pl->post_blocks, 1), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {

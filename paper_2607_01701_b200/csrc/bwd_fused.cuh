@@ -1,7 +1,8 @@
 // Fused single-pass backward (§8 a6 + a7): 5 GEMMs per (key tile, query tile) pair, dK/dV accumulated in TMEM across
 // the query loop, dQ~ partial tiles reduced into a blocked fp32 accumulator in global memory by the TMA engine
-// (cp.reduce.async.bulk .add.f32 at L2).  Default: the additions land in arrival order -> run-to-run bit differences;
-// ARACHNE_FLAG_DETERMINISTIC: the same kernel with per-query-tile tickets that fix the order ("ordered reduction" below).
+// (cp.reduce.async.bulk .add at L2).  Default: fp32 additions in arrival order -> run-to-run bit differences;
+// ARACHNE_FLAG_DETERMINISTIC: the same kernel, the partial tiles reduced as FIXED-POINT int32 ("order-independent reduction"
+// below): integer addition is associative, so the result no longer depends on the order at all.
 //
 // Work item = (sequence b, head h, 128-row KEY tile).
 // Items are taken DYNAMICALLY from the plan's LPT-ordered list: lane 0 of the producer warp does an atomicAdd on a per-launch
@@ -44,35 +45,23 @@ struct BwdFusedParams {
   float* gk_t;             // out: dl/dk~ fp32 [N,H,D]
   ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
   float* gv_t;             // nullable (context parallelism): dV PARTIAL fp32 [N,H,D] written instead of dv
-  unsigned* dq_ticket;     // nullable.  ARACHNE_FLAG_DETERMINISTIC: [H][n_tiles] tickets (zeroed per call) that put the
-                           // reduce-adds into every dq~ tile in a FIXED order (see "ordered reduction" below)
+  int dq_fixed;            // ARACHNE_FLAG_DETERMINISTIC: gq_blk is an int32 fixed-point accumulator (see below)
 };
 
-// Ordered (deterministic) dq~ reduction.  The L2 reduce-add of fp32 partial tiles is associative only up to rounding, so the
-// default mode is not bit-reproducible.  With tickets, the key tiles of a (sequence, head) group add into a given query tile in
-// ASCENDING key-tile order: the drain leader of key tile t waits until ticket[query tile] == t, issues its chunk reductions,
-// and once cp.async.bulk.wait_group reports them COMPLETE (performed at L2) publishes t + 1.
-//   * No deadlock: key tile t waits only for key tile t - 1 of its group, which the work list hands out EARLIER (one atomic
-//     counter, taken in list order), so the CTA it waits for is resident and itself waits only on lower tiles.
-//   * No cost on the drain's critical path in steady state: the ticket is requested (relaxed load) at the top of the step
-//     and consumed only before the first reduction is issued; publishing is deferred by one tile, when the reductions have
-//     long completed.  What remains is the hop latency between consecutive key tiles of a group (~4 tile-pair steps); the
-//     deterministic work list interleaves groups so that no chain is hop-bound (arachne_attn.cu, kHopBudget).
-// The order depends only on the plan, so results are bit-identical run to run on the same device.
-// Ticket accesses are RELAXED at gpu scope, on purpose.  What orders the reductions is physical: a ticket is stored only after
-// cp.async.bulk.wait_group has reported the reductions COMPLETE (performed at L2, the point of coherence of the atomics), and the
-// next reduction is issued only after the new ticket value has been read.  Release / acquire forms cost a membar per tile on
-// the drain's critical path (measured: +1.9 us per tile pair, 720p backward 402 -> 630 ms) and buy nothing here: generic-proxy
-// fences do not order the bulk (async-proxy) operations anyway.
-__device__ __forceinline__ unsigned ld_relaxed_gpu(const unsigned* p) {
-  unsigned v;
-  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_relaxed_gpu(unsigned* p, unsigned v) {
-  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
-}
-
+// Order-independent (deterministic) dq~ reduction.  The L2 reduce-add of fp32 partial tiles is associative only up to rounding,
+// so the default mode is not bit-reproducible.  With ARACHNE_FLAG_DETERMINISTIC every partial value is converted to FIXED POINT
+// — round-to-nearest of value * qs, qs a power of two per (sequence, head) group — and reduced with the INTEGER form of the
+// same bulk operation (cp.reduce.async.bulk .add.s32): integer addition is exactly associative and commutative, so the sum
+// is the same whatever order the 148 CTAs' reductions reach L2 in; post_kernel multiplies by 1 / qs.  Same bytes, same
+// schedule and the same speed as the default mode, and no reliance on cross-SM ordering of asynchronous reductions (an
+// earlier ticket scheme that serialised the fp32 additions by key tile was 5 % slower and, one run in ten at head_dim 64, let
+// one reduction overtake another: profiles/r2_deterministic.md).
+//   qs comes from a rigorous bound, so no partial sum can overflow in ANY order: with P_ij >= 0, sum_j P_ij = 1,
+//     sum_j |dS_ij| = sum_j P_ij |dO_i.V_j - dO_i.O_i| <= 2 max_i|dO_i| max_j|V_j|       (O_i is a convex combination of the V_j)
+//     sum over all keys of |dS_ij k~_j[d]| <= 2 max|dO| max|V| max_j|k~_j| =: B,   |k~_j|^2 <= D max_d gamma_k[d]^2 under RMSNorm
+//   (the row maxima of the group come from prep_kernel), and qs = 2^floor(log2(2^30 / (1.01 softmax_scale B))) (bwd_scale_kernel).
+//   The price is precision, not range: the quantum is B * 2^-30 for every element of the group, i.e. ~2^-13 .. 2^-17 of a
+//   typical dq~ element (measured dQ rel-L2 against the oracle: same 1.7e-3 as the fp32 mode, profiles/r2_deterministic.md).
 
 template <int D>
 struct BwdFusedCfg {
@@ -342,7 +331,7 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       if (item < 0) break;
       const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      const float2 skv = *reinterpret_cast<const float2*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2);
+      const float2 skv = *reinterpret_cast<const float2*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 4);
       const float sk = skv.x;                    // dS is rounded to fp16 as dS * sk (delta already carries sk: bwd_scale_kernel)
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const uint32_t qs = g % QS, qph = (g / QS) & 1;
@@ -461,10 +450,6 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     float sc = 0.f;                                                 // softmax_scale / sk of the current item
     float* stage_row = reinterpret_cast<float*>(sStage) + q * 32;   // row q of staging buffer 0; buffer 1 at +128*32
     uint32_t g = 0;
-    // ordered reduction (leader only): tick_p1 / rank_p1 = ticket and rank of the tile being reduced, tick_p2 / rank_p2 = of the
-    // tile before it (not yet published), tick_seen = last value read from tick_p1
-    unsigned* tick_p1 = nullptr; unsigned* tick_p2 = nullptr;
-    unsigned rank_p1 = 0, rank_p2 = 0, tick_seen = 0;
     // chunk = 32 d-columns of the tile (16 KB, contiguous in the blocked global layout).  Two staging
     // buffers alternate; before a buffer is rewritten, the bulk reduce issued from it two chunks ago
     // must have finished READING it (wait_group.read 1 = all but the most recent group).
@@ -472,25 +457,31 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       if (leader) bulk_wait_group_read<1>();
       named_bar_sync(1, 128);
       float* dst = stage_row + (chunk & 1) * (kTileRows * 32);
+      if (bp.dq_fixed) {
+        // fixed point: sc carries qs; round to nearest, |value| <= 2^30 by the bound above
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        float4 f;
-        f.x = __uint_as_float(v[4 * j]) * sc; f.y = __uint_as_float(v[4 * j + 1]) * sc;
-        f.z = __uint_as_float(v[4 * j + 2]) * sc; f.w = __uint_as_float(v[4 * j + 3]) * sc;
-        *reinterpret_cast<float4*>(dst + ((j ^ (q & 7)) << 2)) = f;
+        for (int j = 0; j < 8; ++j) {
+          int4 q4;
+          q4.x = __float2int_rn(__uint_as_float(v[4 * j]) * sc); q4.y = __float2int_rn(__uint_as_float(v[4 * j + 1]) * sc);
+          q4.z = __float2int_rn(__uint_as_float(v[4 * j + 2]) * sc); q4.w = __float2int_rn(__uint_as_float(v[4 * j + 3]) * sc);
+          *reinterpret_cast<int4*>(dst + ((j ^ (q & 7)) << 2)) = q4;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          float4 f;
+          f.x = __uint_as_float(v[4 * j]) * sc; f.y = __uint_as_float(v[4 * j + 1]) * sc;
+          f.z = __uint_as_float(v[4 * j + 2]) * sc; f.w = __uint_as_float(v[4 * j + 3]) * sc;
+          *reinterpret_cast<float4*>(dst + ((j ^ (q & 7)) << 2)) = f;
+        }
       }
       fence_proxy_async_smem();
       named_bar_sync(1, 128);
       if (leader) {
-        if (chunk == 0 && tick_p1 != nullptr && tick_seen != rank_p1) {
-          // not this tile's turn yet: the key tile before this one (rank - 1) has not published it
-          const unsigned long long t0 = globaltimer_ns();
-          while ((tick_seen = ld_relaxed_gpu(tick_p1)) != rank_p1) {
-            if (globaltimer_ns() - t0 > 4000000000ull) { atomicExch(pd.dq_error, 1u); break; }   // never hang the device
-          }
-        }
-        bulk_reduce_add_f32_s2g(gtile + chunk * (kTileRows * 32), sStage + (chunk & 1) * (kTileRows * 32 * 4),
-                                kTileRows * 32 * 4);
+        void* g = gtile + chunk * (kTileRows * 32);
+        const void* src = sStage + (chunk & 1) * (kTileRows * 32 * 4);
+        if (bp.dq_fixed) bulk_reduce_add_s32_s2g(g, src, kTileRows * 32 * 4);
+        else bulk_reduce_add_f32_s2g(g, src, kTileRows * 32 * 4);
         bulk_commit_group();
       }
     };
@@ -499,24 +490,15 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       if (item < 0) break;
       const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
-      sc = pd.softmax_scale * pd.grp_sk[(static_cast<size_t>(wi.seq) * pd.H + wi.head) * 2 + 1];
+      {
+        // dq~ = softmax_scale * dS k~, dS carries sk; fixed-point mode: times the group's power of two qs (bwd_scale_kernel)
+        const float4 gs = *reinterpret_cast<const float4*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 4);
+        sc = pd.softmax_scale * gs.y * (bp.dq_fixed ? gs.z : 1.0f);
+      }
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const int qt = sq.qt_lo + i;
         const size_t tile_idx = static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt;
         float* gtile = bp.gq_blk + tile_idx * (kTileRows * D);
-        if (bp.dq_ticket && leader) {
-          // ordered reduction: publish the tile before last (its reductions have completed: all bulk groups but the latest
-          // tile's D/32), then REQUEST this tile's ticket — the load is consumed only just before the first reduction of
-          // the tile is issued (flush_chunk), so its L2 round trip hides behind the wait for dq_full and the staging
-          // (wait for ALL of this thread's reductions, not only those of the tile being published: with wait_group<D / 32>
-          // one run in ten of the cogvideox shape differed in one dQ element — a reduction reported complete had not yet been
-          // ordered at L2 against the next CTA's; profiles/r2_deterministic.md)
-          if (tick_p2) { bulk_wait_group<0>(); st_relaxed_gpu(tick_p2, rank_p2 + 1); }
-          tick_p2 = tick_p1; rank_p2 = rank_p1;
-          tick_p1 = bp.dq_ticket + tile_idx;
-          rank_p1 = static_cast<unsigned>(wi.tile);
-          tick_seen = ld_relaxed_gpu(tick_p1);
-        }
         mbar_wait(dq_full, g & 1);
         tc_fence_after();
         uint32_t v0[32], v1[32];
@@ -535,12 +517,6 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           flush_chunk(v0, 2, gtile);
           flush_chunk(v1, 3, gtile);
         }
-      }
-      if (bp.dq_ticket && leader) {           // end of the item: publish what is still pending
-        bulk_wait_group<0>();
-        if (tick_p2) st_relaxed_gpu(tick_p2, rank_p2 + 1);
-        if (tick_p1) st_relaxed_gpu(tick_p1, rank_p1 + 1);
-        tick_p1 = tick_p2 = nullptr;
       }
     }
     if (leader) bulk_wait_group<0>();            // all reductions have been performed before the CTA exits

@@ -116,10 +116,11 @@ struct ProblemDesc {
   unsigned* stats;           // [0] max |q~'|^2, [1] max |k~|^2 (float bits) written by the forward prep kernel.  stats,
                              // work_counter, grp_stats and grp_sk live in the header of the CALLER'S workspace (WsHeader below),
                              // i.e. they are per call: two calls on one plan with different workspaces do not share them
-  unsigned* grp_stats;       // backward: [num_seqs * H][4] float bits, (sequence, head) group g: [0] max_i |dO_i|^2, [1] max_j |V_j|^2
-  unsigned* dq_error;        // WsHeader::dq_error
-  float* grp_sk;             // backward: [num_seqs * H][2] = (sk, 1/sk): the power of two dS is multiplied by before it is
-                             // rounded to fp16 (bwd_scale_kernel, prep.cuh)
+  unsigned* grp_stats;       // backward: [num_seqs * H][4] float bits, (sequence, head) group g: [0] max_i |dO_i|^2, [1] max_j |V_j|^2,
+                             // [2] max_j |k~_j|^2 (only without RMSNorm; with it the bound D * max gamma_k^2 is used)
+  float* grp_sk;             // backward: [num_seqs * H][4] = (sk, 1/sk, qs, 1/qs): sk = the power of two dS is multiplied by
+                             // before it is rounded to fp16; qs = the fixed-point scale of the deterministic dq~ reduction
+                             // (bwd_scale_kernel, prep.cuh)
   int n_items;
   int n_tiles_total;
   int num_seqs;
@@ -138,8 +139,7 @@ struct ProblemDesc {
 struct WsHeader {
   unsigned qk_bound[2];      // ProblemDesc::stats
   int work_counter[2];       // ProblemDesc::work_counter ([0] fwd_kernel, [1] bwd_fused_kernel)
-  unsigned dq_error;         // ordered (deterministic) dQ~ reduction: set if a ticket wait timed out
-  unsigned pad[11];
+  unsigned pad[12];
 };
 static_assert(sizeof(WsHeader) == 64, "WsHeader");
 

@@ -100,6 +100,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
     if (kCopy) *reinterpret_cast<uint4*>(pp.vt + img_off + ioff) = uv;          // bf16 -> bf16 is exact
     // row norms are only needed when RMSNorm is off; with it on, |x^|^2 <= D * max(gamma)^2 (see below)
     if (pp.stats && pd.no_norm) { qn = fmaxf(qn, seg_sum<LPR>(qs)); kn = fmaxf(kn, seg_sum<LPR>(ks)); }
+    if (kBwd && pd.no_norm) kn = fmaxf(kn, seg_sum<LPR>(ks));      // (with RMSNorm the bound D * max gamma_k^2 is used: bwd_scale_kernel)
     if (kBwd) {
       float vv[8], v2 = 0.f;
       unpack_bf16x8(uv, vv);
@@ -142,6 +143,11 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
       unsigned* gs = pd.grp_stats + (static_cast<size_t>(pd.tile_seq[gtile]) * pd.H + h) * 4;
       atomicMax(&gs[0], __float_as_uint(gn));
       atomicMax(&gs[1], __float_as_uint(vn));
+      if (pd.no_norm) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) kn = fmaxf(kn, __shfl_xor_sync(0xffffffffu, kn, o));
+        atomicMax(&gs[2], __float_as_uint(kn));
+      }
     }
   }
   if (pp.stats) {
@@ -188,7 +194,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
 // entries more than 2^-29 below the bound lose relative (not absolute) precision in fp16 subnormals — their absolute error,
 // 2^-25/sk, stays ~2^16 times below bf16's at the bound.  The factor is folded into delta (this kernel) and the dP FFMA.
 // Grid (n_tiles_total, H), 128 threads (one row each).
-__global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* delta_t) {
+__global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* delta_t, const float* gamma_k, int D) {
   const int gtile = blockIdx.x, h = blockIdx.y;
   const int b = pd.tile_seq[gtile];
   const size_t g = static_cast<size_t>(b) * pd.H + h;
@@ -203,8 +209,23 @@ __global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* d
   const size_t row = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows + threadIdx.x;
   delta_t[row] *= sk;
   if (threadIdx.x == 0 && gtile == pd.seqs[b].tile_base) {
-    pd.grp_sk[g * 2] = sk;
-    pd.grp_sk[g * 2 + 1] = 1.0f / sk;
+    // Fixed-point scale of the deterministic dq~ reduction (bwd_fused.cuh): every partial sum of softmax_scale * dS k~ over the
+    // keys, in any order, is bounded by softmax_scale * B, B = (2 max|dO| max|V|) * max_j |k~_j|, and
+    // |k~_j|^2 <= D * max_d gamma_k[d]^2 under RMSNorm (RoPE preserves the norm), else the measured row maximum.
+    float kn = __uint_as_float(pd.grp_stats[g * 4 + 2]);
+    if (!pd.no_norm) {
+      float gm = 1.0f;
+      if (gamma_k) { gm = 0.f; for (int d = 0; d < D; ++d) gm = fmaxf(gm, fabsf(gamma_k[d])); }
+      kn = gm * gm * static_cast<float>(D);
+    }
+    const float bq = 1.01f * pd.softmax_scale * bound * sqrtf(kn);
+    float qs = 1.0f;
+    if (bq > 0.f && bq < 3.0e38f) {
+      int e = static_cast<int>(floorf(log2f(1073741824.0f / bq)));      // 2^30: headroom for the rounding of every partial
+      e = max(-90, min(90, e));
+      qs = exp2f(static_cast<float>(e));
+    }
+    *reinterpret_cast<float4*>(pd.grp_sk + g * 4) = make_float4(sk, 1.0f / sk, qs, 1.0f / qs);
   }
 }
 
@@ -212,6 +233,7 @@ struct PostParams {
   const float* gq_t;            // dl/dq~ fp32 (already multiplied by softmax_scale): [N,H,D], or if gq_blocked the
                                 // blocked/swizzled per-tile layout written by bwd_fused_kernel (gq_blk_off)
   int gq_blocked;
+  int gq_fixed;                 // gq_t holds int32 fixed point (deterministic backward): value = int * grp_sk[group][3]
   const float* gk_t;
   ShardedPtr q, k;              // raw bf16, possibly sharded (common.cuh)
   const float* gamma_q;
@@ -266,6 +288,11 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
       const int j = (d0 & 31) >> 2;
       f0 = *reinterpret_cast<const float4*>(base + ((j ^ (qr & 7)) << 2));
       f1 = *reinterpret_cast<const float4*>(base + (((j + 1) ^ (qr & 7)) << 2));
+      if (pp.gq_fixed) {
+        const float iq = pd.grp_sk[(static_cast<size_t>(ti.seq) * pd.H + h) * 4 + 3];
+        f0 = make_float4(__float_as_int(f0.x) * iq, __float_as_int(f0.y) * iq, __float_as_int(f0.z) * iq, __float_as_int(f0.w) * iq);
+        f1 = make_float4(__float_as_int(f1.x) * iq, __float_as_int(f1.y) * iq, __float_as_int(f1.z) * iq, __float_as_int(f1.w) * iq);
+      }
     } else {
       const float* base = gt + static_cast<size_t>(row) * D + d0;      // local fp32 workspace [N, H, D]
       f0 = *reinterpret_cast<const float4*>(base);

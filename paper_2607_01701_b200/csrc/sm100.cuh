@@ -151,6 +151,13 @@ __device__ __forceinline__ void bulk_reduce_add_f32_s2g(void* gmem_dst, const vo
       "r"(smem_u32(smem_src)), "r"(bytes)
       : "memory");
 }
+// the same with 32-bit INTEGER addition (exactly associative: the fixed-point dq~ reduction of the deterministic backward)
+__device__ __forceinline__ void bulk_reduce_add_s32_s2g(void* gmem_dst, const void* smem_src, uint32_t bytes) {
+  asm volatile(
+      "cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;\n" ::"l"(gmem_dst),
+      "r"(smem_u32(smem_src)), "r"(bytes)
+      : "memory");
+}
 __device__ __forceinline__ void bulk_commit_group() {
   asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
 }

@@ -173,9 +173,10 @@ def test_poison_neighbours_and_permutation():
 
 @pytest.mark.parametrize("name", ["bucket256", "mixed480p", "cogvideox"])
 def test_backward_is_deterministic(name):
-    """ARACHNE_FLAG_DETERMINISTIC: bit-identical run to run — the fused kernel with the ORDERED dq~ reduction (per-query-tile
-    tickets; the work list interleaves groups: bucket256 11..74 at a time, mixed480p 2..10).  The ticket waits must never
-    time out, and the result must not depend on what the workspace held."""
+    """ARACHNE_FLAG_DETERMINISTIC: bit-identical run to run — the fused kernel reduces its dq~ partial tiles as int32 fixed
+    point (integer addition is associative, so the order in which the CTAs' reductions reach L2 cannot matter).  Six runs
+    each (an earlier ordered-fp32 scheme differed in one element in one run of ten at the cogvideox shape); the result
+    must not depend on what the workspace held."""
     from paper_2607_01701_b200 import binding
     st = inputs.structure(name)
     t = inputs.make_inputs(st, device="cuda")
@@ -183,11 +184,10 @@ def test_backward_is_deterministic(name):
     ws = torch.empty(plan.workspace_bytes(True), dtype=torch.uint8, device="cuda")
     o, lse = binding.forward(plan, t["q"], t["k"], t["v"])
     runs = []
-    for _ in range(3):
-        ws.fill_(0xA5)
+    for i in range(6):
+        ws.fill_(0xA5 if i % 2 == 0 else 0x00)
         runs.append(binding.backward(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], workspace=ws))
         torch.cuda.synchronize()
-        assert int(ws[16:20].view(torch.int32).item()) == 0, "a dq~ ticket wait timed out (WsHeader::dq_error)"
     for r in runs[1:]:
         for a, b, k in zip(runs[0], r, ("dQ", "dK", "dV")):
             assert torch.equal(a, b), k
