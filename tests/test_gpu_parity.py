@@ -471,3 +471,35 @@ def test_forward_backward_capture_into_a_cuda_graph():
         ref = pu.run_gpu(st, new, flags=binding.FLAG_DETERMINISTIC)
         for a, k in zip(got, ("O", "LSE", "dQ", "dK", "dV")):
             assert torch.equal(a, ref[k]), (seed, k)
+
+
+@pytest.mark.parametrize("D", [64, 128])
+def test_run_to_run_reproducibility_of_everything_but_default_dq(D):
+    """A race between warp roles, proxies or CTAs shows up as run-to-run bit differences long before it breaks a tolerance.
+    O, LSE, dK, dV have one owner per output tile and must be bit-identical from run to run in EVERY mode, dQ in the deterministic
+    mode; 25 runs of a ragged pack (tails of 5, 2, 8, 123, 127 rows, an 18-tile sequence) per kernel form, the workspace
+    filled with a different byte before every run."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(1, 1, 5), (1, 10, 13), (1, 8, 17), (1, 3, 41), (1, 16, 16), (1, 15, 17), (9, 16, 16)], 3, D, index=5)
+    t = inputs.make_inputs(st, device="cuda")
+    forms = [0, binding.FLAG_DETERMINISTIC, binding.FLAG_FWD_FUSED_Q, binding.FLAG_IMAGE_COPIES | binding.FLAG_DETERMINISTIC]
+    if D == 128:
+        forms += [binding.FLAG_FWD_MULTICAST, binding.FLAG_FWD_CTA_PAIRS]
+    for flags in forms:
+        plan = binding.plan_for(st, flags=flags)
+        ws = torch.empty(max(plan.workspace_bytes(True), plan.workspace_bytes(False)), dtype=torch.uint8, device="cuda")
+        ref = None
+        for run in range(25):
+            ws.fill_(run * 37 % 256)
+            o, lse = binding.forward(plan, t["q"], t["k"], t["v"], workspace=ws)
+            dq, dk, dv = binding.backward(plan, t["q"], t["k"], t["v"], o, lse, t["dO"], workspace=ws)
+            torch.cuda.synchronize()
+            cur = dict(O=o, LSE=lse, dK=dk, dV=dv)
+            if flags & binding.FLAG_DETERMINISTIC:
+                cur["dQ"] = dq
+            if ref is None:
+                ref = {k: v.clone() for k, v in cur.items()}
+                continue
+            for k, v in cur.items():
+                assert torch.equal(v, ref[k]), (flags, run, k)
+        plan.close()
