@@ -285,8 +285,8 @@ int arachne_varlen_attn_bwd_sharded(const arachne_plan* plan, const void* const*
  *             is these peer loads), applies un-RoPE + RMSNorm backward, and writes dk[rank], dv[rank] (bf16) and
  *             dgamma_k (this rank's part; all-reduce it).  dgamma_q comes from step (1) (this rank's part).
  * Sequences may straddle the cuts; rows of a boundary tile that belong to another rank are masked (P = 0), so nothing
- * is counted twice.  ARACHNE_FLAG_DETERMINISTIC is rejected (ARACHNE_ERR_BAD_PARAM): the fixed-point dq~ reduction has not
- * been verified on a context-parallel plan.
+ * is counted twice.  With ARACHNE_FLAG_DETERMINISTIC the whole backward is bit-reproducible here too: dQ by the fixed-point
+ * reduction, dK / dV because the partials are added in rank order.
  * Workspace for both backward calls: arachne_workspace_bytes(plan, 1).  A rank may own no tokens (empty shard). */
 int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params,
                            const int32_t* cu_seqlens_host, const int32_t* grids_host,

@@ -346,7 +346,6 @@ int arachne_plan_create_cp(arachne_plan** out, const arachne_attn_params* params
                            const int32_t* text_lens, int32_t num_shards, const int32_t* shard_starts, int32_t rank) {
   if (!params) return ARACHNE_ERR_NULL_POINTER;
   if (rank < 0 || rank >= num_shards) return ARACHNE_ERR_BAD_SHARDING;
-  if (params->flags & ARACHNE_FLAG_DETERMINISTIC) return ARACHNE_ERR_BAD_PARAM;   // CP runs the fused backward only
   return plan_create_impl(out, params, cu, grids, text_lens, num_shards, shard_starts, params->num_heads, 0, rank);
 }
 

@@ -113,7 +113,7 @@ def test_sharded_validation():
 
 
 # ------------------------------------------------------------------ context parallelism (arachne_plan_create_cp)
-def _run_cp(st, t, starts, gamma=None):
+def _run_cp(st, t, starts, gamma=None, flags=0):
     """k virtual ranks on one GPU: rank r owns the QUERY tokens of shard r (all heads) and reads K, V of every shard."""
     from paper_2607_01701_b200 import binding
     N, H, D = st["N"], st["H"], st["D"]
@@ -122,7 +122,7 @@ def _run_cp(st, t, starts, gamma=None):
     out = {n: [torch.full_like(x, 7.0) for x in sh["q"]] for n in ("o", "dq", "dk", "dv")}
     gq, gk = (None, None) if gamma is None else (torch.as_tensor(g, dtype=torch.float32, device="cuda") for g in gamma)
     plans = [binding.Plan(st["cu_seqlens"], st["grids"], H, D, st["rope_dims"], text_lens=st.get("text_lens"),
-                          shard_starts=starts, cp_rank=r) for r in range(k)]
+                          shard_starts=starts, cp_rank=r, flags=flags) for r in range(k)]
     lses, parts_k, parts_v = [], [], []
     dgq_sum = torch.zeros(D, device="cuda", dtype=torch.float64); dgk_sum = torch.zeros_like(dgq_sum)
     for r in range(k):
@@ -179,9 +179,7 @@ def test_context_parallel_validation():
     with pytest.raises(binding.ArachneError) as e:
         binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=2)
     assert e.value.status == 13
-    with pytest.raises(binding.ArachneError) as e:
-        binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=0, flags=binding.FLAG_DETERMINISTIC)
-    assert e.value.status == 12
+    binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=0, flags=binding.FLAG_DETERMINISTIC).close()      # accepted (test below)
     plan = binding.Plan(**kw, shard_starts=[0, 32, 64], cp_rank=1)
     x = [torch.zeros(32, 2, 64, dtype=torch.bfloat16, device="cuda") for _ in range(2)]
     lse = torch.empty(2, 64, device="cuda"); ws = torch.empty(plan.workspace_bytes(True), dtype=torch.uint8, device="cuda")
@@ -203,3 +201,19 @@ def test_head_range_of_one_unsharded_tensor_uses_the_tensor_map_path(D):
     for k in ("O", "dQ", "dK", "dV"):
         assert torch.equal(halves[k], plain[k]), k
     assert torch.equal(halves["LSE"], plain["LSE"])
+
+
+def test_context_parallel_deterministic_mode(orc):
+    """ARACHNE_FLAG_DETERMINISTIC on context-parallel plans: dQ through the int32 fixed-point reduction (order-independent), dK / dV
+    through the rank-ordered sum of the partials — three runs bit-identical, and inside the oracle gates."""
+    from paper_2607_01701_b200 import binding
+    st = inputs.pack([(2, 9, 11), (1, 8, 8), (3, 10, 13)], 3, 128, index=6)
+    t = inputs.make_inputs(st, device="cuda")
+    starts = [0, 100, 300, 652]
+    runs = [_run_cp(st, t, starts, flags=binding.FLAG_DETERMINISTIC) for _ in range(3)]
+    for r in runs[1:]:
+        for k in ("O", "LSE", "dQ", "dK", "dV"):
+            assert torch.equal(r[k], runs[0][k]), k
+    a = {n: v.float().cpu().numpy().astype(np.float64) for n, v in t.items()}
+    ref = orc.attention(a["q"], a["k"], a["v"], st["cu_seqlens"], st["grids"], dO=a["dO"], rope_dims=st["rope_dims"])
+    pu.check_full(st, runs[0], ref)
