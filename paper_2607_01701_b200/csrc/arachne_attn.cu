@@ -80,7 +80,7 @@ struct arachne_plan {
   ProblemDesc pd{};
   // workspace layout
   size_t tile_bytes = 0, img_bytes = 0, rowvec_bytes = 0, grad_bytes = 0, gradblk_bytes = 0, dgpart_bytes = 0;
-  int post_blocks = 0;   // post_kernel grid.x (grid-stride over the N*H rows); fixes the dgamma summation order
+  int post_blocks = 0;   // post_kernel grid.x (grid-stride over groups of tokens); fixes the dgamma summation order
   // optional per-kernel timing (arachne_plan_enable_profiling): ring of kProfSlots calls per pass,
   // kernels+1 events per call, recorded on the caller's stream (no synchronisation).
   static constexpr int kProfSlots = 32;
@@ -567,9 +567,8 @@ static int plan_create_impl(arachne_plan** out, const arachne_attn_params* param
   pl->grad_bytes = align_up(static_cast<size_t>(p.total_tokens) * p.num_heads * p.head_dim * sizeof(float), 1024);
   pl->gradblk_bytes = align_up(static_cast<size_t>(p.num_heads) * pl->n_tiles_total * kTileRows * p.head_dim * sizeof(float), 1024);
   {
-    const long long rows = static_cast<long long>(p.total_tokens) * p.num_heads;
-    const int rpb = 8 * (32 / (p.head_dim / 8));          // rows per post_kernel block and step (8 warps x RPW)
-    pl->post_blocks = static_cast<int>(std::min<long long>((rows + rpb - 1) / rpb, static_cast<long long>(pl->num_sms) * 8));
+    const int tpb = 8 * (32 / (p.head_dim / 8));          // tokens per post_kernel block and step (8 warps x RPW), all heads each
+    pl->post_blocks = static_cast<int>(std::min<long long>((static_cast<long long>(p.total_tokens) + tpb - 1) / tpb, static_cast<long long>(pl->num_sms) * 8));
     pl->dgpart_bytes = align_up(static_cast<size_t>(2) * pl->post_blocks * p.head_dim * sizeof(float), 1024);
   }
   pl->n_groups = p.num_seqs * p.num_heads;

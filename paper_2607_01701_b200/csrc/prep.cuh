@@ -246,10 +246,15 @@ struct PostParams {
 
 // dx = r*u - r^3 * x * (sum_d u_d x_d)/D,  u = gamma * R^T g~   (§8 a8; oracle: norm_rope_row_bwd)
 // dl/dgamma_d += (R^T g~)_d * x_d * r                            (reading R22)
-// Grid (nblk, 2): y = 0 -> dQ, y = 1 -> dK.  Warps walk the (token, head) rows with a grid stride, RPW rows per
-// warp and step, so a lane's dgamma partial stays in registers until the end; the per-block partials are then
-// summed in block order by dgamma_reduce_kernel (fixed order: run-to-run bit-reproducible for a given plan,
-// whichever backward produced g~).
+// Grid (nblk, 2): y = 0 -> dQ, y = 1 -> dK.  TOKEN-major: a warp takes RPW tokens per step (grid stride over the token groups)
+// and walks ALL heads of them in an inner loop, so everything that depends on the token only — its TokInfo, the cos / sin of
+// its RoPE pairs, its shard and row offsets, its place in the blocked dq~ layout — is set up once per token instead of once
+// per (token, head) row, and consecutive iterations read consecutive 2*D-byte rows of the raw tensor (the kernel was
+// instruction-issue-bound, ~390 instructions per row pair: profiles/r2_prologue.md).  A lane's dgamma partial stays in
+// registers until the end; the per-block partials are then summed in block order by dgamma_reduce_kernel (fixed order:
+// run-to-run bit-reproducible for a given plan, whichever backward produced g~).
+// (4 blocks / SM and no unrolling of the head loop measured best: occupancy matters more than ILP here; 3 blocks / SM without
+// the 40-byte spill is 20 % slower, profiles/r2_prologue.md)
 template <int D>
 __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams pp) {
   constexpr int LPR = D / 8, RPW = 32 / LPR;
@@ -265,73 +270,76 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
   float gam[8], dgam[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) { gam[i] = gamma ? __ldg(&gamma[d0 + i]) : 1.0f; dgam[i] = 0.f; }
-  const int n_rows = pp.tok_hi * pd.H;                         // < 2^31 (checked by the plan)
+  const long long dense = static_cast<long long>(pd.sh.H_total) * D;
+  const size_t blk_head_stride = static_cast<size_t>(pd.n_tiles_total) * (kTileRows * D);     // floats between heads, blocked dq~
   const int stride = gridDim.x * 8 * RPW;
-#pragma unroll 2
-  for (int row0 = pp.tok_lo * pd.H + (blockIdx.x * 8 + warp) * RPW; row0 < n_rows; row0 += stride) {   // warp-uniform trip count
-    const bool live = row0 + sub < n_rows;                     // ragged end: the lane keeps shuffling, stores nothing
-    const int row = live ? row0 + sub : n_rows - 1;            // (token, head)
-    const int tok = row / pd.H, h = row - tok * pd.H;
+  for (int tok0 = pp.tok_lo + (blockIdx.x * 8 + warp) * RPW; tok0 < pp.tok_hi; tok0 += stride) {   // warp-uniform trip count
+    const bool live = tok0 + sub < pp.tok_hi;                  // ragged end: the lane keeps shuffling, stores nothing
+    const int tok = live ? tok0 + sub : pp.tok_hi - 1;
+    // ---- per token
     const TokInfo ti = pd.tok_info[tok];
     const bool rotate = !pd.no_rope && !(ti.t_flag >> 31);     // R21: text tokens were not rotated
+    float2 cs[4];
+    rope_cs4(pd.rope, d0, ti, rotate, cs);
     int shard;
-    const long long dense = static_cast<long long>(pd.sh.H_total) * D;
-    const size_t roff = raw_off(pd.sh, dense, tok, h, D, shard) + d0;                                           // output row (contiguous)
-    const size_t xoff = roff + static_cast<long long>(tok - pd.sh.start[shard]) * (pd.in_stride[is_k ? 1 : 0] - dense);   // raw Q / K row (may be token-strided)
-    const uint4 ux = *reinterpret_cast<const uint4*>(shard_base<const __nv_bfloat16>(xraw_s, shard) + xoff);
-    float4 f0, f1;
+    const size_t roff0 = raw_off(pd.sh, dense, tok, 0, D, shard) + d0;                                        // output row of head 0 (contiguous)
+    const size_t xoff0 = roff0 + static_cast<long long>(tok - pd.sh.start[shard]) * (pd.in_stride[is_k ? 1 : 0] - dense);   // raw Q / K row (may be token-strided)
+    const __nv_bfloat16* xbase = shard_base<const __nv_bfloat16>(xraw_s, shard) + xoff0;
+    __nv_bfloat16* obase = shard_base<__nv_bfloat16>(out_s, shard) + roff0;
+    const float* g0p; const float* g1p; size_t gstep;
     if (blocked) {
       // blocked layout [H][tile][D/32][128 rows][32], 16-byte pieces XOR-swizzled with (row & 7) (bwd_fused.cuh)
-      const int qr = ti.blkrow & (kTileRows - 1);
-      const float* base = gt + (static_cast<size_t>(h) * pd.n_tiles_total + (ti.blkrow >> 7)) * (kTileRows * D) +
-                          static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32;
-      const int j = (d0 & 31) >> 2;
-      f0 = *reinterpret_cast<const float4*>(base + ((j ^ (qr & 7)) << 2));
-      f1 = *reinterpret_cast<const float4*>(base + (((j + 1) ^ (qr & 7)) << 2));
-      if (pp.gq_fixed) {
-        const float iq = pd.grp_sk[(static_cast<size_t>(ti.seq) * pd.H + h) * 4 + 3];
+      const int qr = ti.blkrow & (kTileRows - 1), j = (d0 & 31) >> 2;
+      const float* base = gt + static_cast<size_t>(ti.blkrow >> 7) * (kTileRows * D) + static_cast<size_t>(d0 >> 5) * (kTileRows * 32) + qr * 32;
+      g0p = base + ((j ^ (qr & 7)) << 2); g1p = base + (((j + 1) ^ (qr & 7)) << 2); gstep = blk_head_stride;
+    } else {
+      g0p = gt + static_cast<size_t>(tok) * pd.H * D + d0; g1p = g0p + 4; gstep = D;      // local fp32 workspace [N, H, D]
+    }
+    const float* iqp = pp.gq_fixed && blocked ? pd.grp_sk + static_cast<size_t>(ti.seq) * pd.H * 4 + 3 : nullptr;
+    // ---- per (token, head) row
+#pragma unroll 1
+    for (int h = 0; h < pd.H; ++h) {
+      const uint4 ux = *reinterpret_cast<const uint4*>(xbase + static_cast<size_t>(h) * D);
+      float4 f0 = *reinterpret_cast<const float4*>(g0p + h * gstep);
+      float4 f1 = *reinterpret_cast<const float4*>(g1p + h * gstep);
+      if (iqp) {      // int32 fixed point (deterministic backward): value = int / qs of the (sequence, head) group
+        const float iq = iqp[h * 4];
         f0 = make_float4(__float_as_int(f0.x) * iq, __float_as_int(f0.y) * iq, __float_as_int(f0.z) * iq, __float_as_int(f0.w) * iq);
         f1 = make_float4(__float_as_int(f1.x) * iq, __float_as_int(f1.y) * iq, __float_as_int(f1.z) * iq, __float_as_int(f1.w) * iq);
       }
-    } else {
-      const float* base = gt + static_cast<size_t>(row) * D + d0;      // local fp32 workspace [N, H, D]
-      f0 = *reinterpret_cast<const float4*>(base);
-      f1 = *reinterpret_cast<const float4*>(base + 4);
-    }
-    float g[8] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w};
-    float x[8];
-    unpack_bf16x8(ux, x);
-    float2 cs[4];
-    rope_cs4(pd.rope, d0, ti, rotate, cs);
+      float g[8] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w};
+      float x[8];
+      unpack_bf16x8(ux, x);
 #pragma unroll
-    for (int i = 0; i < 8; i += 2) {
-      const float2 c = cs[i >> 1];
-      const float g0 = g[i], g1 = g[i + 1];
-      g[i] = g0 * c.x + g1 * c.y;          // rotate by -phi
-      g[i + 1] = -g0 * c.y + g1 * c.x;
-    }
-    float y[8];
-    if (!pd.no_norm) {
-      float ss = 0.f, uxs = 0.f;
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        ss += x[i] * x[i];
-        uxs += gam[i] * g[i] * x[i];
+      for (int i = 0; i < 8; i += 2) {
+        const float2 c = cs[i >> 1];
+        const float ga = g[i], gb = g[i + 1];
+        g[i] = ga * c.x + gb * c.y;          // rotate by -phi
+        g[i + 1] = -ga * c.y + gb * c.x;
       }
-      ss = seg_sum<LPR>(ss);
-      uxs = seg_sum<LPR>(uxs);
-      const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
-      const float c = rinv * rinv * rinv * uxs * (1.0f / D);
+      float y[8];
+      if (!pd.no_norm) {
+        float ss = 0.f, uxs = 0.f;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        y[i] = rinv * gam[i] * g[i] - c * x[i];
-        if (live) dgam[i] += g[i] * x[i] * rinv;
+        for (int i = 0; i < 8; ++i) {
+          ss += x[i] * x[i];
+          uxs += gam[i] * g[i] * x[i];
+        }
+        ss = seg_sum<LPR>(ss);
+        uxs = seg_sum<LPR>(uxs);
+        const float rinv = rsqrtf(ss * (1.0f / D) + pd.eps);
+        const float c = rinv * rinv * rinv * uxs * (1.0f / D);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          y[i] = rinv * gam[i] * g[i] - c * x[i];
+          if (live) dgam[i] += g[i] * x[i] * rinv;
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) y[i] = g[i];      // gamma unused: dgamma = 0
       }
-    } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) y[i] = g[i];      // gamma unused: dgamma = 0
+      if (live) *reinterpret_cast<uint4*>(obase + static_cast<size_t>(h) * D) = pack8(y, FMT_BF16);
     }
-    if (live) *reinterpret_cast<uint4*>(shard_base<__nv_bfloat16>(out_s, shard) + roff) = pack8(y, FMT_BF16);
   }
   if (pp.dgamma_part) {
 #pragma unroll
