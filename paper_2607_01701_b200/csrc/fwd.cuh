@@ -9,13 +9,17 @@
 //
 //   issue order   S0_0 S1_0 | PV0_0 S0_1 PV1_0 S1_1 | PV0_1 S0_2 PV1_1 S1_2 | ...
 //
-//   warp 8  producer : cp.async.bulk  Q^ images, then K^_j / V_j images into a ring of tile slots
+//   warp 8  producer : Q^ images (cp.async.bulk), then K^_j (cp.async.bulk of the image) and V_j (tensor-map TMA straight from
+//                      the caller's tensor, rawtile.cuh; an image only for sharded plans) into a ring of tile slots
 //   warp 9  MMA      : S_t,j = Q^_t K^_j^T  (SS, fp16 x fp16 -> fp32 TMEM, one buffer per query tile)
 //                      O_t  += P_t,j V_j    (TS: P bf16 in TMEM aliasing S_t; V MN-major)
-//   warps 0-3 / 4-7  : softmax of query tile 0 / 1, one query row per thread: tcgen05.ld S row,
-//                      online softmax in the exp2 domain with LAZY rescaling (O is only rescaled
-//                      when the row max grew by > 2^8; QK-RMSNorm bounds the logits so this is
-//                      rare), P -> bf16 -> tcgen05.st, final O / l -> bf16, LSE -> fp32.
+//   warps 0-3 / 4-7  : softmax of query tile 0 / 1, one query row per thread: tcgen05.ld S row, exp2, P -> bf16 -> tcgen05.st,
+//                      handed to the MMA warp in two halves of 64 keys (kSplitP) so that PV of the first half runs under the
+//                      exponentiation of the second; final O / l -> bf16, LSE -> fp32.  QK-RMSNorm bounds the logits, so the
+//                      default is a STATIC max (p = 2^s, no running max, no rescale); unbounded logits (no_norm, huge gamma)
+//                      take online softmax with LAZY rescaling (O only rescaled when a row max grew by > 2^8).
+// Forms: fwd_kernel (one CTA per item; <D, true> = fused Q, the in-kernel A/B of §8 a1), fwd_pair_kernel (cluster of 2,
+// cta_group::2 MMAs), fwd_mc_kernel (cluster of 2 sharing the K^/V stream by TMA multicast).
 //
 // Q^, K^ are fp16 (RMSNorm bounds |x^_d| <= gamma_max * sqrt(D)); fp16 operands put the LSE
 // error floor at ~2e-4 instead of ~1.5e-3 for bf16.  P and V are bf16.

@@ -1,13 +1,17 @@
-// Elementwise (HBM-bound) kernels around the tensor-core kernels:
-//   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> fp16 operand tile images;
-//                 V, dO -> tile images (zero-padded tails); D_i = rowsum(dO*O); LSE*log2e padded.
-//   post_kernel : §8 a8.  dq~, dk~ (fp32) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK (+ dgamma partials, R22).
+// Elementwise (HBM / issue-bound) kernels around the tensor-core kernels:
+//   prep_kernel : §8 a1 + a5.  raw Q,K -> RMSNorm -> 3D RoPE -> fp16 operand tile images; backward: D_i = rowsum(dO*O),
+//                 LSE*log2e (padded), per-group maxima for the dS / fixed-point scales; V, dO -> tile images (zero-padded
+//                 tails) ONLY in the copy variant (sharded plans, ARACHNE_FLAG_IMAGE_COPIES) — otherwise the main kernels read
+//                 them from the raw tensors by tensor-map TMA (rawtile.cuh).
+//   post_kernel : §8 a8.  dq~, dk~ (fp32, or int32 fixed point) -> un-RoPE -> RMSNorm backward -> bf16 dQ, dK (+ dgamma
+//                 partials, R22).
 // Thread mapping: a lane owns 8 contiguous elements (one 16-byte bf16 load / store, one swizzle chunk of a tile
 // image), so a (token, head) row takes LPR = D/8 lanes and a warp works on RPW = 32/LPR rows at once (2 at D = 128,
 // 4 at D = 64).  Both elements of every RoPE pair (2p, 2p+1) sit in the same lane; the only cross-lane work is the
 // sum over the LPR lanes of a row.  Token positions come from the plan's per-token table (TokInfo) — no integer
-// divisions and no search over cu_seqlens on the device.  These kernels were instruction-issue-bound with 8-byte
-// accesses and per-row index arithmetic; see profiles/r1_notes.md §7.
+// divisions and no search over cu_seqlens on the device.  prep_kernel: one block per (tile, head); post_kernel: token-major
+// with an inner loop over heads.  Both are bound by instruction issue as much as by HBM (profiles/r1_notes.md §7,
+// profiles/r2_prologue.md).
 #pragma once
 #include "common.cuh"
 #include "normrope.cuh"
