@@ -71,6 +71,21 @@ def test_status_strings_and_validation_without_device():
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5
     p.flags = 256                                                                      # unknown flag bit
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 12
+    # every flag the header declares is accepted (validation goes on to the grid check) ...
+    p.softmax_scale = 0.0
+    for f in (binding.FLAG_DETERMINISTIC, binding.FLAG_NO_NORM, binding.FLAG_NO_ROPE, binding.FLAG_WIDE_LOGITS, binding.FLAG_FWD_CTA_PAIRS,
+              binding.FLAG_IMAGE_COPIES, binding.FLAG_FWD_MULTICAST, binding.FLAG_FWD_FUSED_Q, 255):
+        p.flags = f
+        assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5, f
+    # ... and the token strides of Q / K / V (elements): multiples of 8, >= num_heads * head_dim (no overlapping rows)
+    p.flags = 0
+    for name in ("q_stride", "k_stride", "v_stride"):
+        for bad in (2 * 64 - 8, 2 * 64 + 4, -128):
+            setattr(p, name, bad)
+            assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 12, (name, bad)
+        setattr(p, name, 3 * 2 * 64)                                                    # a slice of a fused [N, 3, H, D] projection
+        assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5
+        setattr(p, name, 0)
 
 
 def test_binding_rejects_tensors_the_c_side_cannot_check():
