@@ -58,7 +58,9 @@ typedef enum {
   ARACHNE_ERR_BAD_SHAPE = 11,        /* num_seqs/num_heads/total_tokens <= 0, or too large  */
   ARACHNE_ERR_BAD_PARAM = 12,        /* non-finite / non-positive theta, eps < 0, bad flags */
   ARACHNE_ERR_BAD_SHARDING = 13,     /* see arachne_plan_create_sharded; or a sharded plan passed to a plain call */
-  ARACHNE_ERR_LOGIT_RANGE = 14       /* tau > 1 without ARACHNE_FLAG_WIDE_LOGITS: see "Verified envelope" below      */
+  ARACHNE_ERR_LOGIT_RANGE = 14,      /* tau > 1 without ARACHNE_FLAG_WIDE_LOGITS: see "Verified envelope" below      */
+  ARACHNE_ERR_BUILTIN_SCRATCH = 15   /* arachne_varlen_attn_fwd_noalloc: the packing needs more scratch than the library's
+                                        built-in ARACHNE_BUILTIN_SCRATCH_BYTES; sizes in arachne_last_error_message      */
 } arachne_status;
 
 enum {
@@ -225,6 +227,46 @@ int arachne_plan_cta_times(const arachne_plan* plan, int kernel, double* start_u
 int arachne_varlen_attn_fwd(const arachne_plan* plan, const void* q, const void* k, const void* v,
                             const float* gamma_q, const float* gamma_k, void* o, float* lse,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Forward for call sites that have NO device memory to offer as a workspace and no way of getting any.
+ *
+ * Who that is.  arachne_varlen_attn_fwd wants a caller-owned workspace, which in practice means somebody called cudaMalloc
+ * (or asked a framework allocator that did).  Some users of this library sit where that is not possible: an attention
+ * layer plugged into a training process whose caching allocator has already reserved the GPU's memory, so a second,
+ * raw cudaMalloc from inside the layer fails or forces the framework to give its cache back; a C host that is handed
+ * tensor pointers by its embedder and nothing else — no allocator handle, no permission to create device buffers of its
+ * own; and per-layer call sites in a steady-state step loop, where cudaMalloc / cudaFree are banned because they
+ * serialise the whole device behind them.  Such a caller still has a plan (built once at set-up by whoever owns the
+ * process, where allocation is allowed) and the tensors q, k, v, o, lse.  This call needs nothing more.
+ *
+ * What it does.  The same two launches as arachne_varlen_attn_fwd (prologue + fwd_kernel, same results), except that the
+ * scratch they share — the workspace header and the Q^ / K^ operand images — lives in an array compiled into the library
+ * (a file-scope `static __device__` array of ARACHNE_BUILTIN_SCRATCH_BYTES bytes).  Every GPU on which the library's code
+ * gets loaded carries those bytes until the process exits, whether or not this call is ever made; that is why the limit
+ * is kept small.  The call itself performs no cudaMalloc, cudaFree or any other allocating routine.
+ *
+ * Limit.  arachne_workspace_bytes(plan, 0) must be <= ARACHNE_BUILTIN_SCRATCH_BYTES (32 MiB: about 65 000 (token, head)
+ * rows at head_dim 128, twice that at 64, counting each sequence rounded up to whole 128-token tiles).  Anything larger
+ * is refused with ARACHNE_ERR_BUILTIN_SCRATCH before a kernel is launched, and arachne_last_error_message says how many
+ * bytes were needed; use arachne_varlen_attn_fwd with a workspace for those.
+ *
+ * First call on a device.  The device address of the array is looked up (cudaGetSymbolAddress) the first time this
+ * function runs on a given device, with that device current, and remembered.  The look-up may make the CUDA runtime load
+ * the library's device code, so make one call on each device during set-up, before any stream capture is begun;
+ * later calls only read the remembered address.  The plan's device must be the current device (else ARACHNE_ERR_BAD_PARAM).
+ *
+ * Sharing.  There is ONE array per device, used by every call of this function from every plan and thread in the process.
+ * It still holds whatever the previous call left in it; the words that have to start at zero (the workspace header:
+ * logit bound, dynamic work counters) are cleared on the stream at the start of every call, everything else is
+ * overwritten before it is read.  Two calls whose kernels can overlap on the GPU — different streams, or different host
+ * threads — would write over each other's operand images: keep all calls on a device ordered on one stream (or by
+ * events).  arachne_varlen_attn_fwd with separate workspaces remains the way to run forwards concurrently.
+ *
+ * Arguments, layouts, alignment and every other status as arachne_varlen_attn_fwd (one-shard plans only). */
+#define ARACHNE_BUILTIN_SCRATCH_BYTES (32u << 20)
+int arachne_varlen_attn_fwd_noalloc(const arachne_plan* plan, const void* q, const void* k, const void* v,
+                                    const float* gamma_q, const float* gamma_k, void* o, float* lse,
+                                    void* cuda_stream);
 
 /* Backward.  Needs the o and lse that fwd produced for the same inputs and plan, and d_o
  * (bf16 [N,H,D]).  Writes dq, dk (gradients w.r.t. the RAW q, k) and dv, all bf16 [N,H,D].

@@ -20,6 +20,8 @@ _lib = ctypes.CDLL(_LIB_PATH)
 
 FLAG_DETERMINISTIC, FLAG_NO_NORM, FLAG_NO_ROPE, FLAG_WIDE_LOGITS, FLAG_FWD_CTA_PAIRS, FLAG_IMAGE_COPIES, FLAG_FWD_MULTICAST, FLAG_FWD_FUSED_Q = 1, 2, 4, 8, 16, 32, 64, 128
 ERR_LOGIT_RANGE = 14
+ERR_BUILTIN_SCRATCH = 15
+BUILTIN_SCRATCH_BYTES = 32 << 20      # ARACHNE_BUILTIN_SCRATCH_BYTES (include/arachne_attn.h)
 
 EXPORTS = [
     "arachne_plan_create", "arachne_plan_destroy", "arachne_workspace_bytes", "arachne_num_launches",
@@ -30,7 +32,7 @@ EXPORTS = [
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
     "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
     "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free", "arachne_plan_cta_times",
-    "arachne_plan_logit_status",
+    "arachne_plan_logit_status", "arachne_varlen_attn_fwd_noalloc",
 ]
 
 
@@ -59,6 +61,8 @@ _lib.arachne_num_launches.restype = ctypes.c_int
 _lib.arachne_num_launches.argtypes = [_vp, ctypes.c_int]
 _lib.arachne_varlen_attn_fwd.restype = ctypes.c_int
 _lib.arachne_varlen_attn_fwd.argtypes = [_vp] * 8 + [_vp, ctypes.c_size_t, _vp]
+_lib.arachne_varlen_attn_fwd_noalloc.restype = ctypes.c_int
+_lib.arachne_varlen_attn_fwd_noalloc.argtypes = [_vp] * 8 + [_vp]
 _lib.arachne_varlen_attn_bwd.restype = ctypes.c_int
 _lib.arachne_varlen_attn_bwd.argtypes = [_vp] * 12 + [_vp, ctypes.c_size_t, _vp]
 _lib.arachne_varlen_attn_bwd_dgamma.restype = ctypes.c_int
@@ -117,7 +121,7 @@ class ArachneError(RuntimeError):
         self.status = status
         msg = _lib.arachne_status_string(status).decode()
         detail = _lib.arachne_last_error_message().decode()
-        super().__init__(f"arachne status {status}: {msg}" + (f" ({detail})" if status == 10 and detail else ""))
+        super().__init__(f"arachne status {status}: {msg}" + (f" ({detail})" if status in (10, ERR_BUILTIN_SCRATCH) and detail else ""))
 
 
 def _check(status: int):
@@ -266,6 +270,21 @@ def arachne_varlen_attn_fwd(plan: Plan, q, k, v, o, lse, workspace, gamma_q=None
     _check(_lib.arachne_varlen_attn_fwd(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
                                         _ptr(lse), _ptr(workspace), workspace.numel() * workspace.element_size(),
                                         _stream_ptr(stream)))
+
+
+def arachne_varlen_attn_fwd_noalloc(plan: Plan, q, k, v, o, lse, gamma_q=None, gamma_k=None, stream=None):
+    """The forward for callers with no workspace to give: same tensors as arachne_varlen_attn_fwd, no workspace argument.
+
+    Meant for code that cannot obtain device memory where it runs — a layer inside a process whose framework allocator
+    already owns the GPU, an embedded C host that is only handed tensor pointers, a step loop where cudaMalloc / cudaFree
+    are off limits because they stall the device.  The scratch is a 32 MiB array built into the library
+    (BUILTIN_SCRATCH_BYTES), one per GPU, shared by every call: plans whose plan.workspace_bytes(False) exceeds it raise
+    ArachneError(ERR_BUILTIN_SCRATCH); calls that could overlap on the GPU (two streams) corrupt each other, so keep them
+    on one stream.  Make the first call on each device during set-up (it looks the array's address up).  Nothing is
+    allocated here either: o and lse come from the caller."""
+    _want_call(plan, dict(q=q, k=k, v=v, o=o), lse, (("gamma_q", gamma_q), ("gamma_k", gamma_k)))
+    _check(_lib.arachne_varlen_attn_fwd_noalloc(plan._h, _ptr(q), _ptr(k), _ptr(v), _ptr(gamma_q), _ptr(gamma_k), _ptr(o),
+                                                _ptr(lse), _stream_ptr(stream)))
 
 
 def arachne_varlen_attn_bwd(plan: Plan, q, k, v, o, lse, d_o, dq, dk, dv, workspace, gamma_q=None, gamma_k=None,

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -321,6 +322,7 @@ const char* arachne_status_string(int s) {
     case ARACHNE_ERR_BAD_PARAM: return "bad parameter";
     case ARACHNE_ERR_BAD_SHARDING: return "bad sharding (1..8 shards, starts 0..N non-decreasing, head_offset + num_heads <= total_heads)";
     case ARACHNE_ERR_LOGIT_RANGE: return "logit range outside the verified envelope (softmax_scale*sqrt(D)*|gamma_q|inf*|gamma_k|inf > 1): pass ARACHNE_FLAG_WIDE_LOGITS";
+    case ARACHNE_ERR_BUILTIN_SCRATCH: return "packing too large for the built-in scratch of arachne_varlen_attn_fwd_noalloc (32 MiB): use arachne_varlen_attn_fwd with a workspace";
     default: return "unknown status";
   }
 }
@@ -1016,3 +1018,62 @@ int arachne_varlen_attn_fwd_bwd_host(const arachne_plan* pl, const void* q_h, co
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------- forward without any caller- or library-allocated scratch
+// arachne_varlen_attn_fwd_noalloc (include/arachne_attn.h): for callers that cannot get device memory at all — a layer
+// living inside a process whose framework allocator already holds the GPU's memory, a C host that only ever receives
+// tensor pointers from its embedder, a step loop in which cudaMalloc / cudaFree are forbidden because they stall the
+// device.  The forward's scratch (workspace header + Q^ / K^ operand images) is this array instead of a workspace argument.
+//
+// The array is part of the library's device image: every GPU that loads the image holds kBuiltinScratchBytes of it until the
+// process ends.  In HOST code the identifier below is only a handle for the runtime's symbol table, never a device address
+// (handing it to a kernel would fault, or quietly address host memory where the GPU can reach it): the host side must ask
+// cudaGetSymbolAddress, with the right device current, and pass the pointer it gets.  Kernels in this file could also name
+// the array directly; launch_fwd's kernels take the workspace as a pointer, so the pointer route serves both entry points.
+constexpr size_t kBuiltinScratchBytes = ARACHNE_BUILTIN_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_builtin_scratch[kBuiltinScratchBytes];
+
+namespace {
+constexpr int kMaxBuiltinDevices = 64;
+std::mutex g_builtin_mu;
+void* g_builtin_ptr[kMaxBuiltinDevices] = {};      // device address of g_builtin_scratch on device i (0 = not looked up yet)
+
+// Once per device, with that device current.  Not an allocation — the bytes came with the module — but the look-up may be
+// what makes a lazily-loading runtime bring the module in, hence the header's "first call before any stream capture".
+int builtin_scratch(int dev, void** out) {
+  if (dev < 0 || dev >= kMaxBuiltinDevices) { g_last_error = "device ordinal beyond the built-in scratch table"; return ARACHNE_ERR_BAD_PARAM; }
+  std::lock_guard<std::mutex> lock(g_builtin_mu);
+  if (!g_builtin_ptr[dev]) {
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_builtin_scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_builtin_scratch)");
+    if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) { g_last_error = "built-in scratch: bad symbol address"; return ARACHNE_ERR_CUDA; }
+    g_builtin_ptr[dev] = ptr;
+  }
+  *out = g_builtin_ptr[dev];
+  return ARACHNE_OK;
+}
+}  // namespace
+
+extern "C" int arachne_varlen_attn_fwd_noalloc(const arachne_plan* pl, const void* q, const void* k, const void* v,
+                                               const float* gamma_q, const float* gamma_k, void* o, float* lse,
+                                               void* stream) {
+  if (!pl || !q || !k || !v || !o || !lse) return ARACHNE_ERR_NULL_POINTER;
+  if (pl->sh.n_shards != 1) return ARACHNE_ERR_BAD_SHARDING;
+  const size_t need = fwd_ws_bytes(pl);
+  if (need > kBuiltinScratchBytes) {      // refused before anything is enqueued
+    g_last_error = "arachne_varlen_attn_fwd_noalloc: this packing needs " + std::to_string(need) + " bytes of scratch, the built-in array has " +
+                   std::to_string(kBuiltinScratchBytes) + "; call arachne_varlen_attn_fwd with a workspace instead";
+    return ARACHNE_ERR_BUILTIN_SCRATCH;
+  }
+  int dev = -1;
+  ARACHNE_CUDA(cudaGetDevice(&dev));
+  if (dev != pl->device) { g_last_error = "arachne_varlen_attn_fwd_noalloc: the plan was built on another device than the current one"; return ARACHNE_ERR_BAD_PARAM; }
+  void* scratch = nullptr;
+  const int rc = builtin_scratch(dev, &scratch);
+  if (rc != ARACHNE_OK) return rc;
+  // From here on this IS arachne_varlen_attn_fwd: same validation, same launches (launch_fwd clears the workspace header —
+  // the only words that must start at zero — on the stream before the prologue; the operand images, tail padding
+  // included, are written by the prologue before fwd_kernel reads them), with the built-in array as the workspace.
+  return arachne_varlen_attn_fwd(pl, q, k, v, gamma_q, gamma_k, o, lse, scratch, kBuiltinScratchBytes, stream);
+}

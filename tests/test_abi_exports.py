@@ -31,7 +31,7 @@ def test_status_strings_and_validation_without_device():
     from paper_2607_01701_b200 import binding
 
     lib = binding._lib
-    for s in range(0, 15):
+    for s in range(0, 16):
         assert lib.arachne_status_string(s).decode() not in ("", "unknown status")
     assert lib.arachne_status_string(99).decode() == "unknown status"
     assert lib.arachne_workspace_bytes(None, 0) == 0
@@ -55,6 +55,7 @@ def test_status_strings_and_validation_without_device():
     gr2 = (ctypes.c_int32 * 3)(1, 8, 9)
     assert lib.arachne_plan_create(ctypes.byref(h), ctypes.byref(p), cu, gr2) == 5    # grid mismatch
     assert lib.arachne_varlen_attn_fwd(None, None, None, None, None, None, None, None, None, 0, None) == 1
+    assert lib.arachne_varlen_attn_fwd_noalloc(None, None, None, None, None, None, None, None, None) == 1
     # 32-bit row indices on the device: tokens x heads must stay below 2^31 (rejected before any CUDA call)
     big = binding.AttnParams()
     big.num_seqs, big.total_tokens, big.num_heads, big.head_dim = 1, 2 ** 27, 16, 64
