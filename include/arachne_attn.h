@@ -272,9 +272,12 @@ int arachne_varlen_attn_fwd_noalloc(const arachne_plan* plan, const void* q, con
  * (bf16 [N,H,D]).  Writes dq, dk (gradients w.r.t. the RAW q, k) and dv, all bf16 [N,H,D].
  * With ARACHNE_FLAG_DETERMINISTIC the result is bit-identical from run to run on the same
  * device and plan: the fused kernel's dQ partial tiles are reduced as int32 FIXED POINT (scale = a power of two per
- * (sequence, head) group from a rigorous bound on every partial sum: no overflow in any order), and integer addition is
- * associative, so the order in which the CTAs' reductions reach L2 cannot matter; everything else has one
- * owner per output tile.  Same speed as the default mode; the quantum is ~2^-13 .. 2^-17 of a typical gradient element.
+ * (token, head) query row from a rigorous bound on every partial sum of that row, 2 |dO_i| max|V| max|k~|: no overflow in any
+ * order), and integer addition is associative, so the order in which the CTAs' reductions reach L2 cannot matter (DESIGN.md
+ * §5); everything else has one owner per output tile.  Same speed as the default mode; the quantum is ~2^-13 .. 2^-17 of a
+ * typical element of the same row, however large or small that row's dO is (an outlying V row 2^k above typical costs every
+ * row of its (sequence, head) group k of those bits).  The bound presumes lse is the forward's own; a dQ row that saw a
+ * non-finite or out-of-range partial comes back as NaN (never silently wrapped or zeroed).
  * V and d_o are read in place by tensor-map TMA as in
  * the forward (one-shard plans). */
 int arachne_varlen_attn_bwd(const arachne_plan* plan, const void* q, const void* k, const void* v,

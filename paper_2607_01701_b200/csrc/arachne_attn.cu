@@ -110,10 +110,11 @@ int configure_kernels() {
 }
 
 struct FwdWs { uint8_t *qt, *kt, *vt; };
-struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *gq_t, *gk_t; };
+struct BwdWs { uint8_t *qt, *kt, *vt, *dot; float *lse2_t, *delta_t, *rowqs_t, *gq_t, *gk_t; };
 
 size_t fwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + pl->n_img_fwd * pl->img_bytes; }
-size_t bwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 2 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
+// (3 row vectors: lse2, delta and the per-row fixed-point scales of the deterministic dq~ reduction)
+size_t bwd_ws_bytes(const arachne_plan* pl) { return pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 3 * pl->rowvec_bytes + pl->grad_bytes + pl->gradblk_bytes + pl->dgpart_bytes; }
 
 // Tensor maps over a raw [tokens, H_total, D] bf16 tensor (rawtile.cuh): encoded on the host per call (the base pointer is a
 // call argument), ~1 us each, passed to the kernel as __grid_constant__ parameters.  cuTensorMapEncodeTiled is taken from
@@ -261,6 +262,7 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   }
   b.lse2_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.delta_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
+  b.rowqs_t = reinterpret_cast<float*>(w); w += pl->rowvec_bytes;
   b.gk_t = reinterpret_cast<float*>(w); w += pl->grad_bytes;
   b.gq_t = reinterpret_cast<float*>(w); w += pl->gradblk_bytes;     // gradblk_bytes >= grad_bytes: either layout fits
   float* dgpart = (dgq || dgk) ? reinterpret_cast<float*>(w) : nullptr;
@@ -272,24 +274,25 @@ int launch_bwd(const arachne_plan* pl, const ShardedPtr& q, const ShardedPtr& k,
   pp.qt = b.qt; pp.kt = b.kt; pp.vt = b.vt; pp.dot = b.dot; pp.lse2_t = b.lse2_t; pp.delta_t = b.delta_t;
   pp.q_prescale = pl->p.softmax_scale * 1.4426950408889634f;   // the forward's operand images, bit for bit
   pp.gq_zero = b.gq_t;
+  pp.rowqs_t = deterministic ? b.rowqs_t : nullptr;
   prof_mark(pl, 1, 0, st);
   ARACHNE_CUDA(cudaMemsetAsync(ws, 0, sizeof(WsHeader) + static_cast<size_t>(pl->n_groups) * 16, st));   // header, group maxima
   if (pl->raw_bwd) prep_kernel<D, true, false><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   else prep_kernel<D, true, true><<<dim3(pl->n_tiles_total, pl->p.num_heads), 256, 0, st>>>(pd, pp);
   ARACHNE_CUDA(cudaGetLastError());
-  bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t, gk, D);
+  bwd_scale_kernel<<<dim3(pl->n_tiles_total, pl->p.num_heads), 128, 0, st>>>(pd, b.delta_t, gk, D, pp.rowqs_t);
   ARACHNE_CUDA(cudaGetLastError());
   prof_mark(pl, 1, 1, st);
   const int grid = pl->n_ctas;
   {
     // fused single-pass (5 GEMM) kernel: dQ~ partial tiles reduce-added at L2 — fp32 in arrival order by default, int32
     // fixed point (order-independent, bit-reproducible) with ARACHNE_FLAG_DETERMINISTIC
-    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, v_raw, do_raw, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? 1 : 0};
+    BwdFusedParams bp{b.qt, b.kt, b.vt, b.dot, v_raw, do_raw, b.lse2_t, b.delta_t, b.gq_t, b.gk_t, dv, cp_gv, deterministic ? 1 : 0, b.rowqs_t};
     if (grid > 0) bwd_fused_kernel<D><<<grid, BwdFusedCfg<D>::kThreads, BwdFusedCfg<D>::kSmemBytes, st>>>(pd, bp, vmaps, domaps);
     ARACHNE_CUDA(cudaGetLastError());
     prof_mark(pl, 1, 2, st);
   }
-  PostParams po{b.gq_t, 1, deterministic ? 1 : 0, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart};
+  PostParams po{b.gq_t, 1, deterministic ? 1 : 0, b.gk_t, q, k, gq, gk, dq, dk, cp ? 1 : 0, pl->pd.cp_lo, pl->pd.cp_hi, dgpart, b.rowqs_t};
   post_kernel<D><<<dim3(pl->post_blocks, cp ? 1 : 2), 256, 0, st>>>(pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {
@@ -796,7 +799,7 @@ template <int D>
 int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const ShardedPtr& gvp, const ShardedPtr& k, const float* gk,
                      const ShardedPtr& dk, const ShardedPtr& dv, float* dgk, void* ws, cudaStream_t st) {
   uint8_t* w = static_cast<uint8_t*>(ws);
-  w += pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 2 * pl->rowvec_bytes;   // same carving as launch_bwd: gk_t, gq_t, dgamma partials
+  w += pl->hdr_bytes + pl->n_img_bwd * pl->img_bytes + 3 * pl->rowvec_bytes;   // same carving as launch_bwd: gk_t, gq_t, dgamma partials
   float* gk_sum = reinterpret_cast<float*>(w); w += pl->grad_bytes + pl->gradblk_bytes;
   float* dgpart = dgk ? reinterpret_cast<float*>(w) : nullptr;
   const int lo = pl->pd.cp_lo, hi = pl->pd.cp_hi;
@@ -808,7 +811,7 @@ int launch_cp_reduce(const arachne_plan* pl, const ShardedPtr& gkp, const Sharde
     ARACHNE_CUDA(cudaGetLastError());
   }
   ShardedPtr none{};
-  PostParams po{nullptr, 0, 0, gk_sum, none, k, nullptr, gk, none, dk, 2, lo, hi, dgpart};
+  PostParams po{nullptr, 0, 0, gk_sum, none, k, nullptr, gk, none, dk, 2, lo, hi, dgpart, nullptr};
   post_kernel<D><<<dim3(pl->post_blocks, 1), 256, 0, st>>>(pl->pd, po);
   ARACHNE_CUDA(cudaGetLastError());
   if (dgpart) {

@@ -46,22 +46,33 @@ struct BwdFusedParams {
   ShardedPtr dv;           // out: bf16 [N,H_total,D], possibly sharded by token range (common.cuh)
   float* gv_t;             // nullable (context parallelism): dV PARTIAL fp32 [N,H,D] written instead of dv
   int dq_fixed;            // ARACHNE_FLAG_DETERMINISTIC: gq_blk is an int32 fixed-point accumulator (see below)
+  float* rowqs_t;          // dq_fixed: [H][n_tiles][128] fixed-point scale of every query row (bwd_scale_kernel); a drain thread
+                           // overwrites its row's entry with NaN when a partial is non-finite or out of range
 };
 
 // Order-independent (deterministic) dq~ reduction.  The L2 reduce-add of fp32 partial tiles is associative only up to rounding,
 // so the default mode is not bit-reproducible.  With ARACHNE_FLAG_DETERMINISTIC every partial value is converted to FIXED POINT
-// — round-to-nearest of value * qs, qs a power of two per (sequence, head) group — and reduced with the INTEGER form of the
-// same bulk operation (cp.reduce.async.bulk .add.s32): integer addition is exactly associative and commutative, so the sum
-// is the same whatever order the 148 CTAs' reductions reach L2 in; post_kernel multiplies by 1 / qs.  Same bytes, same
-// schedule and the same speed as the default mode, and no reliance on cross-SM ordering of asynchronous reductions (an
+// — round-to-nearest of value * qs_i, qs_i a power of two per QUERY ROW i (per (token, head)) — and reduced with the INTEGER
+// form of the same bulk operation (cp.reduce.async.bulk .add.s32): integer addition is exactly associative and commutative, so
+// the sum is the same whatever order the 148 CTAs' reductions reach L2 in; post_kernel multiplies by 1 / qs_i.  Same bytes,
+// same schedule and the same speed as the default mode, and no reliance on cross-SM ordering of asynchronous reductions (an
 // earlier ticket scheme that serialised the fp32 additions by key tile was 5 % slower and, one run in ten at head_dim 64, let
 // one reduction overtake another: profiles/r2_deterministic.md).
-//   qs comes from a rigorous bound, so no partial sum can overflow in ANY order: with P_ij >= 0, sum_j P_ij = 1,
-//     sum_j |dS_ij| = sum_j P_ij |dO_i.V_j - dO_i.O_i| <= 2 max_i|dO_i| max_j|V_j|       (O_i is a convex combination of the V_j)
-//     sum over all keys of |dS_ij k~_j[d]| <= 2 max|dO| max|V| max_j|k~_j| =: B,   |k~_j|^2 <= D max_d gamma_k[d]^2 under RMSNorm
-//   (the row maxima of the group come from prep_kernel), and qs = 2^floor(log2(2^30 / (1.01 softmax_scale B))) (bwd_scale_kernel).
-//   The price is precision, not range: the quantum is B * 2^-30 for every element of the group, i.e. ~2^-13 .. 2^-17 of a
-//   typical dq~ element (measured dQ rel-L2 against the oracle: same 1.7e-3 as the fp32 mode, profiles/r2_deterministic.md).
+//   qs_i comes from a rigorous bound, so no partial sum can overflow in ANY order: with P_ij >= 0, sum_j P_ij = 1,
+//     sum_j |dS_ij| = sum_j P_ij |dO_i.V_j - dO_i.O_i| <= 2 |dO_i| max_j|V_j|                 (O_i is a convex combination of the V_j)
+//     sum over all keys of |dS_ij k~_j[d]| <= 2 |dO_i| max|V| max_j|k~_j| =: B_i,   |k~_j|^2 <= D max_d gamma_k[d]^2 under RMSNorm
+//   (|dO_i| and the group's max|V| come from prep_kernel), and qs_i = 2^floor(log2(2^30 / (1.01 softmax_scale B_i))) (bwd_scale_kernel).
+//   The price is precision, not range: the quantum of row i is B_i * 2^-30, i.e. ~2^-13 .. 2^-17 of a typical element of THAT
+//   row whatever its size (measured dQ rel-L2 against the oracle: same 1.7e-3 as the fp32 mode, profiles/r2_deterministic.md).
+//   Because the scale follows the row's own |dO_i|, a token with an outlying upstream gradient costs the other rows nothing
+//   (a scale per (sequence, head) group, as in round 2, left them log2(outlier / typical) bits short).  What still costs bits
+//   is an outlying VALUE row: max_j|V_j| enters every row's bound, because any row may attend to it; a V row 2^k above typical
+//   takes k of the ~13-17 spare bits from every row of its (sequence, head) group (tests/test_gpu_parity.py, heavy-tailed case).
+//   The bound needs sum_j P_ij = 1, i.e. the LSE passed to the backward must be the forward's for the same inputs (the ABI's
+//   precondition).  A partial that is non-finite or beyond 2^30 after scaling — NaN / inf in the inputs, or an LSE so foreign
+//   that a single tile already breaks the bound — is not silently wrapped or dropped (cvt.rni.s32 turns NaN into 0): the drain
+//   thread overwrites the row's scale with NaN and post_kernel emits NaN for that dQ row, as the fp32 mode would.  A foreign
+//   LSE whose tiles each stay in range but whose SUM leaves int32 cannot be seen by anybody (the additions happen in L2).
 
 template <int D>
 struct BwdFusedCfg {
@@ -447,7 +458,9 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tdQ = tbase + Cfg::kColDP + lane_base;
     const bool leader = threadIdx.x == 256;
-    float sc = 0.f;                                                 // softmax_scale / sk of the current item
+    float sc = 0.f;                                                 // softmax_scale / sk of the current item (x the row's qs, fixed point)
+    float sc_item = 0.f;
+    float amax = 0.f;                                               // fixed point: largest |scaled partial| of the current tile (NaN if any was)
     float* stage_row = reinterpret_cast<float*>(sStage) + q * 32;   // row q of staging buffer 0; buffer 1 at +128*32
     uint32_t g = 0;
     // chunk = 32 d-columns of the tile (16 KB, contiguous in the blocked global layout).  Two staging
@@ -458,12 +471,16 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       named_bar_sync(1, 128);
       float* dst = stage_row + (chunk & 1) * (kTileRows * 32);
       if (bp.dq_fixed) {
-        // fixed point: sc carries qs; round to nearest, |value| <= 2^30 by the bound above
+        // fixed point: sc carries the row's qs; round to nearest, |value| <= 2^30 by the bound above (amax checks it: a
+        // NaN-propagating maximum, one FMNMX per value)
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
+          const float f0 = __uint_as_float(v[4 * j]) * sc, f1 = __uint_as_float(v[4 * j + 1]) * sc;
+          const float f2 = __uint_as_float(v[4 * j + 2]) * sc, f3 = __uint_as_float(v[4 * j + 3]) * sc;
+          amax = max_nan(max_nan(amax, fabsf(f0)), fabsf(f1));
+          amax = max_nan(max_nan(amax, fabsf(f2)), fabsf(f3));
           int4 q4;
-          q4.x = __float2int_rn(__uint_as_float(v[4 * j]) * sc); q4.y = __float2int_rn(__uint_as_float(v[4 * j + 1]) * sc);
-          q4.z = __float2int_rn(__uint_as_float(v[4 * j + 2]) * sc); q4.w = __float2int_rn(__uint_as_float(v[4 * j + 3]) * sc);
+          q4.x = __float2int_rn(f0); q4.y = __float2int_rn(f1); q4.z = __float2int_rn(f2); q4.w = __float2int_rn(f3);
           *reinterpret_cast<int4*>(dst + ((j ^ (q & 7)) << 2)) = q4;
         }
       } else {
@@ -491,14 +508,16 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
       const WorkItem wi = pd.dyn_items[item];
       const SeqInfo sq = pd.seqs[wi.seq];
       {
-        // dq~ = softmax_scale * dS k~, dS carries sk; fixed-point mode: times the group's power of two qs (bwd_scale_kernel)
-        const float4 gs = *reinterpret_cast<const float4*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 4);
-        sc = pd.softmax_scale * gs.y * (bp.dq_fixed ? gs.z : 1.0f);
+        // dq~ = softmax_scale * dS k~, dS carries sk; fixed-point mode: times the query row's power of two qs_i (bwd_scale_kernel)
+        const float2 gs = *reinterpret_cast<const float2*>(pd.grp_sk + (static_cast<size_t>(wi.seq) * pd.H + wi.head) * 4);
+        sc = sc_item = pd.softmax_scale * gs.y;
       }
       for (int i = 0; i < sq.qt_n; ++i, ++g) {
         const int qt = sq.qt_lo + i;
         const size_t tile_idx = static_cast<size_t>(wi.head) * pd.n_tiles_total + sq.tile_base + qt;
         float* gtile = bp.gq_blk + tile_idx * (kTileRows * D);
+        float* row_qs = bp.rowqs_t + tile_idx * kTileRows + q;       // (dereferenced in fixed-point mode only)
+        if (bp.dq_fixed) { sc = sc_item * *row_qs; amax = 0.f; }
         mbar_wait(dq_full, g & 1);
         tc_fence_after();
         uint32_t v0[32], v1[32];
@@ -517,6 +536,9 @@ __global__ void __launch_bounds__(512, 1) bwd_fused_kernel(ProblemDesc pd, BwdFu
           flush_chunk(v0, 2, gtile);
           flush_chunk(v1, 3, gtile);
         }
+        // All writers of a row's mark store the same value and a concurrent reader that picks it up produces NaN partials
+        // (-> 0 after cvt) and marks the row again: the row's dQ is NaN either way.
+        if (bp.dq_fixed && !(amax <= 1073741824.0f)) *row_qs = __int_as_float(0x7fc00000);
       }
     }
     if (leader) bulk_wait_group<0>();            // all reductions have been performed before the CTA exits

@@ -118,9 +118,9 @@ struct ProblemDesc {
                              // i.e. they are per call: two calls on one plan with different workspaces do not share them
   unsigned* grp_stats;       // backward: [num_seqs * H][4] float bits, (sequence, head) group g: [0] max_i |dO_i|^2, [1] max_j |V_j|^2,
                              // [2] max_j |k~_j|^2 (only without RMSNorm; with it the bound D * max gamma_k^2 is used)
-  float* grp_sk;             // backward: [num_seqs * H][4] = (sk, 1/sk, qs, 1/qs): sk = the power of two dS is multiplied by
-                             // before it is rounded to fp16; qs = the fixed-point scale of the deterministic dq~ reduction
-                             // (bwd_scale_kernel, prep.cuh)
+  float* grp_sk;             // backward: [num_seqs * H][4] = (sk, 1/sk, -, -): sk = the power of two dS is multiplied by
+                             // before it is rounded to fp16 (bwd_scale_kernel, prep.cuh).  (The fixed-point scale of the
+                             // deterministic dq~ reduction is per query ROW: BwdFusedParams::rowqs_t.)
   int n_items;
   int n_tiles_total;
   int num_seqs;

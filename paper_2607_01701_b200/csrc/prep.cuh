@@ -32,6 +32,8 @@ struct PrepParams {
   float* lse2_t;               // [H][n_tiles][128]  lse * log2(e); +inf on pad rows
   float* delta_t;              // [H][n_tiles][128]  rowsum(dO*O);  0 on pad rows
   float* gq_zero;              // nullable: blocked dq~ accumulator [H][n_tiles][128*D] to clear (fused backward)
+  float* rowqs_t;              // nullable (deterministic backward): [H][n_tiles][128] out: |dO_i| of every query row, 0 on pad rows;
+                               // bwd_scale_kernel turns it in place into the row's fixed-point scale (bwd_fused.cuh)
   float q_prescale;            // Q^ is multiplied by softmax_scale*log2(e) before it is rounded to fp16, so that S leaves the
                                // tensor core already in the exp2 domain — in the forward AND in the backward's recompute, which
                                // therefore sees bit-identical operands (P = exp2(S - LSE) consistent with the stored LSE)
@@ -124,11 +126,13 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
       float g2 = 0.f;
 #pragma unroll
       for (int i = 0; i < 8; ++i) g2 += g[i] * g[i];
-      gn = fmaxf(gn, seg_sum<LPR>(g2));
+      g2 = seg_sum<LPR>(g2);
+      gn = fmaxf(gn, g2);
       if (d0 == 0) {
         // context parallelism: query rows of other ranks behave like pad rows here (P = 0: no dK/dV contribution)
         const bool live = valid && tok >= pd.cp_lo && tok < pd.cp_hi;
         pp.delta_t[row_off + r] = live ? dsum : 0.f;
+        if (pp.rowqs_t) pp.rowqs_t[row_off + r] = live ? sqrtf(g2) : 0.f;
         // pad rows get +inf so that P = exp2(s - inf) = 0 for them in the backward kernels
         pp.lse2_t[row_off + r] = live ? pp.lse[static_cast<size_t>(h) * pd.N + tok] * 1.4426950408889634f
                                        : __int_as_float(0x7f800000);
@@ -198,7 +202,7 @@ __global__ void __launch_bounds__(256, 4) prep_kernel(ProblemDesc pd, PrepParams
 // entries more than 2^-29 below the bound lose relative (not absolute) precision in fp16 subnormals — their absolute error,
 // 2^-25/sk, stays ~2^16 times below bf16's at the bound.  The factor is folded into delta (this kernel) and the dP FFMA.
 // Grid (n_tiles_total, H), 128 threads (one row each).
-__global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* delta_t, const float* gamma_k, int D) {
+__global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* delta_t, const float* gamma_k, int D, float* rowqs_t) {
   const int gtile = blockIdx.x, h = blockIdx.y;
   const int b = pd.tile_seq[gtile];
   const size_t g = static_cast<size_t>(b) * pd.H + h;
@@ -212,24 +216,35 @@ __global__ void __launch_bounds__(128) bwd_scale_kernel(ProblemDesc pd, float* d
   }
   const size_t row = (static_cast<size_t>(h) * pd.n_tiles_total + gtile) * kTileRows + threadIdx.x;
   delta_t[row] *= sk;
-  if (threadIdx.x == 0 && gtile == pd.seqs[b].tile_base) {
-    // Fixed-point scale of the deterministic dq~ reduction (bwd_fused.cuh): every partial sum of softmax_scale * dS k~ over the
-    // keys, in any order, is bounded by softmax_scale * B, B = (2 max|dO| max|V|) * max_j |k~_j|, and
-    // |k~_j|^2 <= D * max_d gamma_k[d]^2 under RMSNorm (RoPE preserves the norm), else the measured row maximum.
+  if (threadIdx.x == 0 && gtile == pd.seqs[b].tile_base) *reinterpret_cast<float2*>(pd.grp_sk + g * 4) = make_float2(sk, 1.0f / sk);
+  if (rowqs_t) {
+    // Fixed-point scale of the deterministic dq~ reduction (bwd_fused.cuh), one per QUERY ROW: every partial sum of
+    // softmax_scale * dS_i. k~ over the keys, in any order, is bounded by softmax_scale * B_i,
+    //   B_i = 2 |dO_i| max_j|V_j| * max_j |k~_j|,   |k~_j|^2 <= D * max_d gamma_k[d]^2 under RMSNorm (RoPE preserves the norm),
+    // else the measured row maximum.  The scale follows the row's OWN |dO_i| (prep_kernel left it in rowqs_t), so a token with
+    // an outlying upstream gradient takes resolution from nobody else: each row keeps ~30 bits below its own bound.
+    __shared__ float s_gm[4];
     float kn = __uint_as_float(pd.grp_stats[g * 4 + 2]);
     if (!pd.no_norm) {
       float gm = 1.0f;
-      if (gamma_k) { gm = 0.f; for (int d = 0; d < D; ++d) gm = fmaxf(gm, fabsf(gamma_k[d])); }
+      if (gamma_k) {
+        gm = threadIdx.x < D ? fabsf(gamma_k[threadIdx.x]) : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) gm = fmaxf(gm, __shfl_xor_sync(0xffffffffu, gm, o));
+        if ((threadIdx.x & 31) == 0) s_gm[threadIdx.x >> 5] = gm;
+        __syncthreads();
+        gm = fmaxf(fmaxf(s_gm[0], s_gm[1]), fmaxf(s_gm[2], s_gm[3]));
+      }
       kn = gm * gm * static_cast<float>(D);
     }
-    const float bq = 1.01f * pd.softmax_scale * bound * sqrtf(kn);
-    float qs = 1.0f;
-    if (bq > 0.f && bq < 3.0e38f) {
+    const float bq = 1.01f * pd.softmax_scale * 2.02f * rowqs_t[row] * sqrtf(vn) * sqrtf(kn);
+    float qs = 1.0f;                          // |dO_i| = 0 (pad rows too): every partial is exactly 0
+    if (bq > 0.f && bq < 3.0e38f) {           // (false for NaN: the drain then marks the row, bwd_fused.cuh)
       int e = static_cast<int>(floorf(log2f(1073741824.0f / bq)));      // 2^30: headroom for the rounding of every partial
       e = max(-90, min(90, e));
       qs = exp2f(static_cast<float>(e));
     }
-    *reinterpret_cast<float4*>(pd.grp_sk + g * 4) = make_float4(sk, 1.0f / sk, qs, 1.0f / qs);
+    rowqs_t[row] = qs;
   }
 }
 
@@ -237,7 +252,7 @@ struct PostParams {
   const float* gq_t;            // dl/dq~ fp32 (already multiplied by softmax_scale): [N,H,D], or if gq_blocked the
                                 // blocked/swizzled per-tile layout written by bwd_fused_kernel (gq_blk_off)
   int gq_blocked;
-  int gq_fixed;                 // gq_t holds int32 fixed point (deterministic backward): value = int * grp_sk[group][3]
+  int gq_fixed;                 // gq_t holds int32 fixed point (deterministic backward): value = int / rowqs_t[head][blocked row]
   const float* gk_t;
   ShardedPtr q, k;              // raw bf16, possibly sharded (common.cuh)
   const float* gamma_q;
@@ -246,6 +261,8 @@ struct PostParams {
   int which;                    // 0: y = 0 -> dQ, y = 1 -> dK;  1: dQ only (grid.y = 1);  2: dK only (grid.y = 1)
   int tok_lo, tok_hi;           // only (token, head) rows with tok in [tok_lo, tok_hi) are processed (CP; else 0, N)
   float* dgamma_part;           // nullable: [2][gridDim.x][D] per-block partial sums of dl/dgamma_q, dl/dgamma_k (R22)
+  const float* rowqs_t;         // gq_fixed: [H][n_tiles][128] fixed-point scale of every query row (a power of two; NaN = the row
+                                // overflowed or saw a non-finite partial: its dQ is NaN, bwd_fused.cuh)
 };
 
 // dx = r*u - r^3 * x * (sum_d u_d x_d)/D,  u = gamma * R^T g~   (§8 a8; oracle: norm_rope_row_bwd)
@@ -299,15 +316,18 @@ __global__ void __launch_bounds__(256, 4) post_kernel(ProblemDesc pd, PostParams
     } else {
       g0p = gt + static_cast<size_t>(tok) * pd.H * D + d0; g1p = g0p + 4; gstep = D;      // local fp32 workspace [N, H, D]
     }
-    const float* iqp = pp.gq_fixed && blocked ? pd.grp_sk + static_cast<size_t>(ti.seq) * pd.H * 4 + 3 : nullptr;
+    const float* iqp = pp.gq_fixed && blocked ? pp.rowqs_t + ti.blkrow : nullptr;
+    const size_t iq_head_stride = static_cast<size_t>(pd.n_tiles_total) * kTileRows;
     // ---- per (token, head) row
 #pragma unroll 1
     for (int h = 0; h < pd.H; ++h) {
       const uint4 ux = *reinterpret_cast<const uint4*>(xbase + static_cast<size_t>(h) * D);
       float4 f0 = *reinterpret_cast<const float4*>(g0p + h * gstep);
       float4 f1 = *reinterpret_cast<const float4*>(g1p + h * gstep);
-      if (iqp) {      // int32 fixed point (deterministic backward): value = int / qs of the (sequence, head) group
-        const float iq = iqp[h * 4];
+      if (iqp) {      // int32 fixed point (deterministic backward): value = int / qs of this (token, head) row
+        const float qsv = iqp[h * iq_head_stride];
+        // qs = 2^e, |e| <= 90: its reciprocal is the mirrored exponent field (exact); a NaN mark stays NaN
+        const float iq = qsv == qsv ? __uint_as_float(0x7f000000u - __float_as_uint(qsv)) : qsv;
         f0 = make_float4(__float_as_int(f0.x) * iq, __float_as_int(f0.y) * iq, __float_as_int(f0.z) * iq, __float_as_int(f0.w) * iq);
         f1 = make_float4(__float_as_int(f1.x) * iq, __float_as_int(f1.y) * iq, __float_as_int(f1.z) * iq, __float_as_int(f1.w) * iq);
       }

@@ -18,6 +18,13 @@
 
 namespace arachne {
 
+// max(a, b) that returns NaN if either input is NaN (fmaxf drops NaNs): one FMNMX.NAN
+__device__ __forceinline__ float max_nan(float a, float b) {
+  float d;
+  asm("max.NaN.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+
 // ---------------------------------------------------------------- generic helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
