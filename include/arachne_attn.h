@@ -104,6 +104,18 @@ enum {
  *     tau exceeds 1 still runs, and leaves a sticky mark in the plan that arachne_plan_logit_status returns.
  * Callers with learned QK-norm weights either set the flag (accepting the LSE bound above) or poll the status. */
 
+/* ABI version.  arachne_attn_params is passed by pointer and has grown between versions (version 2 appended q_stride, k_stride,
+ * v_stride), so a caller compiled against an older header would hand the library a struct that is too short.  A caller that
+ * may meet a library built from a different header checks, once, that arachne_abi_version() == ARACHNE_ABI_VERSION (the
+ * value it was compiled with) and that arachne_attn_params_size() == sizeof(arachne_attn_params); binding.py does both when
+ * it is imported and refuses to load otherwise.  The number changes whenever a struct layout, an enum value or the meaning
+ * or argument list of an existing entry point changes; new entry points alone do not change it.
+ *   1: round 1.   2: q/k/v_stride appended to arachne_attn_params.   3: arachne_workspace_bytes(plan, 1) larger (per-row
+ *   fixed-point scales), status 15, this pair of functions. */
+#define ARACHNE_ABI_VERSION 3
+int arachne_abi_version(void);
+size_t arachne_attn_params_size(void);
+
 /* Problem description.  Plain data, copied by arachne_plan_create. */
 typedef struct {
   int32_t num_seqs;       /* B                                                            */

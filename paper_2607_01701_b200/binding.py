@@ -32,7 +32,7 @@ EXPORTS = [
     "arachne_plan_create_sharded", "arachne_varlen_attn_fwd_sharded", "arachne_varlen_attn_bwd_sharded",
     "arachne_plan_create_cp", "arachne_varlen_attn_bwd_cp_partial", "arachne_cp_reduce",
     "arachne_ipc_alloc", "arachne_ipc_open", "arachne_ipc_close", "arachne_ipc_free", "arachne_plan_cta_times",
-    "arachne_plan_logit_status", "arachne_varlen_attn_fwd_noalloc",
+    "arachne_plan_logit_status", "arachne_varlen_attn_fwd_noalloc", "arachne_abi_version", "arachne_attn_params_size",
 ]
 
 
@@ -44,6 +44,16 @@ class AttnParams(ctypes.Structure):
         ("q_stride", ctypes.c_int64), ("k_stride", ctypes.c_int64), ("v_stride", ctypes.c_int64),
     ]
 
+
+ABI_VERSION = 3      # ARACHNE_ABI_VERSION of the header this file marshals for (include/arachne_attn.h)
+if not hasattr(_lib, "arachne_abi_version"):
+    raise ImportError(f"{_LIB_PATH} predates arachne_abi_version(): rebuild it (python -m paper_2607_01701_b200.build)")
+_lib.arachne_abi_version.restype = ctypes.c_int
+_lib.arachne_attn_params_size.restype = ctypes.c_size_t
+if _lib.arachne_abi_version() != ABI_VERSION or _lib.arachne_attn_params_size() != ctypes.sizeof(AttnParams):
+    # a stale .so would read q_stride / k_stride / v_stride (or whatever came later) past the end of the struct we pass
+    raise ImportError(f"{_LIB_PATH}: ABI version {_lib.arachne_abi_version()} / params size {_lib.arachne_attn_params_size()}, "
+                      f"binding.py expects {ABI_VERSION} / {ctypes.sizeof(AttnParams)}: rebuild the library")
 
 _vp, _i32p, _fp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int32), ctypes.c_void_p
 _lib.arachne_plan_create.restype = ctypes.c_int

@@ -332,6 +332,9 @@ const char* arachne_status_string(int s) {
 
 const char* arachne_last_error_message(void) { return g_last_error.c_str(); }
 
+int arachne_abi_version(void) { return ARACHNE_ABI_VERSION; }
+size_t arachne_attn_params_size(void) { return sizeof(arachne_attn_params); }
+
 int arachne_plan_create(arachne_plan** out, const arachne_attn_params* params, const int32_t* cu, const int32_t* grids) {
   return arachne_plan_create_joint(out, params, cu, grids, nullptr);
 }

@@ -25,6 +25,13 @@ def test_library_builds_and_exports_every_declared_symbol():
     from paper_2607_01701_b200 import binding
 
     assert sorted(binding.EXPORTS) == names
+    # ABI version handshake (binding.py refuses a library whose struct layout it does not marshal for)
+    with open(os.path.join(ROOT, "include", "arachne_attn.h")) as f:
+        declared = int(re.search(r"#define\s+ARACHNE_ABI_VERSION\s+(\d+)", f.read()).group(1))
+    lib.arachne_abi_version.restype = ctypes.c_int
+    lib.arachne_attn_params_size.restype = ctypes.c_size_t
+    assert lib.arachne_abi_version() == declared == binding.ABI_VERSION
+    assert lib.arachne_attn_params_size() == ctypes.sizeof(binding.AttnParams) == 72
 
 
 def test_status_strings_and_validation_without_device():
