@@ -143,6 +143,41 @@ def oracle_sample(st, tensors_cpu, budget_rows=6, heads=2):
     return flops / dt / 1e12, dt, desc, orc.num_threads()
 
 
+def self_launch_argv(argv, n_gpus, port, python=None):
+    """Command line that re-runs this bench as `n_gpus` ranks of ONE node (one process per GPU): the driver's launch contract,
+    `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py <same flags>`.
+    Pure function of its arguments (tests/test_bench_launch.py)."""
+    return [python or sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(n_gpus)}",
+            "--master-addr", "127.0.0.1", "--master-port", str(int(port)), os.path.join(ROOT, "bench.py")] + list(argv)
+
+
+def needs_self_launch(args, environ) -> bool:
+    """`python bench.py --gpus N` (N > 1) outside torchrun: nobody has started the other ranks, so this process must.
+    The reference arm never needs ranks (rank 0 alone times the oracle on the host cores)."""
+    return args.gpus > 1 and "WORLD_SIZE" not in environ and args.impl != "reference"
+
+
+def free_port() -> int:
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def self_launch(args, argv) -> int:
+    """Start the N ranks and hand their exit code back.  Fails loudly, before anything is launched, when the node has
+    fewer than N GPUs: a bench line that says n_gpus = N must have run on N devices."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus and (args.sp == "none" or have == 0):
+        # (--sp ulysses|cp may run with fewer devices than ranks: sp_bench.py then shares device 0 and says config.emulated)
+        raise SystemExit(f"bench.py --gpus {args.gpus}: this node has {have} CUDA device(s); refusing to emulate ranks on fewer GPUs")
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")            # the communicator log shows which transport (NVLS / P2P) each rank got
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    return subprocess.call(self_launch_argv(argv, args.gpus, free_port()), env=env)
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores (this tier's reference arm)."""
     from paper_2607_01701_b200 import inputs
@@ -192,9 +227,14 @@ class Env:
         self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
         if not torch.cuda.is_available():
             raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU fallback")
+        if self.local_rank >= torch.cuda.device_count():
+            raise SystemExit(f"bench.py: rank {self.rank} has no GPU of its own (LOCAL_RANK {self.local_rank}, "
+                             f"{torch.cuda.device_count()} device(s)): one process per GPU, ranks are never stacked on a device")
         torch.cuda.set_device(self.local_rank)
         self.dev = torch.device("cuda", self.local_rank)
         if self.world > 1:
+            os.environ.setdefault("NCCL_DEBUG", "INFO")          # (before the communicator exists) transport / NVLS lines of the init
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
             dist.init_process_group("nccl", device_id=self.dev)
 
     def barrier(self):
@@ -315,6 +355,9 @@ def main():
     if args.src_hash:
         print(kernel_source_hash())
         return
+    if needs_self_launch(args, os.environ):
+        # plain `python bench.py --gpus N`: become the launcher of N ranks (each re-enters main() with WORLD_SIZE set)
+        raise SystemExit(self_launch(args, sys.argv[1:]))
     if args.impl == "reference":
         return run_reference(args)
     if args.sp != "none":
@@ -323,6 +366,9 @@ def main():
 
     env = Env()
     torch = env.torch
+    if env.world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but {env.world} rank(s) are running (WORLD_SIZE): the line's n_gpus must be "
+                         f"the number of GPUs that did the work")
     from paper_2607_01701_b200 import binding
 
     # Multi-GPU (§8 e): sequences/batches are independent -> each rank owns one batch of the same
@@ -336,13 +382,13 @@ def main():
 
     # ---- e2e through the C-ABI host entry point (pinned host buffers; H2D/D2H inside the timed region)
     e2e = None
+    del r["ws"]                      # the main leg's workspace: the e2e call and the target legs bring their own
+    torch.cuda.empty_cache()
     if not args.no_e2e:
         nb = t["q"].numel() * 2
         hq, hk, hv, hdo = (x.cpu().pin_memory() for x in (t["q"], t["k"], t["v"], t["dO"]))
         ho, hdq, hdk, hdv = (torch.empty_like(hq).pin_memory() for _ in range(4))
         hlse = torch.empty((plan.H, plan.N), dtype=torch.float32).pin_memory()
-        r.pop("ws")
-        torch.cuda.empty_cache()
         binding.arachne_varlen_attn_fwd_bwd_host(plan, hq, hk, hv, hdo, ho, hlse, hdq, hdk, hdv)   # warm-up (allocates the plan's device buffers)
         env.barrier()
         n_e2e = max(5, min(args.steps, 20))
@@ -393,15 +439,18 @@ def main():
     dom = max(kernels, key=lambda k_: k_["ms"])
     dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2
     achieved = dom_flops / (dom["ms"] * 1e-3) / 1e12 if dom["ms"] > 0 else 0.0
-    # Denominator by run length (B200_PROFILING.md): a timed region under a second runs at boost clocks -> the burst figure;
-    # a longer one settles under the 1 kW power cap -> the sustained figure.
-    long_run = r["ms_total"] >= 1000.0
-    peak_kind = "bf16_tflops_sustained (timed region %.1f s >= 1 s: power-capped clocks)" % (r["ms_total"] / 1e3) if long_run \
-        else "bf16_tflops burst (timed region %.2f s < 1 s: boost clocks)" % (r["ms_total"] / 1e3)
+    # Denominator (B200_PROFILING.md): the sustained figure for a kernel timed inside a long step, the burst figure for one
+    # that runs alone at boost clocks.  Decided by the length of ONE step of the workload — a property of the workload, not of
+    # --steps (the loop of warm-up + timed steps is continuous load either way): a step of >= 100 ms keeps the GPU at its 1 kW
+    # cap for seconds even at the minimum of 3 + 1 steps.  `frac_of_burst` / `frac_of_sustained` are always both reported;
+    # `frac_of_burst` is the one north_star's targets are stated in.
+    long_run = r["ms_step"] >= 100.0
+    peak_kind = "bf16_tflops_sustained (%.0f ms / step, warm-up + timed steps back to back: power-capped clocks)" % r["ms_step"] if long_run \
+        else "bf16_tflops burst (%.2f ms / step: boost clocks)" % r["ms_step"]
     peak = peaks["sustained"] if long_run else peaks["burst"]
     traffic, traffic_src = ncu_traffic(args.workload, dom["name"])
     roofline = {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "frac_of_burst": achieved / peaks["burst"], "frac_of_sustained": achieved / peaks["sustained"],
+                "frac": achieved / peak, "frac_denominator": "sustained" if long_run else "burst", "frac_of_burst": achieved / peaks["burst"], "frac_of_sustained": achieved / peaks["sustained"],
                 "traffic": traffic, "traffic_unit": "bytes/launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
                 "traffic_source": traffic_src, "peak_source": peaks["source"] + ", " + peak_kind,
                 "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": r["calls_b"]}
