@@ -13,7 +13,7 @@ TOL_DGAMMA = 2e-2
 # moves the sequence's rel-L2 by far less than the gate, so every row is also held to
 #     |gpu_row - ref_row|_2 <= ROW_REL * max(|ref_row|_2, rms over the sequence's rows of |ref_row|_2)
 # (the rms floor keeps rows whose reference happens to be tiny — cancellation, peaked softmax — on an absolute footing).
-# Rounding alone gives 2e-3..4e-3 on the BASELINE configs (measured: profiles/r2_parity.md), so 5e-2 has > 10x headroom
+# Rounding alone gives 2e-3..4e-3 on the BASELINE configs (measured: profiles/r2_parity.md, profiles/r3_parity.md), so 5e-2 has > 10x headroom
 # and a wrong tile, tail row or scale factor (errors of order 1) fails it.
 ROW_REL = 5e-2
 

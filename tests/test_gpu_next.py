@@ -49,7 +49,7 @@ def test_dgamma_video_only_and_deterministic_mode(orc):
     st = inputs.pack([(2, 16, 20), (1, 5, 7), (5, 9, 11)], 4, 128, index=1)
     w, got, t, ref = _full(orc, st)
     print(w)
-    # the deterministic (two-pass) backward feeds the same post kernel: same dgamma gate, and bit-reproducible
+    # the deterministic (int32 fixed-point reduction) backward feeds the same post kernel: same dgamma gate, and bit-reproducible
     gq, gk = _gammas(128)
     a = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC, gamma_q=gq, gamma_k=gk, with_dgamma=True)
     b = pu.run_gpu(st, t, flags=binding.FLAG_DETERMINISTIC, gamma_q=gq, gamma_k=gk, with_dgamma=True)
@@ -94,9 +94,11 @@ def test_plan_create_joint_validation():
     binding.Plan([0, 70], [(1, 8, 8)], 2, 64, (16, 24, 24), text_lens=[6]).close()
 
 
-def _large_joint(orc, name, heads, per_seq):
-    """Full-size NEXT-2 workloads in bench.py's launch configuration: sampled query rows (always including
-    text rows) exact per row, masked-dO dK / dV / dgamma exact for all key rows."""
+def _large_joint(orc, name, heads=None, per_seq=64, head_group=6):
+    """Full-size NEXT-2 workloads in bench.py's launch configuration: SURVEY §8(c)'s sample of 64 query rows per sequence
+    (always including text rows) x ALL heads, exact per row; masked-dO dK / dV / dgamma exact for all key rows.  The oracle
+    is called one group of `head_group` heads at a time (its dK / dV come back as fp64 [N, heads, D]); dgamma is a sum over
+    heads, so each group gets its own GPU backward with dO masked in rows AND heads."""
     from paper_2607_01701_b200 import binding
     st = inputs.structure(name)
     t = inputs.make_inputs(st, device="cuda")
@@ -109,20 +111,27 @@ def _large_joint(orc, name, heads, per_seq):
         rows.update({cu[b + 1] - nt, cu[b + 1] - nt // 2, cu[b + 1] - 1, cu[b + 1] - nt - 1})
     rows = sorted(rows)
     ridx = torch.as_tensor(rows, device="cuda")
-    tc = {k: v.cpu() for k, v in t.items()}
-    q, k, v, dO = (tc[n].float().numpy() for n in ("q", "k", "v", "dO"))
-    ref = orc.attention_rows(q, k, v, cu, st["grids"], rows, dO=dO, heads=heads, gamma_q=gq, gamma_k=gk,
-                             rope_dims=st["rope_dims"], text_lens=st["text_lens"])
-    w = pu.check_rows(st, got, ref, rows)
-    dOm = torch.zeros_like(t["dO"])
-    hidx = torch.as_tensor(heads, device="cuda")
-    dOm[ridx[:, None], hidx[None, :]] = t["dO"][ridx[:, None], hidx[None, :]]      # masked in rows AND heads
+    tc = {k: v.cpu().float().numpy() for k, v in t.items()}
     g_q = torch.as_tensor(gq, device="cuda"); g_k = torch.as_tensor(gk, device="cuda")
-    dqm, dkm, dvm, dgq, dgk = binding.backward(got["plan"], t["q"], t["k"], t["v"], got["O"], got["LSE"], dOm, g_q, g_k,
-                                               with_dgamma=True)
-    torch.cuda.synchronize()
-    w.update(pu.check_masked_kv(st, {"dK": dkm, "dV": dvm}, ref))
-    w.update(pu.check_dgamma({"dGq": dgq, "dGk": dgk}, ref))
+    all_heads = list(range(st["H"])) if heads is None else list(heads)
+    w = {}
+    for g0 in range(0, len(all_heads), head_group):
+        grp = all_heads[g0:g0 + head_group]
+        ref = orc.attention_rows(tc["q"], tc["k"], tc["v"], cu, st["grids"], rows, dO=tc["dO"], heads=grp, gamma_q=gq, gamma_k=gk,
+                                 rope_dims=st["rope_dims"], text_lens=st["text_lens"])
+        wg = pu.check_rows(st, got, ref, rows)
+        dOm = torch.zeros_like(t["dO"])
+        hidx = torch.as_tensor(grp, device="cuda")
+        dOm[ridx[:, None], hidx[None, :]] = t["dO"][ridx[:, None], hidx[None, :]]      # masked in rows AND heads
+        dqm, dkm, dvm, dgq, dgk = binding.backward(got["plan"], t["q"], t["k"], t["v"], got["O"], got["LSE"], dOm, g_q, g_k,
+                                                   with_dgamma=True)
+        torch.cuda.synchronize()
+        wg.update(pu.check_masked_kv(st, {"dK": dkm, "dV": dvm}, ref))
+        wg.update(pu.check_dgamma({"dGq": dgq, "dGk": dgk}, ref))
+        for k_, v_ in wg.items():
+            w[k_] = max(w.get(k_, 0.0), v_)
+        del ref, dOm, dqm, dkm, dvm
+    w["rows_x_heads"] = (len(rows), len(all_heads))
     for b in range(len(cu) - 1):
         s, e = cu[b], cu[b + 1]
         lhs, rhs = got["dV"][s:e].float().sum(0), t["dO"][s:e].float().sum(0)
@@ -131,11 +140,11 @@ def _large_joint(orc, name, heads, per_seq):
 
 
 def test_cogvideox_shape_full_size(orc):
-    _large_joint(orc, "cogvideox", heads=[0, 14, 29], per_seq=24)
+    _large_joint(orc, "cogvideox")
 
 
 def test_joint720p_full_size(orc):
-    _large_joint(orc, "joint720p", heads=[5, 23], per_seq=24)
+    _large_joint(orc, "joint720p")
 
 
 def test_guard_bands_no_out_of_bounds_writes(orc):

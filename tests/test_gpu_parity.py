@@ -239,29 +239,46 @@ def test_deterministic_backward_keeps_precision_with_heavy_tailed_dO_and_V(orc, 
 _REF_CACHE = {}
 
 
+HEAD_GROUP = 6      # heads per oracle call: its masked-dO dK / dV come back as fp64 [N, heads, D] (1.6 GB at 262k tokens x 6 heads)
+
+
 def _large_config(orc, name, heads, per_seq=64, order="listed", flags=0):
-    """flags: 0 = fused backward (default), FLAG_DETERMINISTIC = the deterministic mode; the oracle's sampled rows are
-    computed once per (config, order) and serve both."""
+    """SURVEY §8(c)'s sample: per_seq = 64 query rows per sequence x ALL heads (heads=None), the oracle called one group of
+    HEAD_GROUP heads at a time so that host memory stays bounded.  flags: 0 = fused backward (default), FLAG_DETERMINISTIC =
+    the deterministic mode; the oracle's O / LSE / dQ rows are computed once per (config, order) and serve both (the second
+    user skips the masked-dO dK / dV comparison of the groups it finds cached: those two tensors are not kept)."""
     st = inputs.structure(name, order=order)
     t = inputs.make_inputs(st, device="cuda")
     got = pu.run_gpu(st, t, flags=flags)
     rows = inputs.sample_rows(st, per_seq=per_seq, seed=7)
     ridx = torch.as_tensor(rows, device="cuda")
-    # oracle on the sampled rows (needs all K, V of each sequence; Q, dO only at the rows)
-    key = (name, order, per_seq, None if heads is None else tuple(heads))
-    if key not in _REF_CACHE:
-        tc = {k: v.cpu() for k, v in t.items()}
-        q, k, v, dO = (tc[n].float().numpy() for n in ("q", "k", "v", "dO"))
-        _REF_CACHE[key] = orc.attention_rows(q, k, v, st["cu_seqlens"], st["grids"], rows, dO=dO, heads=heads, rope_dims=st["rope_dims"])
-    ref = _REF_CACHE[key]
-    w = pu.check_rows(st, got, ref, rows)
-    # masked-dO backward: dK, dV for ALL key rows depend only on the sampled rows
+    # masked-dO backward: dK, dV for ALL key rows depend only on the sampled rows (every head)
     dOm = torch.zeros_like(t["dO"])
     dOm[ridx] = t["dO"][ridx]
     from paper_2607_01701_b200 import binding
     dqm, dkm, dvm = binding.backward(got["plan"], t["q"], t["k"], t["v"], got["O"], got["LSE"], dOm)
     torch.cuda.synchronize()
-    w.update(pu.check_masked_kv(st, {"dK": dkm, "dV": dvm}, ref))
+    # oracle on the sampled rows (needs all K, V of each sequence; Q, dO only at the rows)
+    all_heads = list(range(st["H"])) if heads is None else list(heads)
+    tc = None
+    w = {}
+    for g0 in range(0, len(all_heads), HEAD_GROUP):
+        grp = all_heads[g0:g0 + HEAD_GROUP]
+        key = (name, order, per_seq, tuple(grp))
+        ref = _REF_CACHE.get(key)
+        if ref is None:
+            if tc is None:
+                tc = {k: v.cpu().float().numpy() for k, v in t.items()}
+            ref = orc.attention_rows(tc["q"], tc["k"], tc["v"], st["cu_seqlens"], st["grids"], rows, dO=tc["dO"], heads=grp,
+                                     rope_dims=st["rope_dims"])
+            for k_, v_ in pu.check_masked_kv(st, {"dK": dkm, "dV": dvm}, ref).items():
+                w[k_] = max(w.get(k_, 0.0), v_)
+            _REF_CACHE[key] = {k_: v_ for k_, v_ in ref.items() if k_ not in ("dK", "dV")}
+        for k_, v_ in pu.check_rows(st, got, ref, rows).items():
+            w[k_] = max(w.get(k_, 0.0), v_)
+        del ref
+    del tc
+    w["rows_x_heads"] = (len(rows), len(all_heads))
     # linearity of the backward in dO (GPU): bwd(dOm) + bwd(dO - dOm) == bwd(dO) within bf16 rounding
     rest = (t["dO"].float() - dOm.float()).to(torch.bfloat16)
     dqr, dkr, dvr = binding.backward(got["plan"], t["q"], t["k"], t["v"], got["O"], got["LSE"], rest)
@@ -292,11 +309,11 @@ def test_config1_bucket256_reversed_order(orc):
 
 
 def test_config2_mixed480p(orc):
-    _large_config(orc, "mixed480p", heads=[0, 7, 23], per_seq=32, order="shuffled")
+    _large_config(orc, "mixed480p", heads=None, per_seq=64, order="shuffled")
 
 
 def test_config3_long720p(orc):
-    st, t, got = _large_config(orc, "long720p", heads=[0, 11, 23], per_seq=32)
+    st, t, got = _large_config(orc, "long720p", heads=None, per_seq=64)
     # V == 1  =>  O == 1 at full size (softmax normalisation; bf16 rounding of P only)
     from paper_2607_01701_b200 import binding
     ones = torch.ones_like(t["v"])
@@ -305,19 +322,19 @@ def test_config3_long720p(orc):
 
 
 def test_config4_heavytail(orc):
-    _large_config(orc, "heavytail", heads=[3, 17], per_seq=16)
+    _large_config(orc, "heavytail", heads=None, per_seq=64)
 
 
 # ------------------------------------------------------------------ the deterministic backward at FULL size against the oracle
 # (sampled rows + masked-dO + invariants, the same harness and the same oracle rows as the fused default above)
 def test_config2_mixed480p_deterministic(orc):
     from paper_2607_01701_b200 import binding
-    _large_config(orc, "mixed480p", heads=[0, 7, 23], per_seq=32, order="shuffled", flags=binding.FLAG_DETERMINISTIC)
+    _large_config(orc, "mixed480p", heads=None, per_seq=64, order="shuffled", flags=binding.FLAG_DETERMINISTIC)
 
 
 def test_config3_long720p_deterministic(orc):
     from paper_2607_01701_b200 import binding
-    _large_config(orc, "long720p", heads=[0, 11, 23], per_seq=32, flags=binding.FLAG_DETERMINISTIC)
+    _large_config(orc, "long720p", heads=None, per_seq=64, flags=binding.FLAG_DETERMINISTIC)
 
 
 # ------------------------------------------------------------------ BASELINE.json configs[1] IN FULL, element by element
