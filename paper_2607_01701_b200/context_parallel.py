@@ -67,7 +67,7 @@ class ContextParallelAttention:
     forward(): barrier -> fwd_sharded -> barrier (a rank writes only its own O shard, but it READS its peers' Q, K, V
     shards: nobody may overwrite its inputs for the next layer until every rank's kernels are done with them).
     backward(): barrier -> bwd_cp_partial -> barrier -> cp_reduce -> all-reduce of the dgamma parts -> barrier.
-    The barriers are stream-ordered under NCCL (ulysses.RankSync), host barriers under gloo."""
+    The barriers are ulysses.RankSync's: host barriers by default, stream-ordered under NCCL with ARACHNE_SP_BARRIER=stream."""
 
     def __init__(self, st: dict, group=None, starts=None, transport: str = "symm"):
         import torch

@@ -5,7 +5,8 @@ The data-parallel replica mode of bench.py (weak scaling, no data-path collectiv
 peer-visible memory, the All-to-All (Ulysses) or the K/V exchange and dK/dV reduce-scatter (context parallelism) folded into the
 kernels as peer loads / stores over NVLink — `ulysses.UlyssesAttention` / `context_parallel.ContextParallelAttention`.
 
-Launch exactly like bench.py (torchrun, one rank per GPU, NCCL).  Rank barriers are stream-ordered (ulysses.RankSync); shards live
+Launch exactly like bench.py (torchrun, one rank per GPU, NCCL).  Rank barriers: host sync + group barrier by default,
+stream-ordered with ARACHNE_SP_BARRIER=stream (ulysses.RankSync; opt-in until it has run on >= 2 GPUs); shards live
 in symmetric memory.  When the node exposes fewer GPUs than ranks (this pool: one), the ranks share device 0, barriers fall
 back to gloo and shards to CUDA IPC — a functional check of the same code path, not a scaling number (`config.emulated`).
 Holds no attention arithmetic.
@@ -88,7 +89,7 @@ def run(args):
             "n_gpus": world, "steps": args.steps, "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": args.workload, "parallelism": par, "transport": transport, "emulated": emulated,
-                       "barrier": "stream-ordered NCCL all-reduce" if not emulated else "host sync + gloo barrier",
+                       "barrier": drv._sync.describe(),
                        "shard_tokens": [drv.starts[r + 1] - drv.starts[r] for r in range(world)],
                        "num_seqs": len(st["grids"]), "total_tokens": st["N"], "heads": st["H"], "head_dim": st["D"],
                        "flop_per_step": flops, "wall_ms_per_step": wall_ms / args.steps,

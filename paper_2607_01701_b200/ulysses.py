@@ -142,19 +142,41 @@ class IpcShards:
 class RankSync:
     """Orders the ranks of an SP / CP group around a kernel that reads or writes peer memory.
 
-    NCCL group: a one-element all-reduce ENQUEUED ON THE CURRENT STREAM.  It starts after this rank's earlier kernels on the
-    stream (whose remote stores are then complete) and finishes only when every rank has entered it, and later kernels on
-    the stream start after it — a device-side barrier with no host synchronisation, so the host runs ahead and the
-    launch of the next kernel overlaps the wait.  gloo group (the CPU / one-GPU tests, no device collective): host
-    synchronisation of the stream + a host barrier, as before."""
+    Two modes (constructor argument `mode`, else the environment variable ARACHNE_SP_BARRIER, else "host"):
 
-    def __init__(self, group, device):
+    "host" (default): host synchronisation of the current stream — this rank's kernels, remote stores included, have
+    completed — then a host-visible barrier of the group.  Correct by construction on any backend; it is the only mode
+    that has ever executed (gloo, in the CPU and one-GPU two-process tests) and therefore the default also under NCCL.
+
+    "stream" (opt-in, NCCL groups only): a one-element all-reduce ENQUEUED ON THE CURRENT STREAM.  It starts after this
+    rank's earlier kernels on the stream and finishes only when every rank has entered it, and later kernels on the
+    stream start after it — a device-side barrier with no host synchronisation, so the host runs ahead and the launch of
+    the next kernel overlaps the wait.  NOT VERIFIED ON HARDWARE: no run on two or more GPUs has taken place (DESIGN.md
+    §9), so neither the visibility of the peers' remote stores behind NCCL's kernel nor the ordering has been observed;
+    switch it on only together with tests/test_gpu_multiproc.py on a multi-GPU node."""
+
+    MODES = ("host", "stream")
+
+    def __init__(self, group, device, mode=None):
+        import os
+
         import torch
         import torch.distributed as dist
 
+        mode = mode or os.environ.get("ARACHNE_SP_BARRIER", "host")
+        if mode not in self.MODES:
+            raise ValueError(f"ARACHNE_SP_BARRIER / mode must be one of {self.MODES}, got {mode!r}")
         self._dist, self.group = dist, group
-        self.on_stream = dist.get_backend(group) == "nccl"
+        self.nccl = dist.get_backend(group) == "nccl"
+        if mode == "stream" and not self.nccl:
+            raise ValueError("the stream-ordered barrier needs an NCCL group (gloo has no device collective)")
+        self.on_stream = mode == "stream"
+        self.mode = mode
         self._flag = torch.zeros(1, dtype=torch.float32, device=device) if self.on_stream else None
+
+    def describe(self) -> str:
+        backend = "NCCL" if self.nccl else "gloo"
+        return f"stream-ordered {backend} all-reduce (opt-in, unverified on hardware)" if self.on_stream else f"host sync + {backend} barrier"
 
     def barrier(self):
         import torch
@@ -167,8 +189,8 @@ class RankSync:
 
     def all_reduce_sum(self, t):
         """Sum a small device tensor over the group (dgamma partials: 2 x D floats)."""
-        if self.on_stream:
-            self._dist.all_reduce(t, group=self.group)
+        if self.nccl:
+            self._dist.all_reduce(t, group=self.group)              # an ordinary device collective on the tensor's own data
             return t
         host = t.cpu()
         self._dist.all_reduce(host, group=self.group)

@@ -98,7 +98,7 @@ def test_large_gamma_rescale_path(orc):
     configs): attention is nearly one-hot, the running max grows by more than 2^8 across tiles, so the online-softmax path
     with lazy O-rescale must fire and be right.  O and every gradient are held to north_star's gates, unchanged: the
     backward recomputes S from the forward's fp16 operand images, so P = exp2(S - LSE) stays consistent however large
-    the logits are.  (LSE itself is outside the verified envelope here: test_envelope_lse_gamma3.)"""
+    the logits are.  (LSE itself is outside the verified envelope here: test_envelope_lse_gamma3_is_bounded_as_documented.)"""
     from paper_2607_01701_b200 import binding
     st, got, ref = _large_gamma_case(orc, binding.FLAG_WIDE_LOGITS)
     w = pu.check_full(st, got, ref, lse=False)
@@ -122,25 +122,34 @@ def test_envelope_status_is_raised_without_the_flag(orc):
     assert got1["plan"].logit_status() == (0, 0.0)
 
 
-@pytest.mark.xfail(strict=False, reason="documented envelope limit (arachne_attn.h 'Verified envelope', DESIGN.md R19): tau = 9; "
-                   "fp16 operand rounding bounds LSE only by 2^-10*beta; north_star's 1e-3 is claimed for tau <= 1")
-def test_envelope_lse_gamma3(orc):
+# Outside the verified envelope (tau > 1) north_star's LSE gate of 1e-3 is NOT claimed (arachne_attn.h "Verified envelope",
+# DESIGN.md R19).  What IS claimed there, and therefore tested as a pass / fail statement rather than left as an expected
+# failure: the rigorous operand-rounding bound |LSE error| <= 2^-10 * beta, beta = softmax_scale * D * |gamma_q|inf * |gamma_k|inf,
+# and the ceiling the header quotes from measurement.  If the forward ever gets a compensated S for wide logits, the
+# `> TOL` half of the first test fails and the header's paragraph has to be rewritten.
+def test_envelope_lse_gamma3_is_bounded_as_documented(orc):
     from paper_2607_01701_b200 import binding
-    st, got, ref = _large_gamma_case(orc, binding.FLAG_WIDE_LOGITS)
-    assert float(np.max(np.abs(pu.to_np(got["LSE"]) - ref["LSE"]))) <= pu.TOL["LSE_abs"]
+    st, got, ref = _large_gamma_case(orc, binding.FLAG_WIDE_LOGITS)              # gamma_q = gamma_k = 3: tau = 9
+    err = float(np.max(np.abs(pu.to_np(got["LSE"]) - ref["LSE"])))
+    beta = (1.0 / np.sqrt(128.0)) * 128.0 * 9.0
+    print("LSE max-abs at tau = 9:", err, "bound", 2.0 ** -10 * beta)
+    assert err <= 2.0 ** -10 * beta                                               # rigorous
+    assert err <= 1.5e-2                                                          # header: "9e-3 at tau = 9" (measured 9.6e-3)
+    assert err > pu.TOL["LSE_abs"], "LSE now meets 1e-3 at tau = 9: update the 'Verified envelope' text and this test"
 
 
-@pytest.mark.xfail(strict=False, reason="documented envelope limit (arachne_attn.h 'Verified envelope', DESIGN.md R19): tau = 1.6; "
-                   "measured 5e-4..1.2e-3 over seeds and heads, i.e. at the edge of north_star's 1e-3 (claimed for tau <= 1)")
-def test_envelope_lse_scale_0p2(orc):
+def test_envelope_lse_scale_0p2_is_bounded_as_documented(orc):
     from paper_2607_01701_b200 import binding
     st2 = inputs.pack([(2, 9, 11), (1, 8, 8)], 2, 64, index=2)
     t = inputs.make_inputs(st2, device="cuda")
     t = {k: (v.float() * (0.5 if k in ("q", "k") else 1.0)).to(torch.bfloat16) for k, v in t.items()}
-    got = pu.run_gpu(st2, t, flags=binding.FLAG_WIDE_LOGITS, plan_kw=dict(softmax_scale=0.2), with_bwd=False)
+    got = pu.run_gpu(st2, t, flags=binding.FLAG_WIDE_LOGITS, plan_kw=dict(softmax_scale=0.2), with_bwd=False)   # tau = 1.6
     a = _np(t)
     ref = orc.attention(a["q"], a["k"], a["v"], st2["cu_seqlens"], st2["grids"], scale=0.2)
-    assert float(np.max(np.abs(pu.to_np(got["LSE"]) - ref["LSE"]))) <= pu.TOL["LSE_abs"]
+    err = float(np.max(np.abs(pu.to_np(got["LSE"]) - ref["LSE"])))
+    print("LSE max-abs at tau = 1.6:", err, "bound", 2.0 ** -10 * 0.2 * 64.0)
+    assert err <= 2.0 ** -10 * 0.2 * 64.0                                         # rigorous: 1.25e-2
+    assert err <= 2.0e-3                                                          # header: "5e-4..1.2e-3 at tau = 1.6" (at the edge of 1e-3)
 
 
 # ------------------------------------------------------------------ block-diagonality on the GPU path

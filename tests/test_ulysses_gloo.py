@@ -133,3 +133,27 @@ def test_context_parallel_bookkeeping():
         st = cp.balanced_starts(cu, k)
         costs = [cp.rank_cost(cu, st[r], st[r + 1]) for r in range(k)]
         assert max(costs) <= sum(costs) / k + max(cu[i + 1] - cu[i] for i in range(len(cu) - 1))
+
+
+def test_rank_sync_defaults_to_the_host_barrier_and_stream_mode_is_opt_in(tmp_path, monkeypatch):
+    """ulysses.RankSync: the stream-ordered NCCL barrier has never run on two GPUs, so it must be asked for
+    (mode="stream" / ARACHNE_SP_BARRIER=stream) and is refused on a group that has no device collective."""
+    import pytest
+    import torch.distributed as dist
+
+    from paper_2607_01701_b200 import ulysses
+
+    monkeypatch.delenv("ARACHNE_SP_BARRIER", raising=False)
+    dist.init_process_group("gloo", init_method=f"file://{tmp_path}/rdzv", rank=0, world_size=1)
+    try:
+        s = ulysses.RankSync(dist.group.WORLD, "cpu")
+        assert s.mode == "host" and not s.on_stream and "host sync" in s.describe()
+        with pytest.raises(ValueError):
+            ulysses.RankSync(dist.group.WORLD, "cpu", mode="stream")          # gloo: no device collective
+        with pytest.raises(ValueError):
+            ulysses.RankSync(dist.group.WORLD, "cpu", mode="sometimes")
+        monkeypatch.setenv("ARACHNE_SP_BARRIER", "stream")
+        with pytest.raises(ValueError):
+            ulysses.RankSync(dist.group.WORLD, "cpu")                          # the variable is honoured (and refused on gloo)
+    finally:
+        dist.destroy_process_group()
