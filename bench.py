@@ -31,7 +31,7 @@ sys.path.insert(0, ROOT)
 METRIC = "varlen 3D attention fwd+bwd TFLOPS"
 UNIT = "TFLOP/s"
 WORKLOADS = ["tiny", "bucket256", "mixed480p", "long720p", "heavytail", "joint720p", "cogvideox"]
-TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")      # written by hand from an `ncu --set full` capture (profiles/r2_ncu.md)
+TRAFFIC_CSV = os.path.join("profiles", "r3_traffic.csv")      # transcribed from ncu captures (profiles/r3_ncu.md names the commands)
 
 
 def load_peaks():
@@ -57,18 +57,31 @@ def kernel_source_hash() -> str:
 
 
 def ncu_traffic(workload: str, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed capture — only if the capture
-    was taken from the kernels as they are now (source hash); otherwise None and the reason."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed captures — only those taken
+    from the kernels as they are now (source hash).  The figure moves from launch to launch (what the 126 MB L2 happens to
+    keep of the backward's ~122 MB per-head working set), so the CSV holds SEVERAL captures per kernel and this returns
+    their median with the spread: (median or None, {"min", "max", "captures", "source"} or the reason)."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
     if not os.path.exists(path):
-        return None, f"{TRAFFIC_CSV} absent"
+        return None, {"source": f"{TRAFFIC_CSV} absent"}
+    vals, stale, reports = [], None, []
     with open(path) as f:
         for row in csv.DictReader(f):
             if row["workload"] == workload and row["kernel"] in kernel:
                 if row["src_sha"] != kernel_source_hash():
-                    return None, f"{TRAFFIC_CSV}: capture predates the current kernels (src {row['src_sha']} != {kernel_source_hash()})"
-                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), f"{TRAFFIC_CSV} ({row['report']}, src {row['src_sha']})"
-    return None, f"{TRAFFIC_CSV}: no row for {workload} / {kernel}"
+                    stale = row["src_sha"]
+                    continue
+                vals.append(float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
+                if row["report"] not in reports:
+                    reports.append(row["report"])
+    if not vals:
+        why = (f"capture predates the current kernels (src {stale} != {kernel_source_hash()})" if stale
+               else f"no row for {workload} / {kernel}")
+        return None, {"source": f"{TRAFFIC_CSV}: {why}"}
+    vals.sort()
+    n = len(vals)
+    med = vals[n // 2] if n % 2 else 0.5 * (vals[n // 2 - 1] + vals[n // 2])
+    return med, {"min": vals[0], "max": vals[-1], "captures": n, "source": f"{TRAFFIC_CSV} ({'; '.join(reports)}, src {kernel_source_hash()})"}
 
 
 class ClockSampler:
@@ -319,6 +332,36 @@ def time_workload(env: Env, workload, steps, warmup, deterministic=False, order=
     return r
 
 
+def roofline_block(r, peaks):
+    """`roofline` object of one measurement (time_workload result): the dominant kernel against the tensor roofline.
+    Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); backward main kernel 10*D*H*S2 (S, dP, dV,
+    dK, dQ — the 5-GEMM backward convention), S2 = sum_b L_b^2."""
+    st = r["st"]
+    s2 = r["flops"] / (14.0 * st["D"] * st["H"])
+    alg = {"fwd_kernel": 4.0, "bwd_fused_kernel": 10.0}
+    kernels = [{"name": n, "ms": ms} for n, ms in r["kt_f"] + r["kt_b"]]
+    dom = max(kernels, key=lambda k_: k_["ms"])
+    dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2
+    achieved = dom_flops / (dom["ms"] * 1e-3) / 1e12 if dom["ms"] > 0 else 0.0
+    # Denominator (B200_PROFILING.md): the sustained figure for a kernel timed inside a long step, the burst figure for one
+    # that runs alone at boost clocks.  Decided by the length of ONE step of the workload — a property of the workload, not of
+    # --steps (the loop of warm-up + timed steps is continuous load either way): a step of >= 100 ms keeps the GPU at its 1 kW
+    # cap for seconds even at the minimum of 3 + 1 steps.  `frac_of_burst` / `frac_of_sustained` are always both reported;
+    # `frac_of_burst` is the one north_star's targets are stated in.
+    long_run = r["ms_step"] >= 100.0
+    peak_kind = "bf16_tflops_sustained (%.0f ms / step, warm-up + timed steps back to back: power-capped clocks)" % r["ms_step"] if long_run \
+        else "bf16_tflops burst (%.2f ms / step: boost clocks)" % r["ms_step"]
+    peak = peaks["sustained"] if long_run else peaks["burst"]
+    traffic, tinfo = ncu_traffic(r["workload"], dom["name"])
+    return {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "frac": achieved / peak, "frac_denominator": "sustained" if long_run else "burst", "frac_of_burst": achieved / peaks["burst"],
+            "frac_of_sustained": achieved / peaks["sustained"],
+            "traffic": traffic, "traffic_unit": "bytes/launch (ncu dram__bytes_read.sum + dram__bytes_write.sum; median of the captures)",
+            "traffic_min": tinfo.get("min"), "traffic_max": tinfo.get("max"), "traffic_captures": tinfo.get("captures", 0),
+            "traffic_source": tinfo["source"], "peak_source": peaks["source"] + ", " + peak_kind,
+            "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": r["calls_b"]}
+
+
 def target_entry(r, peaks, target_pct=None):
     e = {"tflops": round(r["value"], 1), "ms_per_step": round(r["ms_step"], 3), "steps": r["steps"],
          "pct_of_measured_bf16_burst": round(100.0 * r["value"] / r["world"] / peaks["burst"], 2),
@@ -418,6 +461,7 @@ def main():
         targets = {"long720p": target_entry(r, peaks, 60.0)}
         ht = time_workload(env, "heavytail", 5, 3); ht["world"] = env.world
         targets["heavytail"] = target_entry(ht, peaks, 50.0)
+        targets["heavytail"]["roofline"] = roofline_block(ht, peaks) if env.rank == 0 else None
         torch.cuda.empty_cache()
         det = time_workload(env, "long720p", 3, 3, deterministic=True); det["world"] = env.world
         targets["long720p_deterministic"] = target_entry(det, peaks, 60.0)
@@ -432,28 +476,7 @@ def main():
         return
 
     # ---- roofline of the dominant kernel: dense contraction -> tensor roofline.
-    # Algorithmic FLOPs per launch: fwd_kernel 4*D*H*S2 (2 GEMMs); backward main kernel
-    # 10*D*H*S2 (S, dP, dV, dK, dQ — the 5-GEMM backward convention).
-    alg = {"fwd_kernel": 4.0, "bwd_fused_kernel": 10.0}
-    kernels = [{"name": n, "ms": ms} for n, ms in r["kt_f"] + r["kt_b"]]
-    dom = max(kernels, key=lambda k_: k_["ms"])
-    dom_flops = alg.get(dom["name"], 0.0) * st["D"] * st["H"] * s2
-    achieved = dom_flops / (dom["ms"] * 1e-3) / 1e12 if dom["ms"] > 0 else 0.0
-    # Denominator (B200_PROFILING.md): the sustained figure for a kernel timed inside a long step, the burst figure for one
-    # that runs alone at boost clocks.  Decided by the length of ONE step of the workload — a property of the workload, not of
-    # --steps (the loop of warm-up + timed steps is continuous load either way): a step of >= 100 ms keeps the GPU at its 1 kW
-    # cap for seconds even at the minimum of 3 + 1 steps.  `frac_of_burst` / `frac_of_sustained` are always both reported;
-    # `frac_of_burst` is the one north_star's targets are stated in.
-    long_run = r["ms_step"] >= 100.0
-    peak_kind = "bf16_tflops_sustained (%.0f ms / step, warm-up + timed steps back to back: power-capped clocks)" % r["ms_step"] if long_run \
-        else "bf16_tflops burst (%.2f ms / step: boost clocks)" % r["ms_step"]
-    peak = peaks["sustained"] if long_run else peaks["burst"]
-    traffic, traffic_src = ncu_traffic(args.workload, dom["name"])
-    roofline = {"bound": "tensor", "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "frac_denominator": "sustained" if long_run else "burst", "frac_of_burst": achieved / peaks["burst"], "frac_of_sustained": achieved / peaks["sustained"],
-                "traffic": traffic, "traffic_unit": "bytes/launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
-                "traffic_source": traffic_src, "peak_source": peaks["source"] + ", " + peak_kind,
-                "kernel_ms": {k_["name"]: round(k_["ms"], 4) for k_ in kernels}, "calls": r["calls_b"]}
+    roofline = roofline_block(r, peaks)
 
     cpu = None
     if not args.no_cpu_baseline:
