@@ -70,7 +70,7 @@ enum {
   ARACHNE_FLAG_WIDE_LOGITS = 8,      /* the caller accepts logits outside the verified envelope (below) */
   ARACHNE_FLAG_FWD_CTA_PAIRS = 16,   /* A-B: run the forward as CTA pairs (cluster of 2, tcgen05 cta_group::2; head_dim 128
                                         only, ignored otherwise).  Correct (same parity tests) but SLOWER than the default
-                                        one-CTA kernel — 720p forward 180 vs 152 ms: the forward loop is bound by the
+                                        one-CTA kernel — 720p forward 202 vs 147 ms (profiles/r2_bench_final.md): the forward loop is bound by the
                                         softmax <-> MMA hand-off latency, which the cross-CTA hops lengthen, not by the
                                         shared-memory operand bandwidth the pairing relieves           */
   ARACHNE_FLAG_FWD_MULTICAST = 64,   /* forward as clusters of 2 CTAs that share the K^/V stream: each CTA fetches half of
